@@ -1,0 +1,149 @@
+/*
+ * ra_mppi.h — C ABI of the B200-native RA-MPPI hot path (arXiv 2209.12842).
+ *
+ * One controller iteration of Risk-Aware MPPI (Algorithm 1, :167-223;
+ * Fig. 1 :74) as hand-written sm_100a CUDA kernels.  Letters follow BASELINE.json:
+ * K control samples (paper's M), M noise realisations per sample (paper's N),
+ * T horizon steps (paper's K).
+ *
+ * Conventions for every entry point
+ *  - Pointers named d_* are DEVICE pointers on the context's device; all other
+ *    pointers are HOST pointers.  Row-major, fp32 unless stated.
+ *  - ra_mppi_step / ra_mppi_rollout_costs / ra_mppi_plant_shift only enqueue work on
+ *    `cuda_stream` (a cudaStream_t passed as void*; NULL = legacy default stream).
+ *    They do not synchronise, allocate or free, so they can be captured in a graph.
+ *  - The context owns its scratch (copies of the environment, u[T,K], S, CVaR, S~,
+ *    optional materialised noise).  The caller owns every pointer it passes; the
+ *    library keeps none of them past the enqueued work.
+ *  - Errors are returned as ra_status; nothing throws, nothing calls exit().
+ *    There is no CPU fallback: without an sm_100 device ra_mppi_create fails.
+ *  - One context per stream; not re-entrant.
+ */
+#ifndef RA_MPPI_H
+#define RA_MPPI_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ra_mppi_ctx ra_mppi_ctx; /* opaque */
+
+typedef enum {
+  RA_OK = 0,
+  RA_EINVAL = 1,       /* null pointer, size <= 0, parameter out of its domain, struct_size mismatch */
+  RA_EUNSUPPORTED = 2, /* M or T outside the supported set, device is not sm_100 */
+  RA_ECUDA = 3,        /* a CUDA call failed (see ra_mppi_last_error) */
+  RA_ENOMEM = 4        /* device allocation failed */
+} ra_status;
+
+typedef enum { RA_DYN_KINEMATIC_BICYCLE = 0, RA_DYN_SINGLE_TRACK = 1 } ra_dyn;
+typedef enum { RA_NOM_GOAL = 0, RA_NOM_ELLIPSE_TRACK = 1 } ra_nominal;
+typedef enum { RA_RISK_CIRCLES = 0, RA_RISK_COSTMAP = 1, RA_RISK_LINEAR_STATE = 2 /* test-only */ } ra_risk;
+typedef enum { RA_NOISE_GAUSSIAN = 0, RA_NOISE_UNIFORM = 1, RA_NOISE_JUMP = 2 } ra_noise_kind;
+typedef enum { RA_NOISE_FUSED = 0, RA_NOISE_MATERIALISED = 1 } ra_noise_mode;
+
+#define RA_MAX_M 512 /* realisations per sample: 1..RA_MAX_M                                  */
+#define RA_MAX_T 128 /* horizon steps: 1..RA_MAX_T                                            */
+
+/* Problem statement (8a)-(8c) PAPER.md:78-85 and Algorithm 1 "Given" :170. */
+typedef struct {
+  uint32_t struct_size; /* = sizeof(ra_mppi_config)                                           */
+  int32_t K, M, T;      /* samples, realisations, horizon (PAPER.md:247 gives 1024, 300, 30)   */
+  float dt;             /* Euler step of F (1) PAPER.md:29                                    */
+  int32_t dyn;          /* ra_dyn                                                             */
+  float dyn_p[8];       /* bicycle {wheelbase}; single-track {m,Iz,lf,lr,Cf,Cr,vx_floor}      */
+  float u_min[2], u_max[2]; /* control clamps, applied inside F and to v+                     */
+  float sigma_eps[2];   /* sqrt(diag Sigma_eps), control sampling noise (2c) PAPER.md:42      */
+  float sigma_w[6];     /* per-step additive state noise scale, w_k of (6) PAPER.md:63        */
+  float alpha;          /* CVaR confidence level in (0,1), (8b) PAPER.md:81-87                */
+  float lambda;         /* temperature of (5)/(17) PAPER.md:55,:134; > 0                      */
+  float gamma;          /* control-cost weight of (3) PAPER.md:47-49; >= 0                    */
+  float A;              /* CVaR penalty weight (14) PAPER.md:120                              */
+  float B;              /* risk sensitivity scale (18) PAPER.md:144; > 0                      */
+  float C_u;            /* CVaR bound (8b)/(15) PAPER.md:81,:124                              */
+  float eta;            /* fraction of zero-mean samples, Alg.1 l.7 PAPER.md:183,:247; [0,1)  */
+  int32_t nominal;      /* ra_nominal: q(x), phi(x) of (3)                                    */
+  float nom_p[8];       /* goal {w,gx,gy,w_phi}; track {a,b,half_w,w_lat,w_v,v_ref,w_bdry,w_phi} */
+  int32_t risk;         /* ra_risk: l(x~) of (9) PAPER.md:93                                  */
+  float risk_p[4];      /* circles {weight,margin}; costmap {weight}; linear {weight,index}   */
+  int32_t noise_kind;   /* ra_noise_kind                                       */
+  float noise_p[4];     /* jump {probability}; otherwise unused                               */
+  int32_t noise_mode;   /* ra_noise_mode: fused = Philox in registers; materialised = w[K,T,M,nx] in HBM */
+  uint64_t seed;        /* Philox4x32-10 key                                                  */
+  int32_t device;       /* CUDA device ordinal                                                */
+} ra_mppi_config;
+
+/* Environment; HOST pointers, copied at create (caller keeps ownership). */
+typedef struct {
+  const float* circles; /* [n_circles,3] x,y,r (obstacle set)                */
+  int32_t n_circles;
+  const float* costmap; /* [map_h][map_w] row-major; cell (iy,ix) centre = origin + (i+0.5)*res */
+  int32_t map_h, map_w;
+  float map_res, map_ox, map_oy;
+} ra_mppi_env;
+
+/* Allocate a controller context on cfg->device.  cfg/env: host.  *out receives the
+ * context (NULL on failure).  RA_EINVAL / RA_EUNSUPPORTED / RA_ECUDA / RA_ENOMEM.        */
+ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_mppi_ctx** out);
+
+/* One full iteration, Alg.1 l.3-31: sample u^k = v + eps^k, nominal
+ * and noisy rollouts, risk costs (9), CVaR (12), soft filter (14)-(16), weights (17),
+ * update (4).  d_x0 [n_x] current state; d_v [T,2] in: mean control v, out: v+ (clamped).
+ * `iteration` enters the Philox counter (low 28 bits).                                    */
+ra_status ra_mppi_step(ra_mppi_ctx* ctx, const float* d_x0, float* d_v, uint64_t iteration,
+                       void* cuda_stream);
+
+/* The same iteration stopped after Alg.1 l.29: per-sample costs.  Outputs (device, any may
+ * be NULL): d_S [K] nominal cost (3); d_cvar [K] CVaR_alpha of the (scaled) risk costs;
+ * d_S_tilde [K] modified cost (16); d_L [K,M] raw risk costs (9); d_xT [K,M,n_x] final
+ * noisy states; d_u [K,T,2] sampled controls u^k (unclamped).  d_v is not modified.       */
+ra_status ra_mppi_rollout_costs(ra_mppi_ctx* ctx, const float* d_x0, const float* d_v,
+                                uint64_t iteration, float* d_S, float* d_cvar, float* d_S_tilde,
+                                float* d_L, float* d_xT, float* d_u, void* cuda_stream);
+
+/* The fp64 cost scratch of the most recent step / rollout_costs on this context: d_S64 [K],
+ * d_S_tilde64 [K] (device, fp64, either may be NULL).  The weights (17) are formed from these
+ * fp64 values; the fp32 outputs of ra_mppi_rollout_costs are their roundings.               */
+ra_status ra_mppi_export_costs_f64(ra_mppi_ctx* ctx, double* d_S64, double* d_S_tilde64, void* cuda_stream);
+
+/* Weights (17)/(5) and update (4) alone, from caller-supplied costs and controls:
+ * d_S_tilde [K], d_u [K,T,2] -> d_v_plus [T,2] (clamped), d_w [K] normalised weights or
+ * NULL, d_stats [2] = {beta~, Z} or NULL.                                                 */
+ra_status ra_mppi_weights_update(ra_mppi_ctx* ctx, const float* d_S_tilde, const float* d_u,
+                                 float* d_v_plus, float* d_w, float* d_stats, void* cuda_stream);
+
+/* Closed-loop glue, Alg.1 l.32-33 on a simulated plant (BASELINE config 4):
+ * d_x0 <- F~(d_x0, v+_0, w_plant(iteration)); d_u_applied [2] <- v+_0 (or NULL);
+ * d_v[t] <- d_v[t+1], d_v[T-1] kept (warm-start shift).                                   */
+ra_status ra_mppi_plant_shift(ra_mppi_ctx* ctx, float* d_x0, float* d_v, float* d_u_applied,
+                              uint64_t iteration, void* cuda_stream);
+
+/* n_iter receding-horizon iterations (step + plant_shift) replayed from one captured CUDA
+ * graph with a device-resident iteration counter starting at `iteration0`.  d_log
+ * [n_iter, n_x+2] receives (state after the plant step, applied control) per iteration, or
+ * NULL.  h_ms [n_iter] (HOST) receives per-iteration device milliseconds (CUDA events) or
+ * NULL; when non-NULL the call synchronises the stream before returning.                  */
+ra_status ra_mppi_closed_loop(ra_mppi_ctx* ctx, float* d_x0, float* d_v, uint64_t iteration0,
+                              int32_t n_iter, float* d_log, float* h_ms, void* cuda_stream);
+
+/* Raw generator access for parity tests: out[n,4] = Philox4x32-10(ctr[n,4], key(seed)).   */
+ra_status ra_mppi_philox(ra_mppi_ctx* ctx, const uint32_t* d_ctr, int32_t n, uint32_t* d_out,
+                         void* cuda_stream);
+/* State-noise draws exactly as the rollout kernel makes them: d_w [n, n_x] for the n
+ * triples d_kmt [n,3] = (k, m, t) of stream W at `iteration`.                             */
+ra_status ra_mppi_state_noise(ra_mppi_ctx* ctx, const int32_t* d_kmt, int32_t n,
+                              uint64_t iteration, float* d_w, void* cuda_stream);
+
+/* Number of kernels one ra_mppi_step launches (for launch accounting).                   */
+int32_t ra_mppi_launches_per_step(const ra_mppi_ctx* ctx);
+/* Last error text, owned by the context (valid until the next call on it).               */
+const char* ra_mppi_last_error(const ra_mppi_ctx* ctx);
+/* Free everything the context owns.  NULL is a no-op.                                    */
+ra_status ra_mppi_destroy(ra_mppi_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RA_MPPI_H */

@@ -1,0 +1,199 @@
+"""Thin ctypes binding of libra_mppi.so (argument marshalling only).
+
+Function names mirror include/ra_mppi.h.  Every step of the path runs in the CUDA kernels
+behind the C ABI; torch is used only for device buffers and streams.  There is no CPU
+fallback: a missing library or a failing call raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libra_mppi.so")
+
+RA_OK, RA_EINVAL, RA_EUNSUPPORTED, RA_ECUDA, RA_ENOMEM = range(5)
+_STATUS = {0: "RA_OK", 1: "RA_EINVAL", 2: "RA_EUNSUPPORTED", 3: "RA_ECUDA", 4: "RA_ENOMEM"}
+
+
+class RaMppiError(RuntimeError):
+    def __init__(self, status, where, detail=""):
+        self.status = status
+        super().__init__(f"{where}: {_STATUS.get(status, status)} {detail}".strip())
+
+
+class ra_mppi_config(C.Structure):
+    _fields_ = [
+        ("struct_size", C.c_uint32),
+        ("K", C.c_int32), ("M", C.c_int32), ("T", C.c_int32),
+        ("dt", C.c_float),
+        ("dyn", C.c_int32), ("dyn_p", C.c_float * 8),
+        ("u_min", C.c_float * 2), ("u_max", C.c_float * 2),
+        ("sigma_eps", C.c_float * 2), ("sigma_w", C.c_float * 6),
+        ("alpha", C.c_float), ("lam", C.c_float), ("gamma", C.c_float),
+        ("A", C.c_float), ("B", C.c_float), ("C_u", C.c_float), ("eta", C.c_float),
+        ("nominal", C.c_int32), ("nom_p", C.c_float * 8),
+        ("risk", C.c_int32), ("risk_p", C.c_float * 4),
+        ("noise_kind", C.c_int32), ("noise_p", C.c_float * 4),
+        ("noise_mode", C.c_int32),
+        ("seed", C.c_uint64),
+        ("device", C.c_int32),
+    ]
+
+
+class ra_mppi_env(C.Structure):
+    _fields_ = [
+        ("circles", C.POINTER(C.c_float)), ("n_circles", C.c_int32),
+        ("costmap", C.POINTER(C.c_float)), ("map_h", C.c_int32), ("map_w", C.c_int32),
+        ("map_res", C.c_float), ("map_ox", C.c_float), ("map_oy", C.c_float),
+    ]
+
+
+EXPORTS = (
+    "ra_mppi_create", "ra_mppi_step", "ra_mppi_rollout_costs", "ra_mppi_weights_update",
+    "ra_mppi_export_costs_f64", "ra_mppi_plant_shift", "ra_mppi_closed_loop", "ra_mppi_philox", "ra_mppi_state_noise",
+    "ra_mppi_launches_per_step", "ra_mppi_last_error", "ra_mppi_destroy",
+)
+
+_lib = None
+
+
+def load():
+    """Load libra_mppi.so; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RaMppiError(RA_ECUDA, "load",
+                          f"{LIB_PATH} is missing: run `python -m paper_2209_12842_b200.build` "
+                          "(or __graft_entry__.build()); there is no CPU fallback")
+    L = C.CDLL(LIB_PATH)
+    vp, fp, u64, i32 = C.c_void_p, C.c_void_p, C.c_uint64, C.c_int32
+    L.ra_mppi_create.argtypes = [C.POINTER(ra_mppi_config), C.POINTER(ra_mppi_env), C.POINTER(vp)]
+    L.ra_mppi_step.argtypes = [vp, fp, fp, u64, vp]
+    L.ra_mppi_rollout_costs.argtypes = [vp, fp, fp, u64, fp, fp, fp, fp, fp, fp, vp]
+    L.ra_mppi_weights_update.argtypes = [vp, fp, fp, fp, fp, fp, vp]
+    L.ra_mppi_export_costs_f64.argtypes = [vp, vp, vp, vp]
+    L.ra_mppi_plant_shift.argtypes = [vp, fp, fp, fp, u64, vp]
+    L.ra_mppi_closed_loop.argtypes = [vp, fp, fp, u64, i32, fp, C.POINTER(C.c_float), vp]
+    L.ra_mppi_philox.argtypes = [vp, vp, i32, vp, vp]
+    L.ra_mppi_state_noise.argtypes = [vp, vp, i32, u64, fp, vp]
+    L.ra_mppi_launches_per_step.argtypes = [vp]
+    L.ra_mppi_launches_per_step.restype = i32
+    L.ra_mppi_last_error.argtypes = [vp]
+    L.ra_mppi_last_error.restype = C.c_char_p
+    L.ra_mppi_destroy.argtypes = [vp]
+    for name in EXPORTS:
+        if name not in ("ra_mppi_launches_per_step", "ra_mppi_last_error"):
+            getattr(L, name).restype = C.c_int
+    _lib = L
+    return L
+
+
+def _fill(dst, src):
+    src = list(src)
+    for i in range(len(dst)):
+        dst[i] = float(src[i]) if i < len(src) else 0.0
+
+
+def make_config(p, device=0) -> ra_mppi_config:
+    """Marshal a workloads.Problem-like record into the C struct (fp32)."""
+    c = ra_mppi_config()
+    c.struct_size = C.sizeof(ra_mppi_config)
+    c.K, c.M, c.T, c.dt = int(p.K), int(p.M), int(p.T), float(p.dt)
+    c.dyn, c.nominal, c.risk = int(p.dyn), int(p.nominal), int(p.risk)
+    _fill(c.dyn_p, p.dyn_p); _fill(c.u_min, p.u_min); _fill(c.u_max, p.u_max)
+    _fill(c.sigma_eps, p.sigma_eps); _fill(c.sigma_w, p.sigma_w)
+    c.alpha, c.lam, c.gamma = float(p.alpha), float(p.lam), float(p.gamma)
+    c.A, c.B, c.C_u, c.eta = float(p.A), float(p.B), float(p.C_u), float(p.eta)
+    _fill(c.nom_p, p.nom_p); _fill(c.risk_p, p.risk_p)
+    c.noise_kind = int(getattr(p, "noise_kind", 0))
+    _fill(c.noise_p, getattr(p, "noise_p", [0, 0, 0, 0]))
+    c.noise_mode = int(getattr(p, "noise_mode", 0))
+    c.seed = int(p.seed)
+    c.device = int(device)
+    return c
+
+
+def make_env(p):
+    """Marshal the environment; returns (struct, keepalive arrays)."""
+    e = ra_mppi_env()
+    keep = []
+    if getattr(p, "circles", None) is not None:
+        a = np.ascontiguousarray(p.circles, dtype=np.float32)
+        keep.append(a)
+        e.circles, e.n_circles = a.ctypes.data_as(C.POINTER(C.c_float)), int(a.shape[0])
+    if getattr(p, "costmap", None) is not None:
+        m = np.ascontiguousarray(p.costmap, dtype=np.float32)
+        keep.append(m)
+        e.costmap = m.ctypes.data_as(C.POINTER(C.c_float))
+        e.map_h, e.map_w = int(m.shape[0]), int(m.shape[1])
+        e.map_res, e.map_ox, e.map_oy = float(p.map_res), float(p.map_ox), float(p.map_oy)
+    return e, keep
+
+
+def _check(ctx, st, where):
+    if st != RA_OK:
+        detail = ""
+        if ctx:
+            msg = load().ra_mppi_last_error(ctx)
+            detail = msg.decode() if msg else ""
+        raise RaMppiError(st, where, detail)
+
+
+# ---- functions with the header's names (pointers are ints: tensor.data_ptr(), stream.cuda_stream)
+def ra_mppi_create(cfg: ra_mppi_config, env: ra_mppi_env):
+    ctx = C.c_void_p()
+    st = load().ra_mppi_create(C.byref(cfg), C.byref(env), C.byref(ctx))
+    _check(None, st, "ra_mppi_create")
+    return ctx
+
+
+def ra_mppi_step(ctx, d_x0, d_v, iteration, stream=0):
+    _check(ctx, load().ra_mppi_step(ctx, d_x0, d_v, int(iteration), stream), "ra_mppi_step")
+
+
+def ra_mppi_rollout_costs(ctx, d_x0, d_v, iteration, d_S=None, d_cvar=None, d_S_tilde=None, d_L=None,
+                          d_xT=None, d_u=None, stream=0):
+    _check(ctx, load().ra_mppi_rollout_costs(ctx, d_x0, d_v, int(iteration), d_S, d_cvar, d_S_tilde, d_L,
+                                             d_xT, d_u, stream), "ra_mppi_rollout_costs")
+
+
+def ra_mppi_weights_update(ctx, d_S_tilde, d_u, d_v_plus, d_w=None, d_stats=None, stream=0):
+    _check(ctx, load().ra_mppi_weights_update(ctx, d_S_tilde, d_u, d_v_plus, d_w, d_stats, stream),
+           "ra_mppi_weights_update")
+
+
+def ra_mppi_export_costs_f64(ctx, d_S64=None, d_S_tilde64=None, stream=0):
+    _check(ctx, load().ra_mppi_export_costs_f64(ctx, d_S64, d_S_tilde64, stream), "ra_mppi_export_costs_f64")
+
+
+def ra_mppi_plant_shift(ctx, d_x0, d_v, d_u_applied, iteration, stream=0):
+    _check(ctx, load().ra_mppi_plant_shift(ctx, d_x0, d_v, d_u_applied, int(iteration), stream),
+           "ra_mppi_plant_shift")
+
+
+def ra_mppi_closed_loop(ctx, d_x0, d_v, iteration0, n_iter, d_log=None, h_ms=None, stream=0):
+    ms_ptr = h_ms.ctypes.data_as(C.POINTER(C.c_float)) if h_ms is not None else None
+    _check(ctx, load().ra_mppi_closed_loop(ctx, d_x0, d_v, int(iteration0), int(n_iter), d_log, ms_ptr,
+                                           stream), "ra_mppi_closed_loop")
+
+
+def ra_mppi_philox(ctx, d_ctr, n, d_out, stream=0):
+    _check(ctx, load().ra_mppi_philox(ctx, d_ctr, int(n), d_out, stream), "ra_mppi_philox")
+
+
+def ra_mppi_state_noise(ctx, d_kmt, n, iteration, d_w, stream=0):
+    _check(ctx, load().ra_mppi_state_noise(ctx, d_kmt, int(n), int(iteration), d_w, stream),
+           "ra_mppi_state_noise")
+
+
+def ra_mppi_launches_per_step(ctx):
+    return int(load().ra_mppi_launches_per_step(ctx))
+
+
+def ra_mppi_destroy(ctx):
+    if ctx:
+        load().ra_mppi_destroy(ctx)

@@ -1,0 +1,65 @@
+"""Build libra_mppi.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a.
+
+    python -m paper_2209_12842_b200.build [--force]
+
+The rollout kernel is instantiated per (dynamics, risk) pair in separate translation units
+so they compile in parallel.  No torch headers are involved: the library is plain CUDA.
+"""
+from __future__ import annotations
+
+import os
+import subprocess
+import sys
+from concurrent.futures import ThreadPoolExecutor
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
+LIB = os.path.join(HERE, "libra_mppi.so")
+INCLUDE = os.path.join(os.path.dirname(HERE), "include")
+
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
+              "--extended-lambda", "-Xcompiler", "-fPIC", f"-I{INCLUDE}", f"-I{CSRC}"]
+
+
+def _sources():
+    return [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC))] + [os.path.join(INCLUDE, "ra_mppi.h")]
+
+
+def _jobs():
+    jobs = [(os.path.join(CSRC, "ra_mppi.cu"), os.path.join(OBJ, "ra_mppi.o"), [])]
+    for d in (0, 1):
+        for r in (0, 1, 2):
+            jobs.append((os.path.join(CSRC, "rollout_inst.cu"), os.path.join(OBJ, f"rollout_{d}_{r}.o"),
+                         [f"-DRA_INST_DYN={d}", f"-DRA_INST_RISK={r}"]))
+    return jobs
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    newest = max(os.path.getmtime(s) for s in _sources() + [os.path.abspath(__file__)])
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
+        return LIB
+    os.makedirs(OBJ, exist_ok=True)
+    extra = ["-Xptxas", "-v"] if verbose else []
+
+    def compile_one(job):
+        src, obj, defs = job
+        cmd = ["nvcc", *NVCC_FLAGS, *extra, *defs, "-c", src, "-o", obj]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError(f"nvcc failed: {' '.join(cmd)}\n{r.stdout}\n{r.stderr}")
+        return r.stderr
+
+    with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
+        logs = list(ex.map(compile_one, _jobs()))
+    if verbose:
+        with open(os.path.join(OBJ, "ptxas.log"), "w") as f:
+            f.write("\n".join(logs))
+    objs = [j[1] for j in _jobs()]
+    cmd = ["nvcc", "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB, *objs, "-lcudart"]
+    subprocess.run(cmd, check=True)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

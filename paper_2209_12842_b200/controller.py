@@ -1,0 +1,105 @@
+"""RaMppi: a convenience holder around the C-ABI calls (torch tensors in, torch tensors out).
+
+Allocation and pointer marshalling only -- all arithmetic runs in libra_mppi.so.
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from . import binding as B
+
+
+class RaMppi:
+    def __init__(self, problem, device: int = 0):
+        if not torch.cuda.is_available():
+            raise B.RaMppiError(B.RA_ECUDA, "RaMppi", "no CUDA device: this package has no CPU fallback")
+        self.problem = problem
+        self.device = torch.device("cuda", device)
+        self.cfg = B.make_config(problem, device)
+        self.env, self._keep = B.make_env(problem)
+        self.ctx = B.ra_mppi_create(self.cfg, self.env)
+        self.K, self.M, self.T, self.nx = problem.K, problem.M, problem.T, problem.nx
+
+    def close(self):
+        if getattr(self, "ctx", None):
+            B.ra_mppi_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- helpers
+    def tensor(self, a, dtype=torch.float32):
+        return torch.as_tensor(np.ascontiguousarray(a), dtype=dtype).to(self.device).contiguous()
+
+    @staticmethod
+    def _stream():
+        return torch.cuda.current_stream().cuda_stream
+
+    # ---- the C-ABI calls
+    def step(self, d_x0: torch.Tensor, d_v: torch.Tensor, iteration: int = 0):
+        """In place: d_v [T,2] <- v+ (ra_mppi_step)."""
+        assert d_x0.is_cuda and d_v.is_cuda and d_v.dtype == torch.float32 and d_v.is_contiguous()
+        B.ra_mppi_step(self.ctx, d_x0.data_ptr(), d_v.data_ptr(), iteration, self._stream())
+        return d_v
+
+    def rollout_costs(self, d_x0, d_v, iteration: int = 0, want_L=True, want_xT=True, want_u=True):
+        f = dict(device=self.device, dtype=torch.float32)
+        out = dict(S=torch.empty(self.K, **f), cvar=torch.empty(self.K, **f), S_tilde=torch.empty(self.K, **f))
+        out["L"] = torch.empty(self.K, self.M, **f) if want_L else None
+        out["xT"] = torch.empty(self.K, self.M, self.nx, **f) if want_xT else None
+        out["u"] = torch.empty(self.K, self.T, 2, **f) if want_u else None
+        ptr = lambda t: t.data_ptr() if t is not None else None
+        B.ra_mppi_rollout_costs(self.ctx, d_x0.data_ptr(), d_v.data_ptr(), iteration, ptr(out["S"]),
+                                ptr(out["cvar"]), ptr(out["S_tilde"]), ptr(out["L"]), ptr(out["xT"]),
+                                ptr(out["u"]), self._stream())
+        return out
+
+    def costs_f64(self):
+        """fp64 S and S~ of the most recent step / rollout_costs."""
+        S = torch.empty(self.K, device=self.device, dtype=torch.float64)
+        St = torch.empty(self.K, device=self.device, dtype=torch.float64)
+        B.ra_mppi_export_costs_f64(self.ctx, S.data_ptr(), St.data_ptr(), self._stream())
+        return S, St
+
+    def weights_update(self, d_S_tilde, d_u):
+        f = dict(device=self.device, dtype=torch.float32)
+        v_plus, w, stats = torch.empty(self.T, 2, **f), torch.empty(self.K, **f), torch.empty(2, **f)
+        B.ra_mppi_weights_update(self.ctx, d_S_tilde.data_ptr(), d_u.data_ptr(), v_plus.data_ptr(),
+                                 w.data_ptr(), stats.data_ptr(), self._stream())
+        return dict(v_plus=v_plus, w=w, stats=stats)
+
+    def plant_shift(self, d_x0, d_v, iteration: int):
+        u = torch.empty(2, device=self.device, dtype=torch.float32)
+        B.ra_mppi_plant_shift(self.ctx, d_x0.data_ptr(), d_v.data_ptr(), u.data_ptr(), iteration, self._stream())
+        return u
+
+    def closed_loop(self, d_x0, d_v, iteration0: int, n_iter: int, log=True, timing=True):
+        d_log = torch.zeros(n_iter, self.nx + 2, device=self.device, dtype=torch.float32) if log else None
+        h_ms = np.zeros(n_iter, dtype=np.float32) if timing else None
+        B.ra_mppi_closed_loop(self.ctx, d_x0.data_ptr(), d_v.data_ptr(), iteration0, n_iter,
+                              d_log.data_ptr() if log else None, h_ms, self._stream())
+        return d_log, h_ms
+
+    def philox(self, ctr: torch.Tensor):
+        assert ctr.dtype == torch.int64 or ctr.dtype == torch.uint32 or ctr.dtype == torch.int32
+        c = ctr.to(torch.int64).to(self.device)
+        c32 = (c & 0xFFFFFFFF).to(torch.int64)
+        packed = torch.where(c32 >= 2**31, c32 - 2**32, c32).to(torch.int32).contiguous()
+        out = torch.empty_like(packed)
+        B.ra_mppi_philox(self.ctx, packed.data_ptr(), packed.shape[0], out.data_ptr(), self._stream())
+        return out.to(torch.int64) & 0xFFFFFFFF
+
+    def state_noise(self, kmt: torch.Tensor, iteration: int = 0):
+        kmt = kmt.to(self.device, torch.int32).contiguous()
+        w = torch.empty(kmt.shape[0], self.nx, device=self.device, dtype=torch.float32)
+        B.ra_mppi_state_noise(self.ctx, kmt.data_ptr(), kmt.shape[0], iteration, w.data_ptr(), self._stream())
+        return w
+
+    @property
+    def launches_per_step(self):
+        return B.ra_mppi_launches_per_step(self.ctx)

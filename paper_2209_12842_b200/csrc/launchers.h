@@ -1,0 +1,27 @@
+// Host-side launch entry points of the per-(dynamics, risk) rollout translation units.
+// rollout_inst.cu is compiled once per (RA_INST_DYN, RA_INST_RISK) pair so the template
+// instantiations build in parallel; ra_mppi.cu picks the launcher at ra_mppi_create.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "ra_params.cuh"
+
+namespace ra {
+
+// noise: NOISE_GAUSSIAN / NOISE_UNIFORM / NOISE_JUMP / 3 (materialised); rc in {1,2,4};
+// half: two samples per warp (M <= 16, rc must be 1).
+using RolloutLaunchFn = cudaError_t (*)(const Params& p, int noise, int rc, bool half, const float* d_x0,
+                                        float* d_L, float* d_xT, cudaStream_t stream);
+
+#define RA_DECLARE_ROLLOUT(D, R) \
+  cudaError_t launch_rollout_##D##_##R(const Params& p, int noise, int rc, bool half, const float* d_x0, \
+                                       float* d_L, float* d_xT, cudaStream_t stream);
+RA_DECLARE_ROLLOUT(0, 0)
+RA_DECLARE_ROLLOUT(0, 1)
+RA_DECLARE_ROLLOUT(0, 2)
+RA_DECLARE_ROLLOUT(1, 0)
+RA_DECLARE_ROLLOUT(1, 1)
+RA_DECLARE_ROLLOUT(1, 2)
+#undef RA_DECLARE_ROLLOUT
+
+}  // namespace ra

@@ -1,0 +1,145 @@
+// Vehicle models and cost functions of the BASELINE configs (device side, fp32).
+// Dynamics: x_{t+1} = F(x_t, u_t) (1) PAPER.md:29, forward Euler with derivatives at the
+// pre-step state; controls clamped inside F.  Positions are integrated in a frame centred at
+// x0's position (exactly translation-invariant models), which keeps fp32 rounding of the
+// Euler sums at the scale of the travelled distance instead of the world coordinate.
+#pragma once
+#include "ra_params.cuh"
+
+namespace ra {
+
+__device__ __forceinline__ float clampf(float x, float lo, float hi) { return fminf(fmaxf(x, lo), hi); }
+
+// sin/cos by three-term Cody-Waite reduction to [-pi/4, pi/4] and FMA-pipe polynomials.
+// Valid (<= 2 ulp) for |x| < ~6000 rad; yaw angles here stay within a few turns.
+__device__ __forceinline__ void sincos_cw(float x, float& s, float& c) {
+  const float j = rintf(x * 0.636619747f);
+  float r = fmaf(j, -1.5703125f, x);
+  r = fmaf(j, -4.837512969970703e-4f, r);
+  r = fmaf(j, -7.549790126404332e-8f, r);
+  const float r2 = r * r;
+  float ps = 2.75573192e-6f;            //  1/9!
+  ps = fmaf(ps, r2, -1.98412698e-4f);   // -1/7!
+  ps = fmaf(ps, r2, 8.33333333e-3f);    //  1/5!
+  ps = fmaf(ps, r2, -1.66666667e-1f);   // -1/3!
+  const float sr = fmaf(r * r2, ps, r);
+  float pc = 2.48015873e-5f;            //  1/8!
+  pc = fmaf(pc, r2, -1.38888889e-3f);   // -1/6!
+  pc = fmaf(pc, r2, 4.16666667e-2f);    //  1/4!
+  pc = fmaf(pc, r2, -0.5f);
+  const float cr = fmaf(pc, r2, 1.0f);
+  const int q = (int)j;
+  const float cs = (q & 1) ? -sr : cr;
+  const float sn = (q & 1) ? cr : sr;
+  c = (q & 2) ? -cs : cs;
+  s = (q & 2) ? -sn : sn;
+}
+
+// Control effects: everything F needs from u^k_t that is the same for all M realisations,
+// computed once per (k,t) by the sampling kernel.
+//   bicycle:       (dt tan(delta_c)/L, dt a_c, -, -)
+//   single-track:  (delta_c, Fx_c, sin delta_c, cos delta_c)
+template <int DYN>
+__device__ __forceinline__ float4 control_effect(const Params& p, float u0, float u1) {
+  const float d = clampf(u0, p.u_min[0], p.u_max[0]);
+  const float a = clampf(u1, p.u_min[1], p.u_max[1]);
+  if constexpr (DYN == DYN_BICYCLE) {
+    return make_float4(p.dt * tanf(d) / p.dyn_p[0], p.dt * a, 0.0f, 0.0f);
+  } else {
+    float s, c;
+    sincos_cw(d, s, c);
+    return make_float4(d, a, s, c);
+  }
+}
+
+template <int DYN> struct StateDim { static constexpr int value = DYN == DYN_SINGLE_TRACK ? 6 : 4; };
+
+// One Euler step in the x0-centred frame.  x: (X,Y,psi,v) or (X,Y,psi,vx,vy,r).
+template <int DYN>
+__device__ __forceinline__ void dynamics_step(const Params& p, float (&x)[StateDim<DYN>::value],
+                                              const float4 ce) {
+  float s, c;
+  sincos_cw(x[2], s, c);
+  if constexpr (DYN == DYN_BICYCLE) {
+    const float dv = p.dt * x[3];
+    x[0] = fmaf(dv, c, x[0]);
+    x[1] = fmaf(dv, s, x[1]);
+    x[2] = fmaf(x[3], ce.x, x[2]);
+    x[3] = x[3] + ce.y;
+  } else {
+    const float m_inv = 1.0f / p.dyn_p[0], iz_inv = 1.0f / p.dyn_p[1];
+    const float lf = p.dyn_p[2], lr = p.dyn_p[3], Cf = p.dyn_p[4], Cr = p.dyn_p[5];
+    const float vx = x[3], vy = x[4], r = x[5];
+    const float alpha_f = ce.x - atan2f(fmaf(lf, r, vy), vx);
+    const float alpha_r = -atan2f(fmaf(-lr, r, vy), vx);
+    const float Fyf = Cf * alpha_f, Fyr = Cr * alpha_r;
+    const float vx_dot = fmaf(vy, r, (ce.y - Fyf * ce.z) * m_inv);
+    const float vy_dot = fmaf(-vx, r, fmaf(Fyf, ce.w, Fyr) * m_inv);
+    const float r_dot = (lf * Fyf * ce.w - lr * Fyr) * iz_inv;
+    const float X_dot = vx * c - vy * s;
+    const float Y_dot = fmaf(vx, s, vy * c);
+    x[0] = fmaf(p.dt, X_dot, x[0]);
+    x[1] = fmaf(p.dt, Y_dot, x[1]);
+    x[2] = fmaf(p.dt, r, x[2]);
+    x[3] = fmaxf(fmaf(p.dt, vx_dot, vx), p.dyn_p[6]);
+    x[4] = fmaf(p.dt, vy_dot, vy);
+    x[5] = fmaf(p.dt, r_dot, r);
+  }
+}
+
+// Nominal running cost q(x) (state part; "arbitrary form" PAPER.md:45) at absolute position
+// (X, Y) = frame origin + x[0..1]; v = x[3].  BASELINE configs 0/3 (goal) and 1/2/4 (track).
+template <int NOM>
+__device__ __forceinline__ float nominal_cost(const Params& p, float Xabs, float Yabs, float v) {
+  if constexpr (NOM == NOM_GOAL) {
+    const float dx = Xabs - p.nom_p[1], dy = Yabs - p.nom_p[2];
+    return p.nom_p[0] * fmaf(dx, dx, dy * dy);
+  } else {
+    const float a = p.nom_p[0], b = p.nom_p[1];
+    const float xa = Xabs / a, yb = Yabs / b;
+    const float f = fmaf(xa, xa, fmaf(yb, yb, -1.0f));
+    const float gx = xa / a, gy = yb / b;
+    const float g = sqrtf(fmaf(gx, gx, gy * gy));
+    const float e = f / (2.0f * fmaxf(g, 1e-12f));   // first-order signed offset, + outside
+    const float over = fmaxf(0.0f, fabsf(e) - p.nom_p[2]);
+    const float dv = v - p.nom_p[5];
+    return fmaf(p.nom_p[3] * e, e, fmaf(p.nom_p[4] * dv, dv, p.nom_p[6] * over * over));
+  }
+}
+
+// Bilinear costmap lookup between cell centres with clamp-to-edge.  The grid coordinate is
+// split as (integer bias) + (fractional bias + X_rel / res) so the fraction keeps full
+// precision wherever the vehicle is on the map.
+struct MapFrame {
+  float bxf, byf;  // fractional part of (x0 - origin)/res - 1/2
+  int bxi, byi;    // integer part
+};
+
+__device__ __forceinline__ MapFrame make_map_frame(const Params& p, float x0X, float x0Y) {
+  MapFrame f;
+  const float bx = fmaf(x0X - p.map_ox, p.map_inv_res, -0.5f);
+  const float by = fmaf(x0Y - p.map_oy, p.map_inv_res, -0.5f);
+  const float fx = floorf(bx), fy = floorf(by);
+  f.bxf = bx - fx; f.byf = by - fy;
+  f.bxi = (int)fx; f.byi = (int)fy;
+  return f;
+}
+
+__device__ __forceinline__ float bilinear(const Params& p, const MapFrame& f, float Xrel, float Yrel) {
+  const float gx = fmaf(Xrel, p.map_inv_res, f.bxf);
+  const float gy = fmaf(Yrel, p.map_inv_res, f.byf);
+  const float flx = floorf(gx), fly = floorf(gy);
+  const float tx = gx - flx, ty = gy - fly;
+  const int ix = (int)flx + f.bxi, iy = (int)fly + f.byi;
+  const int ix0 = min(max(ix, 0), p.map_w - 1), ix1 = min(max(ix + 1, 0), p.map_w - 1);
+  const int iy0 = min(max(iy, 0), p.map_h - 1), iy1 = min(max(iy + 1, 0), p.map_h - 1);
+  const float* r0 = p.costmap + (size_t)iy0 * p.map_w;
+  const float* r1 = p.costmap + (size_t)iy1 * p.map_w;
+  const float c00 = __ldg(r0 + ix0), c01 = __ldg(r0 + ix1);
+  const float c10 = __ldg(r1 + ix0), c11 = __ldg(r1 + ix1);
+  const float top = fmaf(tx, c01 - c00, c00);
+  const float bot = fmaf(tx, c11 - c10, c10);
+  return fmaf(ty, bot - top, top);
+}
+
+}  // namespace ra

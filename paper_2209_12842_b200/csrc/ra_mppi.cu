@@ -1,0 +1,477 @@
+// C ABI of the B200-native RA-MPPI hot path (see include/ra_mppi.h).
+// Host side: context, validation, kernel dispatch, CUDA-graph closed loop.
+#include "../../include/ra_mppi.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "launchers.h"
+#include "rollout.cuh"
+#include "update.cuh"
+
+using namespace ra;
+
+struct ra_mppi_ctx {
+  ra_mppi_config cfg{};
+  Params p{};
+  int rc = 1;          // realisations interleaved per lane in the rollout kernel
+  bool half = false;   // two samples per warp
+  int noise_variant = 0;
+  RolloutLaunchFn rollout = nullptr;
+  // device allocations owned by the context
+  float4* d_circles = nullptr;
+  float* d_costmap = nullptr;
+  float2* d_u_raw = nullptr;
+  float4* d_ce = nullptr;
+  double* d_S = nullptr;
+  float* d_cvar = nullptr;
+  double* d_S_tilde = nullptr;
+  float* d_w_mat = nullptr;
+  LoopState* d_loop = nullptr;
+  // closed-loop graph cache
+  cudaGraphExec_t graph_exec = nullptr;
+  float *g_x0 = nullptr, *g_v = nullptr, *g_log = nullptr;
+  std::string err;
+};
+
+namespace {
+
+ra_status fail(ra_mppi_ctx* c, ra_status s, const std::string& msg) {
+  if (c) c->err = msg;
+  return s;
+}
+
+ra_status cuda_fail(ra_mppi_ctx* c, cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return RA_OK;
+  const ra_status s = (e == cudaErrorMemoryAllocation) ? RA_ENOMEM : RA_ECUDA;
+  return fail(c, s, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define RA_CUDA(ctx, call)                                  \
+  do {                                                      \
+    cudaError_t e__ = (call);                               \
+    if (e__ != cudaSuccess) return cuda_fail(ctx, e__, #call); \
+  } while (0)
+
+bool finite_nonneg(float x) { return std::isfinite(x) && x >= 0.0f; }
+
+// ceil((1-alpha) M) (G11), clamped to [1, M].  alpha arrives as fp32, so the guard
+// against representation error is 1e-6 M (0.7f -> (1-alpha) 10 = 3.0000001 must count 3).
+int tail_count(double alpha, int M) {
+  int k = (int)std::ceil((1.0 - alpha) * (double)M - 1e-6 * (double)M);
+  return k < 1 ? 1 : (k > M ? M : k);
+}
+
+const char* validate(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_status* st) {
+  *st = RA_EINVAL;
+  if (cfg->struct_size != sizeof(ra_mppi_config)) return "struct_size mismatch";
+  if (cfg->K <= 0 || cfg->M <= 0 || cfg->T <= 0) return "K, M, T must be positive";
+  if (!(cfg->dt > 0.0f) || !std::isfinite(cfg->dt)) return "dt must be positive";
+  if (cfg->dyn != RA_DYN_KINEMATIC_BICYCLE && cfg->dyn != RA_DYN_SINGLE_TRACK) return "unknown dyn";
+  if (cfg->nominal != RA_NOM_GOAL && cfg->nominal != RA_NOM_ELLIPSE_TRACK) return "unknown nominal cost";
+  if (cfg->risk < RA_RISK_CIRCLES || cfg->risk > RA_RISK_LINEAR_STATE) return "unknown risk cost";
+  if (cfg->noise_kind < RA_NOISE_GAUSSIAN || cfg->noise_kind > RA_NOISE_JUMP) return "unknown noise kind";
+  if (cfg->noise_mode != RA_NOISE_FUSED && cfg->noise_mode != RA_NOISE_MATERIALISED) return "unknown noise mode";
+  if (!(cfg->alpha > 0.0f && cfg->alpha < 1.0f)) return "alpha must be in (0,1) (PAPER.md:87)";
+  if (!(cfg->lambda > 0.0f) || !std::isfinite(cfg->lambda)) return "lambda must be positive";
+  if (!finite_nonneg(cfg->gamma)) return "gamma must be >= 0";
+  if (!(cfg->eta >= 0.0f && cfg->eta < 1.0f)) return "eta must be in [0,1)";
+  if (!(cfg->B > 0.0f) || !std::isfinite(cfg->B)) return "B must be positive";
+  if (!std::isfinite(cfg->A) || !std::isfinite(cfg->C_u)) return "A, C_u must be finite";
+  for (int i = 0; i < 2; ++i) {
+    if (!finite_nonneg(cfg->sigma_eps[i])) return "sigma_eps must be >= 0";
+    if (!(cfg->u_min[i] <= cfg->u_max[i])) return "u_min must be <= u_max";
+  }
+  for (int i = 0; i < 6; ++i)
+    if (!finite_nonneg(cfg->sigma_w[i])) return "sigma_w must be >= 0";
+  if (cfg->dyn == RA_DYN_KINEMATIC_BICYCLE && !(cfg->dyn_p[0] > 0.0f)) return "wheelbase must be positive";
+  if (cfg->dyn == RA_DYN_SINGLE_TRACK && (!(cfg->dyn_p[0] > 0.0f) || !(cfg->dyn_p[1] > 0.0f) || !(cfg->dyn_p[6] > 0.0f)))
+    return "single-track needs m, Iz, vx_floor > 0";
+  if (cfg->nominal == RA_NOM_ELLIPSE_TRACK && (!(cfg->nom_p[0] > 0.0f) || !(cfg->nom_p[1] > 0.0f)))
+    return "track semi-axes must be positive";
+  if (cfg->risk == RA_RISK_CIRCLES) {
+    if (!env || env->n_circles < 0 || (env->n_circles > 0 && !env->circles)) return "circle risk needs env->circles";
+  }
+  if (cfg->risk == RA_RISK_COSTMAP) {
+    if (!env || !env->costmap || env->map_h < 1 || env->map_w < 1 || !(env->map_res > 0.0f))
+      return "costmap risk needs env->costmap";
+  }
+  if (cfg->risk == RA_RISK_LINEAR_STATE) {
+    const int nx = cfg->dyn == RA_DYN_SINGLE_TRACK ? 6 : 4;
+    if (!(cfg->risk_p[1] >= 0.0f && cfg->risk_p[1] < (float)nx)) return "linear risk index out of range";
+  }
+  if (cfg->noise_kind == RA_NOISE_JUMP && !(cfg->noise_p[0] >= 0.0f && cfg->noise_p[0] <= 1.0f))
+    return "jump probability must be in [0,1]";
+  *st = RA_EUNSUPPORTED;
+  if (cfg->M > RA_MAX_M) return "M above RA_MAX_M";
+  if (cfg->T > RA_MAX_T) return "T above RA_MAX_T";
+  if (cfg->risk == RA_RISK_CIRCLES && env->n_circles > kMaxCirclesSmem) return "too many circles";
+  *st = RA_OK;
+  return nullptr;
+}
+
+RolloutLaunchFn pick_rollout(int dyn, int risk) {
+  static const RolloutLaunchFn table[2][3] = {
+      {launch_rollout_0_0, launch_rollout_0_1, launch_rollout_0_2},
+      {launch_rollout_1_0, launch_rollout_1_1, launch_rollout_1_2}};
+  return table[dyn][risk];
+}
+
+void philox_round_keys(uint64_t seed, uint32_t rk[20]) {
+  uint32_t k0 = (uint32_t)(seed & 0xFFFFFFFFull), k1 = (uint32_t)(seed >> 32);
+  for (int r = 0; r < 10; ++r) {
+    rk[2 * r] = k0; rk[2 * r + 1] = k1;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+}
+
+template <typename T>
+cudaError_t dev_alloc(T** p, size_t n) { return cudaMalloc(reinterpret_cast<void**>(p), n * sizeof(T)); }
+
+}  // namespace
+
+extern "C" {
+
+ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_mppi_ctx** out) {
+  if (!out) return RA_EINVAL;
+  *out = nullptr;
+  if (!cfg) return RA_EINVAL;
+  ra_status st;
+  if (const char* why = validate(cfg, env, &st)) {
+    std::fprintf(stderr, "ra_mppi_create: %s\n", why);
+    return st;
+  }
+  int n_dev = 0;
+  if (cudaGetDeviceCount(&n_dev) != cudaSuccess || cfg->device < 0 || cfg->device >= n_dev) {
+    std::fprintf(stderr, "ra_mppi_create: no CUDA device %d (this library has no CPU fallback)\n", cfg->device);
+    return RA_ECUDA;
+  }
+  cudaDeviceProp prop{};
+  if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess) return RA_ECUDA;
+  if (prop.major != 10) {
+    std::fprintf(stderr, "ra_mppi_create: device is sm_%d%d, built for sm_100a only\n", prop.major, prop.minor);
+    return RA_EUNSUPPORTED;
+  }
+  ra_mppi_ctx* c = new (std::nothrow) ra_mppi_ctx();
+  if (!c) return RA_ENOMEM;
+  c->cfg = *cfg;
+  auto bail = [&](ra_status s) { ra_mppi_destroy(c); return s; };
+  if (cudaSetDevice(cfg->device) != cudaSuccess) return bail(RA_ECUDA);
+
+  Params& p = c->p;
+  p.K = cfg->K; p.M = cfg->M; p.T = cfg->T;
+  p.K0 = (int)std::ceil((1.0 - (double)cfg->eta) * (double)cfg->K - 1e-9);
+  p.k_tail = tail_count((double)cfg->alpha, cfg->M);
+  c->half = cfg->M <= 16;
+  p.G = c->half ? 16 : 32;
+  p.R_total = (cfg->M + p.G - 1) / p.G;
+  c->rc = c->half ? 1 : (p.R_total % 4 == 0 ? 4 : (p.R_total % 2 == 0 ? 2 : 1));
+  p.nx = cfg->dyn == RA_DYN_SINGLE_TRACK ? 6 : 4;
+  p.dt = cfg->dt;
+  std::memcpy(p.dyn_p, cfg->dyn_p, sizeof p.dyn_p);
+  std::memcpy(p.nom_p, cfg->nom_p, sizeof p.nom_p);
+  std::memcpy(p.risk_p, cfg->risk_p, sizeof p.risk_p);
+  std::memcpy(p.noise_p, cfg->noise_p, sizeof p.noise_p);
+  std::memcpy(p.sigma_w, cfg->sigma_w, sizeof p.sigma_w);
+  for (int i = 0; i < 2; ++i) {
+    p.u_min[i] = cfg->u_min[i]; p.u_max[i] = cfg->u_max[i];
+    p.sigma_eps[i] = cfg->sigma_eps[i];
+    // gamma v^T Sigma^-1 u (3) PAPER.md:47; a component with sigma_eps = 0 is not sampled and is skipped
+    p.ctrl_w[i] = cfg->sigma_eps[i] > 0.0f
+                      ? (float)((double)cfg->gamma / ((double)cfg->sigma_eps[i] * (double)cfg->sigma_eps[i]))
+                      : 0.0f;
+  }
+  p.neg_log2e_over_lambda = (float)(-1.4426950408889634 / (double)cfg->lambda);
+  p.A = cfg->A; p.B = cfg->B; p.C_u = cfg->C_u;
+  const int J = (p.nx + 3) / 4;
+  p.Jc = cfg->noise_kind == RA_NOISE_JUMP ? J + 1 : J;
+  philox_round_keys(cfg->seed, p.rk);
+  c->noise_variant = cfg->noise_mode == RA_NOISE_MATERIALISED ? NOISE_MATERIALISED : cfg->noise_kind;
+  c->rollout = pick_rollout(cfg->dyn, cfg->risk);
+
+  // environment copies
+  if (cfg->risk == RA_RISK_CIRCLES) {
+    p.n_circles = env->n_circles;
+    std::vector<float4> h((size_t)std::max(env->n_circles, 1));
+    for (int i = 0; i < env->n_circles; ++i)
+      h[i] = make_float4(env->circles[3 * i], env->circles[3 * i + 1], env->circles[3 * i + 2] + cfg->risk_p[1], 0.0f);
+    if (cuda_fail(c, dev_alloc(&c->d_circles, h.size()), "alloc circles")) return bail(RA_ENOMEM);
+    if (cudaMemcpy(c->d_circles, h.data(), h.size() * sizeof(float4), cudaMemcpyHostToDevice) != cudaSuccess)
+      return bail(RA_ECUDA);
+    p.circles = c->d_circles;
+  }
+  if (cfg->risk == RA_RISK_COSTMAP) {
+    const size_t n = (size_t)env->map_h * env->map_w;
+    if (cuda_fail(c, dev_alloc(&c->d_costmap, n), "alloc costmap")) return bail(RA_ENOMEM);
+    if (cudaMemcpy(c->d_costmap, env->costmap, n * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess)
+      return bail(RA_ECUDA);
+    p.costmap = c->d_costmap;
+    p.map_h = env->map_h; p.map_w = env->map_w;
+    p.map_inv_res = (float)(1.0 / (double)env->map_res);
+    p.map_ox = env->map_ox; p.map_oy = env->map_oy;
+  }
+  // scratch
+  const size_t KT = (size_t)cfg->K * cfg->T;
+  if (dev_alloc(&c->d_u_raw, KT) != cudaSuccess || dev_alloc(&c->d_ce, KT) != cudaSuccess ||
+      dev_alloc(&c->d_S, (size_t)cfg->K) != cudaSuccess || dev_alloc(&c->d_cvar, (size_t)cfg->K) != cudaSuccess ||
+      dev_alloc(&c->d_S_tilde, (size_t)cfg->K) != cudaSuccess || dev_alloc(&c->d_loop, 1) != cudaSuccess)
+    return bail(RA_ENOMEM);
+  p.u_raw = c->d_u_raw; p.ce = c->d_ce; p.S = c->d_S; p.cvar = c->d_cvar; p.S_tilde = c->d_S_tilde;
+  if (cudaMemset(c->d_loop, 0, sizeof(LoopState)) != cudaSuccess) return bail(RA_ECUDA);
+  p.M_pad = p.R_total * p.G;
+  if (cfg->noise_mode == RA_NOISE_MATERIALISED) {
+    const size_t n = KT * (size_t)p.nx * (size_t)p.M_pad;
+    if (dev_alloc(&c->d_w_mat, n) != cudaSuccess) return bail(RA_ENOMEM);
+    p.w_mat = c->d_w_mat;
+  }
+  p.d_iter = nullptr; p.iter_imm = 0;
+  *out = c;
+  return RA_OK;
+}
+
+ra_status ra_mppi_destroy(ra_mppi_ctx* c) {
+  if (!c) return RA_OK;
+  cudaSetDevice(c->cfg.device);
+  if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+  cudaFree(c->d_circles); cudaFree(c->d_costmap); cudaFree(c->d_u_raw); cudaFree(c->d_ce);
+  cudaFree(c->d_S); cudaFree(c->d_cvar); cudaFree(c->d_S_tilde); cudaFree(c->d_w_mat); cudaFree(c->d_loop);
+  delete c;
+  return RA_OK;
+}
+
+const char* ra_mppi_last_error(const ra_mppi_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+
+}  // extern "C"
+
+namespace {
+
+cudaError_t launch_sample_nominal(const ra_mppi_ctx* c, const Params& p, const float* d_x0, const float* d_v,
+                                  cudaStream_t s) {
+  const int threads = 128, grid = (p.K + threads - 1) / threads;
+  const size_t smem = (size_t)2 * p.T * sizeof(float);
+  const int dyn = c->cfg.dyn, nom = c->cfg.nominal;
+  if (dyn == 0 && nom == 0) sample_nominal_kernel<0, 0><<<grid, threads, smem, s>>>(p, d_x0, d_v);
+  else if (dyn == 0 && nom == 1) sample_nominal_kernel<0, 1><<<grid, threads, smem, s>>>(p, d_x0, d_v);
+  else if (dyn == 1 && nom == 0) sample_nominal_kernel<1, 0><<<grid, threads, smem, s>>>(p, d_x0, d_v);
+  else sample_nominal_kernel<1, 1><<<grid, threads, smem, s>>>(p, d_x0, d_v);
+  return cudaGetLastError();
+}
+
+template <int NX>
+cudaError_t launch_materialise(const ra_mppi_ctx* c, const Params& p, cudaStream_t s) {
+  const long long n = (long long)p.K * p.T * p.M_pad;
+  const int grid = (int)std::min<long long>((n + 255) / 256, 148LL * 16);
+  switch (c->cfg.noise_kind) {
+    case RA_NOISE_GAUSSIAN: materialise_noise_kernel<NX, NOISE_GAUSSIAN><<<grid, 256, 0, s>>>(p, c->d_w_mat); break;
+    case RA_NOISE_UNIFORM: materialise_noise_kernel<NX, NOISE_UNIFORM><<<grid, 256, 0, s>>>(p, c->d_w_mat); break;
+    default: materialise_noise_kernel<NX, NOISE_JUMP><<<grid, 256, 0, s>>>(p, c->d_w_mat); break;
+  }
+  return cudaGetLastError();
+}
+
+// Alg.1 l.3-29: sampling, nominal and noisy rollouts, CVaR, soft filter -> context scratch.
+ra_status enqueue_costs(ra_mppi_ctx* c, const Params& p, const float* d_x0, const float* d_v, float* d_L,
+                        float* d_xT, cudaStream_t s) {
+  if (c->cfg.noise_mode == RA_NOISE_MATERIALISED)
+    RA_CUDA(c, p.nx == 4 ? launch_materialise<4>(c, p, s) : launch_materialise<6>(c, p, s));
+  RA_CUDA(c, launch_sample_nominal(c, p, d_x0, d_v, s));
+  RA_CUDA(c, c->rollout(p, c->noise_variant, c->rc, c->half, d_x0, d_L, d_xT, s));
+  return RA_OK;
+}
+
+// Alg.1 l.31: weights (17) and update (4) from the context scratch.
+ra_status enqueue_update(ra_mppi_ctx* c, const Params& p, float* d_v_out, cudaStream_t s) {
+  weights_update_kernel<double><<<p.T, kUpdateThreads, 0, s>>>(
+      p, p.S_tilde, p.u_raw, 1LL, (long long)p.K, d_v_out, nullptr, nullptr);
+  RA_CUDA(c, cudaGetLastError());
+  return RA_OK;
+}
+
+cudaError_t launch_plant(const ra_mppi_ctx* c, const Params& p, float* d_x0, float* d_v, float* d_u,
+                         float* d_log, LoopState* loop, cudaStream_t s) {
+  const int dyn = c->cfg.dyn, nk = c->cfg.noise_kind;
+#define RA_PLANT(D, N) plant_shift_kernel<D, N><<<1, 128, 0, s>>>(p, d_x0, d_v, d_u, d_log, loop)
+  if (dyn == 0) { if (nk == 0) RA_PLANT(0, 0); else if (nk == 1) RA_PLANT(0, 1); else RA_PLANT(0, 2); }
+  else { if (nk == 0) RA_PLANT(1, 0); else if (nk == 1) RA_PLANT(1, 1); else RA_PLANT(1, 2); }
+#undef RA_PLANT
+  return cudaGetLastError();
+}
+
+Params with_iteration(const ra_mppi_ctx* c, uint64_t iteration) {
+  Params p = c->p;
+  p.d_iter = nullptr;
+  p.iter_imm = iteration;
+  return p;
+}
+
+}  // namespace
+
+extern "C" {
+
+ra_status ra_mppi_step(ra_mppi_ctx* c, const float* d_x0, float* d_v, uint64_t iteration, void* stream) {
+  if (!c) return RA_EINVAL;
+  if (!d_x0 || !d_v) return fail(c, RA_EINVAL, "null device pointer");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const Params p = with_iteration(c, iteration);
+  if (ra_status st = enqueue_costs(c, p, d_x0, d_v, nullptr, nullptr, s)) return st;
+  return enqueue_update(c, p, d_v, s);
+}
+
+ra_status ra_mppi_rollout_costs(ra_mppi_ctx* c, const float* d_x0, const float* d_v, uint64_t iteration,
+                                float* d_S, float* d_cvar, float* d_S_tilde, float* d_L, float* d_xT,
+                                float* d_u, void* stream) {
+  if (!c) return RA_EINVAL;
+  if (!d_x0 || !d_v) return fail(c, RA_EINVAL, "null device pointer");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const Params p = with_iteration(c, iteration);
+  if (ra_status st = enqueue_costs(c, p, d_x0, d_v, d_L, d_xT, s)) return st;
+  if (d_S || d_cvar || d_S_tilde) {
+    export_costs_kernel<<<(p.K + 255) / 256, 256, 0, s>>>(p, d_S, d_cvar, d_S_tilde);
+    RA_CUDA(c, cudaGetLastError());
+  }
+  if (d_u) {
+    export_u_kernel<<<148 * 4, 256, 0, s>>>(p, reinterpret_cast<float2*>(d_u));
+    RA_CUDA(c, cudaGetLastError());
+  }
+  return RA_OK;
+}
+
+ra_status ra_mppi_weights_update(ra_mppi_ctx* c, const float* d_S_tilde, const float* d_u, float* d_v_plus,
+                                 float* d_w, float* d_stats, void* stream) {
+  if (!c) return RA_EINVAL;
+  if (!d_S_tilde || !d_u || !d_v_plus) return fail(c, RA_EINVAL, "null device pointer");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const Params p = with_iteration(c, 0);
+  weights_update_kernel<float><<<p.T, kUpdateThreads, 0, s>>>(
+      p, d_S_tilde, reinterpret_cast<const float2*>(d_u), (long long)p.T, 1LL, d_v_plus, d_w, d_stats);
+  RA_CUDA(c, cudaGetLastError());
+  return RA_OK;
+}
+
+ra_status ra_mppi_plant_shift(ra_mppi_ctx* c, float* d_x0, float* d_v, float* d_u_applied, uint64_t iteration,
+                              void* stream) {
+  if (!c) return RA_EINVAL;
+  if (!d_x0 || !d_v) return fail(c, RA_EINVAL, "null device pointer");
+  const Params p = with_iteration(c, iteration);
+  RA_CUDA(c, launch_plant(c, p, d_x0, d_v, d_u_applied, nullptr, nullptr, static_cast<cudaStream_t>(stream)));
+  return RA_OK;
+}
+
+ra_status ra_mppi_export_costs_f64(ra_mppi_ctx* c, double* d_S64, double* d_S_tilde64, void* stream) {
+  if (!c) return RA_EINVAL;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const size_t n = (size_t)c->p.K * sizeof(double);
+  if (d_S64) RA_CUDA(c, cudaMemcpyAsync(d_S64, c->d_S, n, cudaMemcpyDeviceToDevice, s));
+  if (d_S_tilde64) RA_CUDA(c, cudaMemcpyAsync(d_S_tilde64, c->d_S_tilde, n, cudaMemcpyDeviceToDevice, s));
+  return RA_OK;
+}
+
+int32_t ra_mppi_launches_per_step(const ra_mppi_ctx* c) {
+  if (!c) return 0;
+  return 3 + (c->cfg.noise_mode == RA_NOISE_MATERIALISED ? 1 : 0);
+}
+
+ra_status ra_mppi_philox(ra_mppi_ctx* c, const uint32_t* d_ctr, int32_t n, uint32_t* d_out, void* stream) {
+  if (!c) return RA_EINVAL;
+  if (!d_ctr || !d_out || n < 0) return fail(c, RA_EINVAL, "bad arguments");
+  if (n == 0) return RA_OK;
+  philox_probe_kernel<<<(n + 255) / 256, 256, 0, static_cast<cudaStream_t>(stream)>>>(
+      c->p, reinterpret_cast<const uint4*>(d_ctr), n, reinterpret_cast<uint4*>(d_out));
+  RA_CUDA(c, cudaGetLastError());
+  return RA_OK;
+}
+
+ra_status ra_mppi_state_noise(ra_mppi_ctx* c, const int32_t* d_kmt, int32_t n, uint64_t iteration, float* d_w,
+                              void* stream) {
+  if (!c) return RA_EINVAL;
+  if (!d_kmt || !d_w || n < 0) return fail(c, RA_EINVAL, "bad arguments");
+  if (n == 0) return RA_OK;
+  const Params p = with_iteration(c, iteration);
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const int grid = (n + 255) / 256, nk = c->cfg.noise_kind;
+#define RA_PROBE(NX, N) noise_probe_kernel<NX, N><<<grid, 256, 0, s>>>(p, d_kmt, n, d_w)
+  if (p.nx == 4) { if (nk == 0) RA_PROBE(4, 0); else if (nk == 1) RA_PROBE(4, 1); else RA_PROBE(4, 2); }
+  else { if (nk == 0) RA_PROBE(6, 0); else if (nk == 1) RA_PROBE(6, 1); else RA_PROBE(6, 2); }
+#undef RA_PROBE
+  RA_CUDA(c, cudaGetLastError());
+  return RA_OK;
+}
+
+}  // extern "C"
+
+namespace {
+__global__ void set_loop_kernel(LoopState* loop, unsigned long long iter0) {
+  loop->iter = iter0;
+  loop->log_idx = 0ull;
+}
+}  // namespace
+
+extern "C" {
+
+ra_status ra_mppi_closed_loop(ra_mppi_ctx* c, float* d_x0, float* d_v, uint64_t iteration0, int32_t n_iter,
+                              float* d_log, float* h_ms, void* stream) {
+  if (!c) return RA_EINVAL;
+  if (!d_x0 || !d_v || n_iter < 0) return fail(c, RA_EINVAL, "bad arguments");
+  if (n_iter == 0) return RA_OK;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  cudaStream_t own = nullptr;
+  if (s == nullptr) {  // the legacy default stream cannot be captured
+    RA_CUDA(c, cudaStreamCreateWithFlags(&own, cudaStreamNonBlocking));
+    s = own;
+  }
+  ra_status st = RA_OK;
+  std::vector<cudaEvent_t> ev;
+  do {
+    // (re)capture one iteration: step kernels + plant/shift, all reading the device-resident counter
+    if (!c->graph_exec || c->g_x0 != d_x0 || c->g_v != d_v || c->g_log != d_log) {
+      if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+      Params p = c->p;
+      p.d_iter = &c->d_loop->iter;
+      p.iter_imm = 0;
+      cudaGraph_t graph = nullptr;
+      if (cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { st = fail(c, RA_ECUDA, "begin capture"); break; }
+      st = enqueue_costs(c, p, d_x0, d_v, nullptr, nullptr, s);
+      if (st == RA_OK) st = enqueue_update(c, p, d_v, s);
+      if (st == RA_OK) st = cuda_fail(c, launch_plant(c, p, d_x0, d_v, nullptr, d_log, c->d_loop, s), "plant");
+      cudaError_t e = cudaStreamEndCapture(s, &graph);
+      if (st != RA_OK) { if (graph) cudaGraphDestroy(graph); break; }
+      if (e != cudaSuccess) { st = cuda_fail(c, e, "end capture"); break; }
+      e = cudaGraphInstantiate(&c->graph_exec, graph, 0);
+      cudaGraphDestroy(graph);
+      if (e != cudaSuccess) { c->graph_exec = nullptr; st = cuda_fail(c, e, "graph instantiate"); break; }
+      c->g_x0 = d_x0; c->g_v = d_v; c->g_log = d_log;
+    }
+    set_loop_kernel<<<1, 1, 0, s>>>(c->d_loop, (unsigned long long)iteration0);
+    if ((st = cuda_fail(c, cudaGetLastError(), "set_loop")) != RA_OK) break;
+    if (h_ms) {
+      ev.resize((size_t)n_iter + 1);
+      for (auto& e : ev) if (cudaEventCreate(&e) != cudaSuccess) { st = fail(c, RA_ECUDA, "event create"); break; }
+      if (st != RA_OK) break;
+      cudaEventRecord(ev[0], s);
+    }
+    for (int i = 0; i < n_iter; ++i) {
+      cudaError_t e = cudaGraphLaunch(c->graph_exec, s);
+      if (e != cudaSuccess) { st = cuda_fail(c, e, "graph launch"); break; }
+      if (h_ms) cudaEventRecord(ev[(size_t)i + 1], s);
+    }
+    if (st != RA_OK) break;
+    if (h_ms || own) {
+      cudaError_t e = cudaStreamSynchronize(s);
+      if (e != cudaSuccess) { st = cuda_fail(c, e, "closed loop sync"); break; }
+    }
+    if (h_ms)
+      for (int i = 0; i < n_iter; ++i) cudaEventElapsedTime(&h_ms[i], ev[(size_t)i], ev[(size_t)i + 1]);
+  } while (false);
+  for (auto e : ev) if (e) cudaEventDestroy(e);
+  if (own) cudaStreamDestroy(own);
+  return st;
+}
+
+}  // extern "C"

@@ -1,0 +1,60 @@
+// Kernel-side parameter block of the RA-MPPI hot path (sm_100a).
+// Built once per context on the host (ra_mppi.cu) and passed to every kernel by value.
+#pragma once
+#include <cstdint>
+
+namespace ra {
+
+enum : int { DYN_BICYCLE = 0, DYN_SINGLE_TRACK = 1 };
+enum : int { NOM_GOAL = 0, NOM_TRACK = 1 };
+enum : int { RISK_CIRCLES = 0, RISK_COSTMAP = 1, RISK_LINEAR = 2 };
+enum : int { NOISE_GAUSSIAN = 0, NOISE_UNIFORM = 1, NOISE_JUMP = 2 };
+enum : uint32_t { STREAM_EPS = 0u, STREAM_W = 1u, STREAM_PLANT = 2u };
+
+constexpr int kMaxCirclesSmem = 1024;  // obstacle records staged per CTA (16 B each)
+
+struct Params {
+  int K, M, T;
+  int K0;       // samples k < K0 use u = v + eps, the rest u = eps   (Alg.1 l.7-10)
+  int k_tail;   // ceil((1-alpha) M)                                  (Alg.1 l.25)
+  int G;        // lanes per control sample: 32, or 16 when M <= 16
+  int R_total;  // realisations per lane = ceil(M / G)
+  int nx;
+  float dt;
+  float dyn_p[8];
+  float u_min[2], u_max[2];
+  float sigma_eps[2];
+  float ctrl_w[2];  // gamma / sigma_eps^2 (0 where sigma_eps == 0)   (3) PAPER.md:47
+  float sigma_w[6];
+  float neg_log2e_over_lambda;  // weights (17) PAPER.md:134 as exp2
+  float A, B, C_u;
+  float nom_p[8];
+  float risk_p[4];
+  float noise_p[4];
+  int Jc;           // Philox calls per state step (counter stride)
+  uint32_t rk[20];  // the ten Philox round keys (k0_r, k1_r), key = seed
+  // environment (device copies owned by the context)
+  const float4* circles;  // [n] absolute (cx, cy, r + margin, unused)
+  int n_circles;
+  const float* costmap;
+  int map_h, map_w;
+  float map_inv_res, map_ox, map_oy;
+  // scratch owned by the context
+  float2* u_raw;   // [T][K] sampled controls u^k_t (unclamped)
+  float4* ce;      // [T][K] control effects consumed by the rollout kernels
+  double* S;        // [K] nominal cost (3), fp64 so weight errors come from q, not from the sum
+  float* cvar;      // [K]
+  double* S_tilde;  // [K] modified cost (16)
+  const float* w_mat;  // materialised noise [K][T][nx][M_pad] or nullptr
+  int M_pad;
+  // iteration index: device-resident when replayed from a graph, immediate otherwise
+  const unsigned long long* d_iter;
+  unsigned long long iter_imm;
+};
+
+__device__ __forceinline__ uint32_t iteration_field(const Params& p, uint32_t stream) {
+  const unsigned long long it = p.d_iter ? *p.d_iter : p.iter_imm;
+  return (stream << 28) | (uint32_t)(it & 0x0FFFFFFFull);
+}
+
+}  // namespace ra

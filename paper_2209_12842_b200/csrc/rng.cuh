@@ -1,0 +1,113 @@
+// Counter-based noise in registers: Philox4x32-10 + Box-Muller on exact 23-bit uniforms.
+// BASELINE.json fixes the generator; the counter layout is DESIGN.md "RNG layout":
+//   ctr = (k, m, t*Jc + j, stream<<28 | iteration&0x0FFFFFFF),  key = (seed lo, seed hi).
+// No [K,M,T,n] noise tensor goes to HBM in fused mode.
+#pragma once
+#include <cstdint>
+
+#include "ra_params.cuh"
+
+namespace ra {
+
+// One Philox round: two 32x32->64 multiplies (IMAD.WIDE.U32) and two 3-input XORs (LOP3).
+__device__ __forceinline__ void philox_round(uint32_t& c0, uint32_t& c1, uint32_t& c2, uint32_t& c3,
+                                             uint32_t k0, uint32_t k1) {
+  const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0;
+  const unsigned long long p1 = (unsigned long long)0xCD9E8D57u * c2;
+  const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+  const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+  c1 = (uint32_t)p1;
+  c3 = (uint32_t)p0;
+  c0 = n0;
+  c2 = n2;
+}
+
+// rk = the ten (k0,k1) round keys, precomputed on the host because the key is the seed.
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                               const uint32_t* __restrict__ rk) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) philox_round(c0, c1, c2, c3, rk[2 * r], rk[2 * r + 1]);
+  return make_uint4(c0, c1, c2, c3);
+}
+
+// sin(pi r), cos(pi r) for |r| <= 1/4: minimax-style odd/even polynomials on the FMA pipe.
+__device__ __forceinline__ void sincospi_quarter(float r, float& s, float& c) {
+  const float r2 = r * r;
+  // sin(pi r) = r (pi + r2 (s3 + r2 (s5 + r2 s7)))
+  float ps = 0.0821458866f;          //  pi^9/362880
+  ps = fmaf(ps, r2, -0.59926452f);   // -pi^7/5040
+  ps = fmaf(ps, r2, 2.55016404f);    //  pi^5/120
+  ps = fmaf(ps, r2, -5.16771278f);   // -pi^3/6
+  const float r3 = r2 * r;
+  s = fmaf(r, 3.14159265f, r3 * ps);
+  // cos(pi r) = 1 + r2 (c2 + r2 (c4 + r2 (c6 + r2 c8)))
+  float pc = 0.235330630f;           //  pi^8/40320
+  pc = fmaf(pc, r2, -1.33526277f);   // -pi^6/720
+  pc = fmaf(pc, r2, 4.05871213f);    //  pi^4/24
+  pc = fmaf(pc, r2, -4.93480220f);   // -pi^2/2
+  c = fmaf(pc, r2, 1.0f);
+}
+
+// Box-Muller pair from two Philox words.  u1 = ((ra>>9)+1) 2^-23 in (0,1], u2 = (rb>>9) 2^-23
+// in [0,1) are exact in fp32, so this starts from the same reals as the fp64 oracle.
+// The angle 2 pi u2 is reduced exactly in integers: n = rb>>9 in [0,2^23), quadrant q and
+// remainder r = u2*2... in [-1/4,1/4] half-turns, then polynomials (no MUFU sin/cos).
+__device__ __forceinline__ void box_muller(uint32_t ra, uint32_t rb, float& z0, float& z1) {
+  const float u1 = __uint2float_rn((ra >> 9) + 1u) * 1.1920928955078125e-07f;
+  const float rho = sqrtf(-2.0f * logf(u1));
+  const uint32_t n = rb >> 9;                     // angle = n * 2^-22 half-turns in [0,2)
+  const uint32_t q = (n + (1u << 20)) >> 21;      // nearest multiple of 1/2 half-turn, 0..4
+  const int rem = (int)n - (int)(q << 21);        // in [-2^20, 2^20]
+  const float r = __int2float_rn(rem) * 2.384185791015625e-07f;  // * 2^-22, exact
+  float s, c;
+  sincospi_quarter(r, s, c);
+  // rotate by q quarter-turns
+  const float cs = (q & 1u) ? -s : c;
+  const float sn = (q & 1u) ? c : s;
+  const bool neg = ((q + 0u) & 2u) != 0u;
+  z0 = rho * (neg ? -cs : cs);
+  z1 = rho * (neg ? -sn : sn);
+}
+
+// Uniform on (-1,1): (2 (r>>9) + 1) 2^-23 - 1, exact.
+__device__ __forceinline__ float sym_uniform(uint32_t r) {
+  return fmaf(__uint2float_rn(2u * (r >> 9) + 1u), 1.1920928955078125e-07f, -1.0f);
+}
+
+// The n_x per-step state-noise values z (before the sigma_w scale) of realisation (k,m) at
+// step t.  NX = 4 -> one Philox call, NX = 6 -> two.  Jump noise makes one more call.
+template <int NX, int NOISE>
+__device__ __forceinline__ void state_noise(const Params& p, uint32_t k, uint32_t m, uint32_t t,
+                                            uint32_t c3, float (&z)[NX]) {
+  constexpr int J = (NX + 3) / 4;
+  constexpr int Jc = (NOISE == NOISE_JUMP) ? J + 1 : J;
+  const uint32_t c2 = t * (uint32_t)Jc;
+  const uint4 a = philox4x32_10(k, m, c2, c3, p.rk);
+  if constexpr (NOISE == NOISE_UNIFORM) {
+    z[0] = sym_uniform(a.x); z[1] = sym_uniform(a.y); z[2] = sym_uniform(a.z); z[3] = sym_uniform(a.w);
+  } else {
+    box_muller(a.x, a.y, z[0], z[1]);
+    box_muller(a.z, a.w, z[2], z[3]);
+  }
+  if constexpr (NX == 6) {
+    const uint4 b = philox4x32_10(k, m, c2 + 1u, c3, p.rk);
+    if constexpr (NOISE == NOISE_UNIFORM) {
+      z[4] = sym_uniform(b.x); z[5] = sym_uniform(b.y);
+    } else {
+      box_muller(b.x, b.y, z[4], z[5]);
+    }
+  }
+  if constexpr (NOISE == NOISE_JUMP) {
+    const uint4 jr = philox4x32_10(k, m, c2 + (uint32_t)J, c3, p.rk);
+    const float uj = __uint2float_rn(jr.x >> 9) * 1.1920928955078125e-07f;
+    float n2 = 0.0f;
+#pragma unroll
+    for (int i = 0; i < NX; ++i) n2 = fmaf(z[i], z[i], n2);
+    const bool jump = (uj < p.noise_p[0]) && (n2 > 0.0f);
+    const float inv = jump ? rsqrtf(n2) : 0.0f;
+#pragma unroll
+    for (int i = 0; i < NX; ++i) z[i] *= inv;
+  }
+}
+
+}  // namespace ra

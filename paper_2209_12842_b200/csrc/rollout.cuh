@@ -1,0 +1,256 @@
+// Rollout kernels of the RA-MPPI iteration (Alg.1 l.3-29).
+//   sample_nominal_kernel : A1 + A2  (one thread per control sample k)
+//   noisy_rollout_kernel  : A3 + A4 + A5 + A6 + A7 (one warp, or half-warp when M <= 16, per
+//                           control sample; lanes over the M realisations; noise in registers)
+#pragma once
+#include "models.cuh"
+#include "ra_params.cuh"
+#include "rng.cuh"
+
+namespace ra {
+
+constexpr int kRolloutThreads = 256;
+constexpr int kRolloutWarps = kRolloutThreads / 32;
+constexpr int NOISE_MATERIALISED = 3;  // rollout-kernel variant that reads w from HBM
+
+// ---------------------------------------------------------------------------------------
+// A1 + A2.  eps^k_t = sigma_eps (.) z, u^k_t = (k < K0 ? v_t : 0) + eps^k_t   (2c) PAPER.md:42,
+// Alg.1 l.4-10; nominal rollout and S_k = sum_t [q(x_t) + gamma v_t^T Sigma^-1 u_t] + phi(x_T)
+// (3) PAPER.md:47, Alg.1 l.11-15.  S is accumulated in fp64 (K*T adds only) because the
+// softmin weights of (17) are sensitive to absolute errors in S~.
+// ---------------------------------------------------------------------------------------
+template <int DYN, int NOM>
+__global__ void __launch_bounds__(128) sample_nominal_kernel(const __grid_constant__ Params p,
+                                                             const float* __restrict__ x0g,
+                                                             const float* __restrict__ v) {
+  constexpr int NX = StateDim<DYN>::value;
+  extern __shared__ float v_s[];  // [T][2]
+  for (int i = threadIdx.x; i < 2 * p.T; i += blockDim.x) v_s[i] = v[i];
+  __syncthreads();
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= p.K) return;
+
+  const float x0X = x0g[0], x0Y = x0g[1];
+  float x[NX];
+  x[0] = 0.0f; x[1] = 0.0f;
+#pragma unroll
+  for (int i = 2; i < NX; ++i) x[i] = x0g[i];
+  if constexpr (DYN == DYN_SINGLE_TRACK) x[3] = fmaxf(x[3], p.dyn_p[6]);
+
+  const uint32_t c3 = iteration_field(p, STREAM_EPS);
+  const bool with_mean = k < p.K0;
+  double S = 0.0;
+  for (int t = 0; t < p.T; ++t) {
+    const uint4 r = philox4x32_10((uint32_t)k, 0u, (uint32_t)t, c3, p.rk);
+    float z0, z1;
+    box_muller(r.x, r.y, z0, z1);
+    const float v0 = v_s[2 * t], v1 = v_s[2 * t + 1];
+    const float u0 = fmaf(p.sigma_eps[0], z0, with_mean ? v0 : 0.0f);
+    const float u1 = fmaf(p.sigma_eps[1], z1, with_mean ? v1 : 0.0f);
+    const float4 ce = control_effect<DYN>(p, u0, u1);
+    p.u_raw[(size_t)t * p.K + k] = make_float2(u0, u1);
+    p.ce[(size_t)t * p.K + k] = ce;
+    const float q = nominal_cost<NOM>(p, x0X + x[0], x0Y + x[1], x[3]);
+    const float ctrl = fmaf(p.ctrl_w[0] * v0, u0, p.ctrl_w[1] * v1 * u1);
+    S += (double)q + (double)ctrl;
+    dynamics_step<DYN>(p, x, ce);
+  }
+  const float w_phi = (NOM == NOM_GOAL) ? p.nom_p[3] : p.nom_p[7];
+  S += (double)(w_phi * nominal_cost<NOM>(p, x0X + x[0], x0Y + x[1], x[3]));
+  p.S[k] = S;
+}
+
+// order-preserving map float -> uint32 (larger float <=> larger key); 0 is below every float
+__device__ __forceinline__ uint32_t float_key(float f) {
+  const uint32_t b = __float_as_uint(f);
+  return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+__device__ __forceinline__ float key_float(uint32_t k) {
+  return __uint_as_float((k & 0x80000000u) ? (k ^ 0x80000000u) : ~k);
+}
+
+template <int G>
+__device__ __forceinline__ float group_sum(float v, uint32_t mask) {
+#pragma unroll
+  for (int o = G / 2; o > 0; o >>= 1) v += __shfl_xor_sync(mask, v, o);
+  return v;
+}
+
+// ---------------------------------------------------------------------------------------
+// A6: CVaR_k = mean of the k_tail largest of the M risk costs (Alg.1 l.25-26 PAPER.md:204-207,
+// (12) :107), by a bitwise radix select on order-preserving keys: 32 rounds of
+// (compare, warp REDUX) find the k_tail-th largest value exactly; the tail sum is then
+// sum(values above it) + (k_tail - count above) * it, which does not depend on which of
+// several tied values are "picked".  keys: R_total slots per lane in shared memory
+// (slot r of lane l at keys[r*32 + l]; key 0 marks an unused slot).
+// Returns CVaR of the raw costs; *mean_out = (1/M) sum (for (18)-(19)).
+// ---------------------------------------------------------------------------------------
+template <int G>
+__device__ __forceinline__ float cvar_select(const uint32_t* keys, int R_total, int lane, int k_tail,
+                                             int M, uint32_t mask, float* mean_out) {
+  uint32_t prefix = 0u;
+  int k_rem = k_tail;
+  for (int bit = 31; bit >= 0; --bit) {
+    const uint32_t cand = (prefix | (1u << bit)) >> bit;
+    int cnt = 0;
+    for (int r = 0; r < R_total; ++r) cnt += ((keys[r * 32 + lane] >> bit) == cand) ? 1 : 0;
+    cnt = __reduce_add_sync(mask, cnt);
+    if (cnt >= k_rem) prefix |= (1u << bit); else k_rem -= cnt;
+  }
+  // prefix = key of the k_tail-th largest; k_rem = how many copies of it belong to the tail
+  float sum_gt = 0.0f, sum_all = 0.0f;
+  for (int r = 0; r < R_total; ++r) {
+    const uint32_t key = keys[r * 32 + lane];
+    const float val = key ? key_float(key) : 0.0f;
+    sum_all += val;
+    sum_gt += (key > prefix) ? val : 0.0f;
+  }
+  sum_gt = group_sum<G>(sum_gt, mask);
+  sum_all = group_sum<G>(sum_all, mask);
+  *mean_out = sum_all / (float)M;
+  return fmaf((float)k_rem, key_float(prefix), sum_gt) / (float)k_tail;
+}
+
+// Risk running cost l(x~) (9) PAPER.md:93 for RC interleaved realisations of one lane.
+template <int RISK, int RC, int NX>
+__device__ __forceinline__ void risk_accumulate(const Params& p, const float4* circ_s,
+                                                const MapFrame& mf, float x0X, float x0Y,
+                                                const float (&x)[RC][NX], float (&L)[RC]) {
+  if constexpr (RISK == RISK_CIRCLES) {
+    const float w = p.risk_p[0];
+    for (int i = 0; i < p.n_circles; ++i) {
+      const float4 c = circ_s[i];  // (cx - x0X, cy - x0Y, r + margin, (r + margin)^2), broadcast
+#pragma unroll
+      for (int r = 0; r < RC; ++r) {
+        const float dx = x[r][0] - c.x, dy = x[r][1] - c.y;
+        const float d2 = fmaf(dx, dx, dy * dy);
+        if (d2 < c.w) {
+          const float pen = c.z - sqrtf(d2);
+          L[r] = fmaf(w * pen, pen, L[r]);
+        }
+      }
+    }
+  } else if constexpr (RISK == RISK_COSTMAP) {
+#pragma unroll
+    for (int r = 0; r < RC; ++r) L[r] = fmaf(p.risk_p[0], bilinear(p, mf, x[r][0], x[r][1]), L[r]);
+  } else {  // test-only linear risk: weight * x[index]
+    const int idx = (int)p.risk_p[1];
+#pragma unroll
+    for (int r = 0; r < RC; ++r) {
+      float val = 0.0f;
+#pragma unroll
+      for (int i = 0; i < NX; ++i) val = (i == idx) ? x[r][i] : val;
+      val += (idx == 0) ? x0X : ((idx == 1) ? x0Y : 0.0f);
+      L[r] = fmaf(p.risk_p[0], val, L[r]);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+// A3-A7.  HALF: two control samples per warp (G = 16 lanes each, M <= 16).
+// Dynamic shared memory: [n_circles] float4 obstacle records, then per warp R_total*32 keys.
+// ---------------------------------------------------------------------------------------
+template <int DYN, int RISK, int NOISE, int RC, bool HALF>
+__global__ void __launch_bounds__(kRolloutThreads)
+noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__ x0g,
+                     float* __restrict__ L_out, float* __restrict__ xT_out) {
+  constexpr int NX = StateDim<DYN>::value;
+  constexpr int G = HALF ? 16 : 32;
+  extern __shared__ float4 smem4[];
+  float4* circ_s = smem4;
+  const int n_circ_s = (RISK == RISK_CIRCLES) ? p.n_circles : 0;
+  uint32_t* keys_all = reinterpret_cast<uint32_t*>(smem4 + n_circ_s);
+
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const float x0X = x0g[0], x0Y = x0g[1];
+  if constexpr (RISK == RISK_CIRCLES) {
+    for (int i = threadIdx.x; i < p.n_circles; i += blockDim.x) {
+      const float4 c = p.circles[i];
+      circ_s[i] = make_float4(c.x - x0X, c.y - x0Y, c.z, c.z * c.z);
+    }
+    __syncthreads();
+  }
+  MapFrame mf{};
+  if constexpr (RISK == RISK_COSTMAP) mf = make_map_frame(p, x0X, x0Y);
+
+  const int gwarp = blockIdx.x * kRolloutWarps + warp;
+  const int k_raw = HALF ? gwarp * 2 + (lane >> 4) : gwarp;
+  const int sub = HALF ? (lane & 15) : lane;
+  const uint32_t mask = HALF ? (0xFFFFu << (lane & 16)) : 0xFFFFFFFFu;
+  const bool k_valid = k_raw < p.K;
+  const int k = k_valid ? k_raw : p.K - 1;
+  uint32_t* keys = keys_all + (size_t)warp * p.R_total * 32;
+
+  float x_init[NX];
+  x_init[0] = 0.0f; x_init[1] = 0.0f;
+#pragma unroll
+  for (int i = 2; i < NX; ++i) x_init[i] = x0g[i];
+  if constexpr (DYN == DYN_SINGLE_TRACK) x_init[3] = fmaxf(x_init[3], p.dyn_p[6]);
+
+  const uint32_t c3 = iteration_field(p, STREAM_W);
+  const float4* ce_k = p.ce + k;
+
+  for (int chunk = 0; chunk < p.R_total; chunk += RC) {
+    float x[RC][NX], L[RC];
+    uint32_t m[RC];
+#pragma unroll
+    for (int r = 0; r < RC; ++r) {
+      L[r] = 0.0f;
+      m[r] = (uint32_t)((chunk + r) * G + sub);
+#pragma unroll
+      for (int i = 0; i < NX; ++i) x[r][i] = x_init[i];
+    }
+    float4 ce = __ldg(ce_k);
+    for (int t = 0; t < p.T; ++t) {
+      const float4 ce_next = __ldg(ce_k + (size_t)min(t + 1, p.T - 1) * p.K);  // prefetch
+      risk_accumulate<RISK, RC, NX>(p, circ_s, mf, x0X, x0Y, x, L);            // l(x~_t), pre-step
+#pragma unroll
+      for (int r = 0; r < RC; ++r) {
+        float z[NX];
+        if constexpr (NOISE == NOISE_MATERIALISED) {
+          const float* wp = p.w_mat + (((size_t)k * p.T + t) * NX) * p.M_pad + m[r];
+#pragma unroll
+          for (int i = 0; i < NX; ++i) z[i] = __ldg(wp + (size_t)i * p.M_pad);
+        } else {
+          state_noise<NX, NOISE>(p, (uint32_t)k, m[r], (uint32_t)t, c3, z);
+#pragma unroll
+          for (int i = 0; i < NX; ++i) z[i] *= p.sigma_w[i];
+        }
+        dynamics_step<DYN>(p, x[r], ce);   // x~_{t+1} = F(x~_t, u_t) + w_t   (6) PAPER.md:63
+#pragma unroll
+        for (int i = 0; i < NX; ++i) x[r][i] += z[i];
+        if constexpr (DYN == DYN_SINGLE_TRACK) x[r][3] = fmaxf(x[r][3], p.dyn_p[6]);
+      }
+      ce = ce_next;
+    }
+#pragma unroll
+    for (int r = 0; r < RC; ++r) {
+      const bool valid = (chunk + r) < p.R_total && (int)m[r] < p.M;
+      if (chunk + r < p.R_total) keys[(chunk + r) * 32 + lane] = valid ? float_key(L[r]) : 0u;
+      if (valid && k_valid) {
+        if (L_out) L_out[(size_t)k * p.M + m[r]] = L[r];
+        if (xT_out) {
+          float* o = xT_out + ((size_t)k * p.M + m[r]) * NX;
+          o[0] = x0X + x[r][0]; o[1] = x0Y + x[r][1];
+#pragma unroll
+          for (int i = 2; i < NX; ++i) o[i] = x[r][i];
+        }
+      }
+    }
+  }
+  __syncwarp();
+
+  float Lbar;
+  float cvar = cvar_select<G>(keys, p.R_total, lane, p.k_tail, p.M, mask, &Lbar);
+  // (18)-(19) PAPER.md:144-148: L_a = B (L - Lbar) + Lbar is affine-monotone for B > 0, so
+  // CVaR(L_a) = B (CVaR(L) - Lbar) + Lbar.
+  if (p.B != 1.0f) cvar = fmaf(p.B, cvar - Lbar, Lbar);
+  if (sub == 0 && k_valid) {
+    // soft filter (14)-(16) PAPER.md:120-130, strict threshold (15)
+    const double pen = (cvar > p.C_u) ? (double)(p.A * cvar) : 0.0;
+    p.cvar[k] = cvar;
+    p.S_tilde[k] = p.S[k] + pen;
+  }
+}
+
+}  // namespace ra

@@ -1,0 +1,56 @@
+// Instantiates noisy_rollout_kernel for one (dynamics, risk) pair:
+//   nvcc -DRA_INST_DYN=<0|1> -DRA_INST_RISK=<0|1|2> -c rollout_inst.cu
+#include "launchers.h"
+#include "rollout.cuh"
+
+#ifndef RA_INST_DYN
+#error "define RA_INST_DYN"
+#endif
+#ifndef RA_INST_RISK
+#error "define RA_INST_RISK"
+#endif
+
+namespace ra {
+namespace {
+
+template <int NOISE, int RC, bool HALF>
+cudaError_t launch(const Params& p, const float* d_x0, float* d_L, float* d_xT, cudaStream_t stream) {
+  const int samples_per_cta = HALF ? 2 * kRolloutWarps : kRolloutWarps;
+  const int grid = (p.K + samples_per_cta - 1) / samples_per_cta;
+  const size_t smem = (RA_INST_RISK == RISK_CIRCLES ? (size_t)p.n_circles * sizeof(float4) : 0) +
+                      (size_t)kRolloutWarps * p.R_total * 32 * sizeof(uint32_t);
+  noisy_rollout_kernel<RA_INST_DYN, RA_INST_RISK, NOISE, RC, HALF>
+      <<<grid, kRolloutThreads, smem, stream>>>(p, d_x0, d_L, d_xT);
+  return cudaGetLastError();
+}
+
+template <int NOISE>
+cudaError_t launch_noise(const Params& p, int rc, bool half, const float* d_x0, float* d_L, float* d_xT,
+                         cudaStream_t stream) {
+  if (half) return launch<NOISE, 1, true>(p, d_x0, d_L, d_xT, stream);
+  switch (rc) {
+    case 1: return launch<NOISE, 1, false>(p, d_x0, d_L, d_xT, stream);
+    case 2: return launch<NOISE, 2, false>(p, d_x0, d_L, d_xT, stream);
+    case 4: return launch<NOISE, 4, false>(p, d_x0, d_L, d_xT, stream);
+    default: return cudaErrorInvalidValue;
+  }
+}
+
+}  // namespace
+
+#define RA_CAT2(a, b, c) launch_rollout_##a##_##b
+#define RA_CAT(a, b) RA_CAT2(a, b, _)
+
+cudaError_t RA_CAT(RA_INST_DYN, RA_INST_RISK)(const Params& p, int noise, int rc, bool half,
+                                               const float* d_x0, float* d_L, float* d_xT,
+                                               cudaStream_t stream) {
+  switch (noise) {
+    case NOISE_GAUSSIAN: return launch_noise<NOISE_GAUSSIAN>(p, rc, half, d_x0, d_L, d_xT, stream);
+    case NOISE_UNIFORM: return launch_noise<NOISE_UNIFORM>(p, rc, half, d_x0, d_L, d_xT, stream);
+    case NOISE_JUMP: return launch_noise<NOISE_JUMP>(p, rc, half, d_x0, d_L, d_xT, stream);
+    case NOISE_MATERIALISED: return launch_noise<NOISE_MATERIALISED>(p, rc, half, d_x0, d_L, d_xT, stream);
+    default: return cudaErrorInvalidValue;
+  }
+}
+
+}  // namespace ra

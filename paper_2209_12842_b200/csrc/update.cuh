@@ -1,0 +1,182 @@
+// Weights (17)/(5), update (4), and the closed-loop glue (Alg.1 l.31-33).
+#pragma once
+#include "models.cuh"
+#include "ra_params.cuh"
+#include "rng.cuh"
+
+namespace ra {
+
+constexpr int kUpdateThreads = 1024;
+
+template <typename T, typename Op>
+__device__ __forceinline__ T block_reduce(T v, T* smem, Op op, T identity) {
+  // fixed-order tree: xor-shuffle inside each warp, then warp 0 over the per-warp partials
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = op(v, __shfl_xor_sync(0xFFFFFFFFu, v, o));
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  __syncthreads();  // smem may still be read from a previous reduction
+  if (lane == 0) smem[warp] = v;
+  __syncthreads();
+  v = (lane < (blockDim.x >> 5)) ? smem[lane] : identity;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = op(v, __shfl_xor_sync(0xFFFFFFFFu, v, o));
+  return v;  // every thread holds the result
+}
+
+// ---------------------------------------------------------------------------------------
+// A8 + A9.  One CTA per horizon step t.  Each CTA recomputes beta~ = min_k S~_k (K <= 65536
+// values from L2), then w~_k = exp(-(S~_k - beta~)/lambda), Z = sum w~, and
+// v+_t = clamp(sum_k w~_k u^k_t / Z)   (17) PAPER.md:134, (5) :55, (4) :51.
+// u is addressed as u[k*su_k + t*su_t] so both the internal [T][K] scratch and a caller's
+// [K][T] array work.  Reduction order is fixed => bitwise reproducible.
+// ---------------------------------------------------------------------------------------
+template <typename ST>
+__global__ void __launch_bounds__(kUpdateThreads)
+weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S_tilde,
+                      const float2* __restrict__ u, long long su_k, long long su_t,
+                      float* __restrict__ v_out, float* __restrict__ w_out,
+                      float* __restrict__ stats) {
+  __shared__ ST red_s[32];
+  __shared__ float red_f[32];
+  const int t = blockIdx.x;
+  ST bmin = (ST)INFINITY;
+  for (int k = threadIdx.x; k < p.K; k += blockDim.x) bmin = min(bmin, S_tilde[k]);
+  const ST beta = block_reduce<ST>(bmin, red_s, [](ST a, ST b) { return a < b ? a : b; }, (ST)INFINITY);
+
+  float Z = 0.0f, n0 = 0.0f, n1 = 0.0f;
+  for (int k = threadIdx.x; k < p.K; k += blockDim.x) {
+    const float w = exp2f((float)(S_tilde[k] - beta) * p.neg_log2e_over_lambda);
+    const float2 uk = __ldg(u + (long long)k * su_k + (long long)t * su_t);
+    Z += w;
+    n0 = fmaf(w, uk.x, n0);
+    n1 = fmaf(w, uk.y, n1);
+  }
+  auto add = [](float a, float b) { return a + b; };
+  Z = block_reduce<float>(Z, red_f, add, 0.0f);
+  n0 = block_reduce<float>(n0, red_f, add, 0.0f);
+  n1 = block_reduce<float>(n1, red_f, add, 0.0f);
+  if (threadIdx.x == 0) {
+    v_out[2 * t] = clampf(n0 / Z, p.u_min[0], p.u_max[0]);
+    v_out[2 * t + 1] = clampf(n1 / Z, p.u_min[1], p.u_max[1]);
+    if (t == 0 && stats) { stats[0] = (float)beta; stats[1] = Z; }
+  }
+  if (t == 0 && w_out) {
+    const float invZ = 1.0f / Z;
+    for (int k = threadIdx.x; k < p.K; k += blockDim.x)
+      w_out[k] = exp2f((float)(S_tilde[k] - beta) * p.neg_log2e_over_lambda) * invZ;
+  }
+}
+
+// [T][K] scratch -> caller's [K][T][2] (diagnostic output of ra_mppi_rollout_costs)
+__global__ void export_u_kernel(const __grid_constant__ Params p, float2* __restrict__ out) {
+  const long long n = (long long)p.K * p.T;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+       i += (long long)gridDim.x * blockDim.x) {
+    const int k = (int)(i / p.T), t = (int)(i % p.T);
+    out[i] = p.u_raw[(size_t)t * p.K + k];
+  }
+}
+
+__global__ void export_costs_kernel(const __grid_constant__ Params p, float* __restrict__ S,
+                                    float* __restrict__ cvar, float* __restrict__ S_tilde) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= p.K) return;
+  if (S) S[k] = (float)p.S[k];
+  if (cvar) cvar[k] = p.cvar[k];
+  if (S_tilde) S_tilde[k] = (float)p.S_tilde[k];
+}
+
+// Device-resident loop state for graph replay.
+struct LoopState {
+  unsigned long long iter;     // Philox iteration index of the next step
+  unsigned long long log_idx;  // row of the closed-loop log to write next
+};
+
+// ---------------------------------------------------------------------------------------
+// A10.  ExecuteCommand(v+_0) on the simulated plant (the disturbed dynamics (6) with the
+// PLANT stream), v <- shift(v+) (Alg.1 l.32-33 PAPER.md:218-220 + BASELINE config 4's
+// warm-start shift), iteration++.  One CTA.
+// ---------------------------------------------------------------------------------------
+template <int DYN, int NOISE>
+__global__ void __launch_bounds__(128) plant_shift_kernel(const __grid_constant__ Params p, float* x0g,
+                                                          float* v, float* u_applied, float* log,
+                                                          LoopState* loop) {
+  constexpr int NX = StateDim<DYN>::value;
+  // shift: read everything, then write
+  float2 nxt[2];
+  float2* v2 = reinterpret_cast<float2*>(v);
+  int cnt = 0;
+  for (int t = threadIdx.x; t < p.T; t += blockDim.x) nxt[cnt++] = v2[min(t + 1, p.T - 1)];
+  const float2 v0 = v2[0];
+  __syncthreads();
+  cnt = 0;
+  for (int t = threadIdx.x; t < p.T; t += blockDim.x) v2[t] = nxt[cnt++];
+
+  if (threadIdx.x == 0) {
+    float x[NX];
+    const float x0X = x0g[0], x0Y = x0g[1];
+    x[0] = 0.0f; x[1] = 0.0f;
+#pragma unroll
+    for (int i = 2; i < NX; ++i) x[i] = x0g[i];
+    if constexpr (DYN == DYN_SINGLE_TRACK) x[3] = fmaxf(x[3], p.dyn_p[6]);
+    const float4 ce = control_effect<DYN>(p, v0.x, v0.y);
+    float z[NX];
+    state_noise<NX, NOISE>(p, 0u, 0u, 0u, iteration_field(p, STREAM_PLANT), z);
+    dynamics_step<DYN>(p, x, ce);
+#pragma unroll
+    for (int i = 0; i < NX; ++i) x[i] = fmaf(p.sigma_w[i], z[i], x[i]);
+    if constexpr (DYN == DYN_SINGLE_TRACK) x[3] = fmaxf(x[3], p.dyn_p[6]);
+    x[0] += x0X; x[1] += x0Y;
+#pragma unroll
+    for (int i = 0; i < NX; ++i) x0g[i] = x[i];
+    if (u_applied) { u_applied[0] = v0.x; u_applied[1] = v0.y; }
+    if (log) {
+      float* row = log + (loop ? loop->log_idx : 0ull) * (NX + 2);
+#pragma unroll
+      for (int i = 0; i < NX; ++i) row[i] = x[i];
+      row[NX] = v0.x; row[NX + 1] = v0.y;
+    }
+    if (loop) { loop->iter += 1ull; loop->log_idx += 1ull; }
+  }
+}
+
+// Parity hooks: raw Philox words and state-noise draws exactly as the rollout kernel makes them.
+__global__ void philox_probe_kernel(const __grid_constant__ Params p, const uint4* __restrict__ ctr,
+                                    int n, uint4* __restrict__ out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = philox4x32_10(ctr[i].x, ctr[i].y, ctr[i].z, ctr[i].w, p.rk);
+}
+
+template <int NX, int NOISE>
+__global__ void noise_probe_kernel(const __grid_constant__ Params p, const int* __restrict__ kmt, int n,
+                                   float* __restrict__ w) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  float z[NX];
+  state_noise<NX, NOISE>(p, (uint32_t)kmt[3 * i], (uint32_t)kmt[3 * i + 1], (uint32_t)kmt[3 * i + 2],
+                         iteration_field(p, STREAM_W), z);
+#pragma unroll
+  for (int j = 0; j < NX; ++j) w[(size_t)i * NX + j] = z[j] * p.sigma_w[j];
+}
+
+// Materialised-noise generator: w[K][T][NX][M_pad] = sigma_w (.) z, the same draws the fused
+// kernel makes in registers (HBM-roofline mode of BASELINE.json).
+template <int NX, int NOISE>
+__global__ void __launch_bounds__(256) materialise_noise_kernel(const __grid_constant__ Params p,
+                                                                float* __restrict__ w) {
+  const long long n = (long long)p.K * p.T * p.M_pad;
+  const uint32_t c3 = iteration_field(p, STREAM_W);
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
+       i += (long long)gridDim.x * blockDim.x) {
+    const int m = (int)(i % p.M_pad);
+    const long long kt = i / p.M_pad;
+    const int t = (int)(kt % p.T), k = (int)(kt / p.T);
+    float z[NX];
+    state_noise<NX, NOISE>(p, (uint32_t)k, (uint32_t)m, (uint32_t)t, c3, z);
+    float* o = w + (size_t)kt * NX * p.M_pad + m;
+#pragma unroll
+    for (int j = 0; j < NX; ++j) o[(size_t)j * p.M_pad] = z[j] * p.sigma_w[j];
+  }
+}
+
+}  // namespace ra

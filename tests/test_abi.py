@@ -1,0 +1,113 @@
+"""Host-side checks that need no GPU: the C-ABI library builds, loads and exports every symbol
+include/ra_mppi.h declares; struct layouts agree; invalid configs are rejected before any
+CUDA call; the product path does not fall back to the CPU."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2209_12842_b200 import binding as B
+from paper_2209_12842_b200 import build as cuda_build
+from paper_2209_12842_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    cuda_build.build()
+    return B.load()
+
+
+def test_every_declared_symbol_is_exported(lib):
+    hdr = open(os.path.join(ROOT, "include", "ra_mppi.h")).read()
+    declared = set(re.findall(r"\b(ra_mppi_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(B.EXPORTS), declared ^ set(B.EXPORTS)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_struct_size_is_checked(lib):
+    p = W.config0()
+    cfg = B.make_config(p)
+    env, keep = B.make_env(p)
+    cfg.struct_size += 4
+    with pytest.raises(B.RaMppiError) as e:
+        B.ra_mppi_create(cfg, env)
+    assert e.value.status == B.RA_EINVAL
+
+
+@pytest.mark.parametrize("field,value", [
+    ("K", 0), ("M", -1), ("T", 0), ("dt", 0.0), ("alpha", 0.0), ("alpha", 1.0), ("lam", 0.0),
+    ("gamma", -1.0), ("eta", 1.0), ("B", 0.0), ("dyn", 7), ("risk", 5), ("nominal", 3), ("noise_kind", 9),
+])
+def test_invalid_config_is_einval(lib, field, value):
+    p = W.config0()
+    cfg = B.make_config(p)
+    env, keep = B.make_env(p)
+    setattr(cfg, field, value)
+    with pytest.raises(B.RaMppiError) as e:
+        B.ra_mppi_create(cfg, env)
+    assert e.value.status == B.RA_EINVAL
+
+
+def test_unsupported_sizes(lib):
+    p = W.config0()
+    for field, value in (("M", 513), ("T", 129)):
+        cfg = B.make_config(p)
+        env, keep = B.make_env(p)
+        setattr(cfg, field, value)
+        with pytest.raises(B.RaMppiError) as e:
+            B.ra_mppi_create(cfg, env)
+        assert e.value.status == B.RA_EUNSUPPORTED
+
+
+def test_missing_environment_is_einval(lib):
+    p = W.config0()
+    env, keep = B.make_env(p)
+    env.circles = None   # n_circles > 0 without the array (n_circles = 0 alone is a legal empty scene)
+    with pytest.raises(B.RaMppiError) as e:
+        B.ra_mppi_create(B.make_config(p), env)
+    assert e.value.status == B.RA_EINVAL
+    p3 = W.config3(K=8).replace(costmap=None)
+    with pytest.raises(B.RaMppiError) as e:
+        B.ra_mppi_create(B.make_config(p3), B.make_env(p3)[0])
+    assert e.value.status == B.RA_EINVAL
+
+
+def test_null_context_and_destroy_null(lib):
+    assert lib.ra_mppi_destroy(None) == B.RA_OK
+    assert lib.ra_mppi_step(None, None, None, 0, None) == B.RA_EINVAL
+    assert lib.ra_mppi_launches_per_step(None) == 0
+
+
+def test_no_cpu_fallback_without_gpu(lib):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    p = W.config0()
+    with pytest.raises(B.RaMppiError) as e:   # valid config, but no device: must fail loudly
+        B.ra_mppi_create(B.make_config(p), B.make_env(p)[0])
+    assert e.value.status == B.RA_ECUDA
+    from paper_2209_12842_b200.controller import RaMppi
+    with pytest.raises(B.RaMppiError):
+        RaMppi(p)
+
+
+def test_product_does_not_import_oracle():
+    """The product path never routes through the oracle, and the oracle never uses the product."""
+    pat = re.compile(r"(^\s*(import|from)\s+oracle\b)|(#include\s*[<\"].*oracle)|(libra_mppi_oracle)|(oracle[./])", re.M)
+    pkg = os.path.join(ROOT, "paper_2209_12842_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                if f == "workloads.py":   # mentions the folder in prose only
+                    src = src.replace("``oracle/``", "")
+                assert not pat.search(src), f
+    pat2 = re.compile(r"(^\s*(import|from)\s+paper_2209_12842_b200)|(#include\s*[<\"].*(ra_mppi\.h|\.cuh))|(libra_mppi\.so)", re.M)
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".cpp", ".h")):
+            assert not pat2.search(open(os.path.join(ROOT, "oracle", f)).read()), f
