@@ -1,0 +1,284 @@
+"""RA-MPPI benchmark: noisy state-steps/s (K*M*T per second) and iterations/s on one B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3] [--impl reference]
+
+A "step" is one full controller iteration (ra_mppi_step: sample -> nominal + noisy rollouts ->
+CVaR -> weights -> update) on the named BASELINE.json workload; default C3 = configs[3]
+(K=16384, M=128, T=50, costmap), the configuration BASELINE.json's target is quoted on.
+Prints ONE JSON line.  --impl reference times the fp64 oracle.
+The path does not shard (north_star: no second GPU): --gpus N runs N independent replicas.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2209_12842_b200 import workloads as W  # noqa: E402
+
+METRIC = "noisy_state_steps_per_s"
+UNIT = "state-steps/s"
+
+# Algorithmic lane-operations per noisy state-step: the instructions the
+# method itself needs (Philox, normal transform, dynamics, risk cost), one per FP32-lane slot.
+#   Philox4x32-10 call 40 (20 mul-wide + 20 xor3); Box-Muller 14 per pair + 1 scale-add per normal;
+#   bicycle step 7; single-track step 75; circle test 5 per obstacle; bilinear lookup 21.
+ALGO_OPS = {"C0": 40 + 32 + 7 + 5 * 8, "C1": 40 + 32 + 7 + 5 * 32, "C2": 80 + 48 + 75 + 5 * 128,
+            "C3": 40 + 32 + 7 + 21, "C4": 40 + 32 + 7 + 5 * 64}
+ALU_PEAK_LANE_OPS = 148 * 128 * 1.965e9  # 148 SMs x 128 FP32 lanes x 1.965 GHz (B200_PROFILING.md nominal)
+
+
+def make_problem(name: str, rank: int = 0) -> W.Problem:
+    name = name.upper()
+    if name == "C0":
+        p = W.config0(near_obstacle=True)
+    elif name == "C1":
+        p = W.config1()
+    elif name == "C2":
+        p = W.config2()
+    elif name == "C3":
+        p = W.config3()
+    elif name.startswith("C4"):
+        parts = name.split("-")
+        K = int(parts[1][1:]) if len(parts) > 1 else 8192
+        M = int(parts[2][1:]) if len(parts) > 2 else 64
+        p = W.config4(K=K, M=M)
+    else:
+        raise SystemExit(f"unknown workload {name}")
+    scale = (0.1, 0.5) if p.dyn == W.DYN_BICYCLE else (0.1, 2.0)
+    return p.replace(v=W.random_mean_control(p, rank, scale), seed=p.seed + 1000 * rank)
+
+
+def workload_key(name: str) -> str:
+    return name.upper().split("-")[0]
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML during the timed region."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.samples, self.reasons, self.max_mhz = index, False, [], set(), None
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+            names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "hw_thermal_slowdown": 0x40,
+                     "sw_thermal_slowdown": 0x20, "hw_power_brake": 0x80}
+            while not self.stop_flag:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for n, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(n)
+                time.sleep(0.005)
+        except Exception as e:  # pragma: no cover
+            self.reasons.add(f"nvml_unavailable:{type(e).__name__}")
+
+    def summary(self):
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def cpu_baseline(p: W.Problem, seconds_target: float = 15.0):
+    """The oracle as it stands, timed on the host cores on a bounded slice of the same workload."""
+    from oracle import oracle as O
+    orc = O.Oracle(p)
+    cores = os.cpu_count() or 1
+    per_step = 0.3e-6  # rough single-thread cost; only sizes the sample
+    n_k = int(min(p.K, max(cores, seconds_target / (per_step * p.M * p.T))))
+    t0 = time.perf_counter()
+    orc.rollout_costs(k_begin=0, k_end=n_k, n_threads=cores, want_L=False, want_xT=False)
+    dt = time.perf_counter() - t0
+    return {"value": n_k * p.M * p.T / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"samples k in [0,{n_k}) of {p.name} (K={p.K}, M={p.M}, T={p.T}): {n_k * p.M * p.T} "
+                      f"state-steps of O1 (sampling, nominal + noisy rollouts, CVaR) in {dt:.2f} s wall",
+            "seconds": dt}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores; each step is a bounded slice of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle as O
+    p = make_problem(args.workload)
+    orc = O.Oracle(p)
+    cores = os.cpu_count() or 1
+    n_k = min(p.K, 64 * cores)
+    units = n_k * p.M * p.T
+    for _ in range(args.warmup):
+        orc.rollout_costs(k_begin=0, k_end=n_k, n_threads=cores, want_L=False, want_xT=False)
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        orc.rollout_costs(iteration=i, k_begin=0, k_end=n_k, n_threads=cores, want_L=False, want_xT=False)
+    dt = time.perf_counter() - t0
+    value = units * args.steps / dt
+    sample = (f"each step = samples k in [0,{n_k}) of {p.name} ({units} state-steps of O1) on {cores} threads; "
+              f"the O2-O3 update needs all K samples and is not in the slice")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{p.name} K={p.K} M={p.M} T={p.T}", "slice": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2209_12842_b200.controller import RaMppi
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    p = make_problem(args.workload, rank)
+    ctl = RaMppi(p, device=local)
+    dev = ctl.device
+    d_x0 = ctl.tensor(p.x0)
+    v_init = ctl.tensor(p.v)
+    d_v = v_init.clone()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for i in range(args.warmup):
+        d_v.copy_(v_init)
+        ctl.step(d_x0, d_v, i)
+    barrier()
+
+    # ---- device-resident timing: one event pair per step on the launching stream, L2 flushed between
+    sampler = ClockSampler(local)
+    sampler.start()
+    starts = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    stops = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    barrier()
+    t_wall0 = time.perf_counter()
+    for i in range(args.steps):
+        d_v.copy_(v_init)
+        flush.zero_()
+        starts[i].record(stream)
+        ctl.step(d_x0, d_v, args.warmup + i)
+        stops[i].record(stream)
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    sampler.stop_flag = True
+    sampler.join()
+    ms = np.array([s.elapsed_time(e) for s, e in zip(starts, stops)])
+    total_ms = float(ms.sum())
+
+    # ---- roofline pass: event pair around the fused rollout kernel itself
+    ctl.enable_kernel_timing(True)
+    kms = []
+    for i in range(min(args.steps, 50)):
+        d_v.copy_(v_init)
+        flush.zero_()
+        ctl.step(d_x0, d_v, args.warmup + i)
+        kms.append(ctl.last_rollout_ms())
+    ctl.enable_kernel_timing(False)
+    kernel_ms = float(np.mean(kms))
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): H2D x0,v -> step -> D2H v+
+    h_x0 = torch.tensor(np.asarray(p.x0, dtype=np.float32)).pin_memory()
+    h_v0 = torch.tensor(np.asarray(p.v, dtype=np.float32)).pin_memory()
+    h_v = h_v0.clone().pin_memory()
+    for i in range(3):
+        h_v.copy_(h_v0)
+        ctl.step_host(h_x0, h_v, i)
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        h_v.copy_(h_v0)
+        ctl.step_host(h_x0, h_v, args.warmup + i)   # returns after the D2H copy of v+ has landed
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+
+    # ---- max over ranks
+    t = torch.tensor([total_ms, e2e_s * 1e3, kernel_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms, e2e_ms, kernel_ms = (float(x) for x in t.cpu())
+    units_step = p.state_steps
+    value = world * units_step * args.steps / (total_ms * 1e-3)
+    e2e_value = world * units_step * args.steps / (e2e_ms * 1e-3)
+
+    if rank == 0:
+        key = workload_key(args.workload)
+        ops = ALGO_OPS[key] * units_step
+        achieved = ops / (kernel_ms * 1e-3)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{p.name} K={p.K} M={p.M} T={p.T}", "baseline_config_index": int(key[1]),
+                       "l2_flush_between_steps": True, "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "noise_mode": "fused"},
+            "iterations_per_s": world * args.steps / (total_ms * 1e-3),
+            "wall_ms_per_step_incl_flush": 1e3 * t_wall / args.steps,
+            "clocks": sampler.summary(),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(4 * (p.nx + 2 * p.T)),
+                    "d2h_bytes_per_step": int(4 * 2 * p.T), "ms_per_step": e2e_ms / args.steps,
+                    "api": "ra_mppi_step_host (pinned host x0, v -> v+)"},
+            "gpu_launches": int(ctl.launches_per_step * args.steps),
+            "roofline": {"bound": "alu", "kernel": "noisy_rollout_kernel", "achieved": achieved / 1e12,
+                         "peak": ALU_PEAK_LANE_OPS / 1e12, "unit": "Tlane-op/s (FP32-lane issue slots; FFMA = 1)",
+                         "frac": achieved / ALU_PEAK_LANE_OPS, "traffic": None,
+                         "algorithmic_ops_per_state_step": ALGO_OPS[key], "kernel_ms": kernel_ms,
+                         "kernel_share_of_step": kernel_ms / (total_ms / args.steps),
+                         "peak_source": "derived: 148 SMs x 128 FP32 lanes x 1.965 GHz (DESIGN.md)"},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(p)
+        print(json.dumps(line))
+    ctl.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--workload", default="C3")
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -128,6 +128,18 @@ ra_status ra_mppi_plant_shift(ra_mppi_ctx* ctx, float* d_x0, float* d_v, float* 
 ra_status ra_mppi_closed_loop(ra_mppi_ctx* ctx, float* d_x0, float* d_v, uint64_t iteration0,
                               int32_t n_iter, float* d_log, float* h_ms, void* cuda_stream);
 
+/* ra_mppi_step with HOST buffers: h_x0 [n_x] and h_v [T,2] (in: v, out: v+) are copied to the
+ * context's device staging buffers, the step runs, v+ is copied back, and the call returns after
+ * the stream has drained.  Pinned host memory makes the copies asynchronous; pageable works.  */
+ra_status ra_mppi_step_host(ra_mppi_ctx* ctx, const float* h_x0, float* h_v, uint64_t iteration,
+                            void* cuda_stream);
+
+/* Kernel timing for roofline accounting: when enabled, every step / rollout_costs records a CUDA
+ * event pair around the fused rollout kernel on the launching stream.
+ * ra_mppi_last_rollout_ms waits for that pair and returns its milliseconds in *h_ms (HOST).   */
+ra_status ra_mppi_enable_kernel_timing(ra_mppi_ctx* ctx, int32_t enable);
+ra_status ra_mppi_last_rollout_ms(ra_mppi_ctx* ctx, float* h_ms);
+
 /* Raw generator access for parity tests: out[n,4] = Philox4x32-10(ctr[n,4], key(seed)).   */
 ra_status ra_mppi_philox(ra_mppi_ctx* ctx, const uint32_t* d_ctr, int32_t n, uint32_t* d_out,
                          void* cuda_stream);

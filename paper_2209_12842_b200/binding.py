@@ -53,6 +53,7 @@ class ra_mppi_env(C.Structure):
 
 EXPORTS = (
     "ra_mppi_create", "ra_mppi_step", "ra_mppi_rollout_costs", "ra_mppi_weights_update",
+    "ra_mppi_step_host", "ra_mppi_enable_kernel_timing", "ra_mppi_last_rollout_ms",
     "ra_mppi_export_costs_f64", "ra_mppi_plant_shift", "ra_mppi_closed_loop", "ra_mppi_philox", "ra_mppi_state_noise",
     "ra_mppi_launches_per_step", "ra_mppi_last_error", "ra_mppi_destroy",
 )
@@ -76,6 +77,9 @@ def load():
     L.ra_mppi_rollout_costs.argtypes = [vp, fp, fp, u64, fp, fp, fp, fp, fp, fp, vp]
     L.ra_mppi_weights_update.argtypes = [vp, fp, fp, fp, fp, fp, vp]
     L.ra_mppi_export_costs_f64.argtypes = [vp, vp, vp, vp]
+    L.ra_mppi_step_host.argtypes = [vp, vp, vp, u64, vp]
+    L.ra_mppi_enable_kernel_timing.argtypes = [vp, i32]
+    L.ra_mppi_last_rollout_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.ra_mppi_plant_shift.argtypes = [vp, fp, fp, fp, u64, vp]
     L.ra_mppi_closed_loop.argtypes = [vp, fp, fp, u64, i32, fp, C.POINTER(C.c_float), vp]
     L.ra_mppi_philox.argtypes = [vp, vp, i32, vp, vp]
@@ -164,6 +168,21 @@ def ra_mppi_rollout_costs(ctx, d_x0, d_v, iteration, d_S=None, d_cvar=None, d_S_
 def ra_mppi_weights_update(ctx, d_S_tilde, d_u, d_v_plus, d_w=None, d_stats=None, stream=0):
     _check(ctx, load().ra_mppi_weights_update(ctx, d_S_tilde, d_u, d_v_plus, d_w, d_stats, stream),
            "ra_mppi_weights_update")
+
+
+def ra_mppi_step_host(ctx, h_x0, h_v, iteration, stream=0):
+    """h_x0, h_v: host addresses (e.g. pinned torch tensor .data_ptr() or numpy .ctypes.data)."""
+    _check(ctx, load().ra_mppi_step_host(ctx, h_x0, h_v, int(iteration), stream), "ra_mppi_step_host")
+
+
+def ra_mppi_enable_kernel_timing(ctx, enable=True):
+    _check(ctx, load().ra_mppi_enable_kernel_timing(ctx, 1 if enable else 0), "ra_mppi_enable_kernel_timing")
+
+
+def ra_mppi_last_rollout_ms(ctx):
+    ms = C.c_float()
+    _check(ctx, load().ra_mppi_last_rollout_ms(ctx, C.byref(ms)), "ra_mppi_last_rollout_ms")
+    return float(ms.value)
 
 
 def ra_mppi_export_costs_f64(ctx, d_S64=None, d_S_tilde64=None, stream=0):

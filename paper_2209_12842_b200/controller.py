@@ -59,6 +59,18 @@ class RaMppi:
                                 ptr(out["u"]), self._stream())
         return out
 
+    def step_host(self, h_x0: torch.Tensor, h_v: torch.Tensor, iteration: int = 0):
+        """ra_mppi_step_host: h_x0 [nx], h_v [T,2] are HOST tensors (pinned for async copies); h_v <- v+."""
+        assert not h_x0.is_cuda and not h_v.is_cuda and h_v.is_contiguous() and h_v.dtype == torch.float32
+        B.ra_mppi_step_host(self.ctx, h_x0.data_ptr(), h_v.data_ptr(), iteration, self._stream())
+        return h_v
+
+    def enable_kernel_timing(self, enable=True):
+        B.ra_mppi_enable_kernel_timing(self.ctx, enable)
+
+    def last_rollout_ms(self):
+        return B.ra_mppi_last_rollout_ms(self.ctx)
+
     def costs_f64(self):
         """fp64 S and S~ of the most recent step / rollout_costs."""
         S = torch.empty(self.K, device=self.device, dtype=torch.float64)

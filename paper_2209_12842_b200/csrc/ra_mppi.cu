@@ -35,6 +35,10 @@ struct ra_mppi_ctx {
   float* d_w_mat = nullptr;
   LoopState* d_loop = nullptr;
   // closed-loop graph cache
+  // host-buffer staging (ra_mppi_step_host) and optional kernel timing
+  float* d_stage = nullptr;  // [nx + 2T]
+  bool timing = false;
+  cudaEvent_t ev_k0 = nullptr, ev_k1 = nullptr;
   cudaGraphExec_t graph_exec = nullptr;
   float *g_x0 = nullptr, *g_v = nullptr, *g_log = nullptr;
   std::string err;
@@ -220,7 +224,8 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
   const size_t KT = (size_t)cfg->K * cfg->T;
   if (dev_alloc(&c->d_u_raw, KT) != cudaSuccess || dev_alloc(&c->d_ce, KT) != cudaSuccess ||
       dev_alloc(&c->d_S, (size_t)cfg->K) != cudaSuccess || dev_alloc(&c->d_cvar, (size_t)cfg->K) != cudaSuccess ||
-      dev_alloc(&c->d_S_tilde, (size_t)cfg->K) != cudaSuccess || dev_alloc(&c->d_loop, 1) != cudaSuccess)
+      dev_alloc(&c->d_S_tilde, (size_t)cfg->K) != cudaSuccess || dev_alloc(&c->d_loop, 1) != cudaSuccess ||
+      dev_alloc(&c->d_stage, (size_t)(8 + 2 * cfg->T)) != cudaSuccess)
     return bail(RA_ENOMEM);
   p.u_raw = c->d_u_raw; p.ce = c->d_ce; p.S = c->d_S; p.cvar = c->d_cvar; p.S_tilde = c->d_S_tilde;
   if (cudaMemset(c->d_loop, 0, sizeof(LoopState)) != cudaSuccess) return bail(RA_ECUDA);
@@ -240,6 +245,9 @@ ra_status ra_mppi_destroy(ra_mppi_ctx* c) {
   cudaSetDevice(c->cfg.device);
   if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
   cudaFree(c->d_circles); cudaFree(c->d_costmap); cudaFree(c->d_u_raw); cudaFree(c->d_ce);
+  cudaFree(c->d_stage);
+  if (c->ev_k0) cudaEventDestroy(c->ev_k0);
+  if (c->ev_k1) cudaEventDestroy(c->ev_k1);
   cudaFree(c->d_S); cudaFree(c->d_cvar); cudaFree(c->d_S_tilde); cudaFree(c->d_w_mat); cudaFree(c->d_loop);
   delete c;
   return RA_OK;
@@ -282,7 +290,9 @@ ra_status enqueue_costs(ra_mppi_ctx* c, const Params& p, const float* d_x0, cons
   if (c->cfg.noise_mode == RA_NOISE_MATERIALISED)
     RA_CUDA(c, p.nx == 4 ? launch_materialise<4>(c, p, s) : launch_materialise<6>(c, p, s));
   RA_CUDA(c, launch_sample_nominal(c, p, d_x0, d_v, s));
+  if (c->timing) RA_CUDA(c, cudaEventRecord(c->ev_k0, s));
   RA_CUDA(c, c->rollout(p, c->noise_variant, c->rc, c->half, d_x0, d_L, d_xT, s));
+  if (c->timing) RA_CUDA(c, cudaEventRecord(c->ev_k1, s));
   return RA_OK;
 }
 
@@ -361,6 +371,39 @@ ra_status ra_mppi_plant_shift(ra_mppi_ctx* c, float* d_x0, float* d_v, float* d_
   if (!d_x0 || !d_v) return fail(c, RA_EINVAL, "null device pointer");
   const Params p = with_iteration(c, iteration);
   RA_CUDA(c, launch_plant(c, p, d_x0, d_v, d_u_applied, nullptr, nullptr, static_cast<cudaStream_t>(stream)));
+  return RA_OK;
+}
+
+ra_status ra_mppi_step_host(ra_mppi_ctx* c, const float* h_x0, float* h_v, uint64_t iteration, void* stream) {
+  if (!c) return RA_EINVAL;
+  if (!h_x0 || !h_v) return fail(c, RA_EINVAL, "null host pointer");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  float* d_x0 = c->d_stage;
+  float* d_v = c->d_stage + 8;
+  const size_t nv = (size_t)2 * c->p.T * sizeof(float);
+  RA_CUDA(c, cudaMemcpyAsync(d_x0, h_x0, (size_t)c->p.nx * sizeof(float), cudaMemcpyHostToDevice, s));
+  RA_CUDA(c, cudaMemcpyAsync(d_v, h_v, nv, cudaMemcpyHostToDevice, s));
+  if (ra_status st = ra_mppi_step(c, d_x0, d_v, iteration, stream)) return st;
+  RA_CUDA(c, cudaMemcpyAsync(h_v, d_v, nv, cudaMemcpyDeviceToHost, s));
+  RA_CUDA(c, cudaStreamSynchronize(s));
+  return RA_OK;
+}
+
+ra_status ra_mppi_enable_kernel_timing(ra_mppi_ctx* c, int32_t enable) {
+  if (!c) return RA_EINVAL;
+  if (enable && !c->ev_k0) {
+    RA_CUDA(c, cudaEventCreate(&c->ev_k0));
+    RA_CUDA(c, cudaEventCreate(&c->ev_k1));
+  }
+  c->timing = enable != 0;
+  return RA_OK;
+}
+
+ra_status ra_mppi_last_rollout_ms(ra_mppi_ctx* c, float* h_ms) {
+  if (!c) return RA_EINVAL;
+  if (!h_ms || !c->ev_k0) return fail(c, RA_EINVAL, "kernel timing was never enabled");
+  RA_CUDA(c, cudaEventSynchronize(c->ev_k1));
+  RA_CUDA(c, cudaEventElapsedTime(h_ms, c->ev_k0, c->ev_k1));
   return RA_OK;
 }
 

@@ -49,7 +49,7 @@ __device__ __forceinline__ void sincospi_quarter(float r, float& s, float& c) {
 }
 
 // Box-Muller pair from two Philox words.  u1 = ((ra>>9)+1) 2^-23 in (0,1], u2 = (rb>>9) 2^-23
-// in [0,1) are exact in fp32, so this starts from the same reals as the fp64 oracle.
+// in [0,1) are exact in fp32, so the transform starts from exact reals.
 // The angle 2 pi u2 is reduced exactly in integers: n = rb>>9 in [0,2^23), quadrant q and
 // remainder r = u2*2... in [-1/4,1/4] half-turns, then polynomials (no MUFU sin/cos).
 __device__ __forceinline__ void box_muller(uint32_t ra, uint32_t rb, float& z0, float& z1) {

@@ -1,0 +1,117 @@
+"""Closed-loop glue (A10) and host-buffer entry point, through the C ABI (pytest -m gpu).
+
+The 500-iteration trajectory is not compared as a whole (feedback amplifies rounding):
+parity is teacher-forced -- at chosen iterations the GPU's (x0, v, iteration) is handed to the
+oracle and that single step is compared.
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2209_12842_b200 import workloads as W
+
+from parity_utils import TOL_STATE_ABS, TOL_V_ABS, check_rollout_parity, check_step_parity
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2209_12842_b200 import build
+    build.build()
+    return torch
+
+
+def _ctl(p):
+    from paper_2209_12842_b200.controller import RaMppi
+    return RaMppi(p, device=0)
+
+
+@pytest.mark.parametrize("cfg", ["bicycle", "single_track"])
+def test_plant_and_shift(torch_cuda, cfg):
+    torch = torch_cuda
+    p = W.small(W.config4(), K=64, M=32, T=17) if cfg == "bicycle" else W.small(W.config2(), K=32, M=32, T=9)
+    ctl, orc = _ctl(p), O.Oracle(p)
+    v = W.random_mean_control(p, 3, (0.3, 4.0))          # includes values beyond the clamps
+    d_x0, d_v = ctl.tensor(p.x0), ctl.tensor(v)
+    for it in (0, 7, 499):
+        x_before = d_x0.cpu().numpy().astype(np.float64)
+        v_before = d_v.cpu().numpy().astype(np.float64)
+        u = ctl.plant_shift(d_x0, d_v, it)
+        torch.cuda.synchronize()
+        assert np.array_equal(u.cpu().numpy(), v_before[0].astype(np.float32))        # applied control = v+_0
+        ref_x = orc.plant_step(x_before, v_before[0], it)
+        assert np.abs(d_x0.cpu().numpy() - ref_x).max() < 1e-5
+        assert np.array_equal(d_v.cpu().numpy(), O.shift(v_before).astype(np.float32))  # warm-start shift, exact
+
+
+def test_closed_loop_graph_teacher_forced(torch_cuda):
+    torch = torch_cuda
+    p = W.small(W.config4(), K=512, M=64, T=50)
+    ctl, orc = _ctl(p), O.Oracle(p)
+    n_iter, it0 = 40, 3
+    d_x0, d_v = ctl.tensor(p.x0), ctl.tensor(np.zeros((p.T, 2)))
+    log, ms = ctl.closed_loop(d_x0, d_v, it0, n_iter)
+    torch.cuda.synchronize()
+    log = log.cpu().numpy()
+    assert ms.shape == (n_iter,) and (ms > 0).all()
+    assert np.isfinite(log).all()
+    assert np.array_equal(log[-1, :4], d_x0.cpu().numpy())
+    # the graph replay equals the same sequence issued call by call (same kernels, same counters)
+    e_x0, e_v = ctl.tensor(p.x0), ctl.tensor(np.zeros((p.T, 2)))
+    checkpoints = {}
+    for i in range(n_iter):
+        if i in (0, 1, 2, 10, n_iter - 1):
+            checkpoints[i] = (e_x0.cpu().numpy().astype(np.float64), e_v.cpu().numpy().astype(np.float64))
+        ctl.step(e_x0, e_v, it0 + i)
+        u = ctl.plant_shift(e_x0, e_v, it0 + i)
+        torch.cuda.synchronize()
+        assert np.array_equal(log[i, :4], e_x0.cpu().numpy()), i
+        assert np.array_equal(log[i, 4:], u.cpu().numpy()), i
+    assert np.array_equal(e_v.cpu().numpy(), d_v.cpu().numpy())
+    # teacher-forced single steps against the oracle
+    for i, (x0, v) in checkpoints.items():
+        g, r = check_rollout_parity(p, ctl, orc, iteration=it0 + i, x0=x0, v=v, k_begin=0, k_end=96)
+        rf = orc.rollout_costs(x0=x0, v=v, iteration=it0 + i, n_threads=8, want_L=False, want_xT=False)
+        verdict, err = check_step_parity(p, ctl, orc, rf, iteration=it0 + i, x0=x0, v=v)
+        print(f"iteration {it0 + i}: v+ {verdict}")
+    # the car makes progress along the track and stays near the lane
+    assert np.hypot(log[-1, 0] - p.x0[0], log[-1, 1] - p.x0[1]) > 2.0
+    # second call re-uses the cached graph and restarts the counter
+    d_x0b, d_vb = ctl.tensor(p.x0), ctl.tensor(np.zeros((p.T, 2)))
+    d_x0.copy_(d_x0b); d_v.copy_(d_vb)
+    log2, _ = ctl.closed_loop(d_x0, d_v, it0, n_iter)
+    torch.cuda.synchronize()
+    assert np.array_equal(log2.cpu().numpy(), log)
+
+
+def test_step_host_equals_step(torch_cuda):
+    torch = torch_cuda
+    p = W.small(W.config3(), K=256, M=128, T=50)
+    p = p.replace(v=W.random_mean_control(p, 1))
+    ctl = _ctl(p)
+    d_x0, d_v = ctl.tensor(p.x0), ctl.tensor(p.v)
+    ctl.step(d_x0, d_v, 5)
+    torch.cuda.synchronize()
+    h_x0 = torch.tensor(np.asarray(p.x0, dtype=np.float32)).pin_memory()
+    h_v = torch.tensor(np.asarray(p.v, dtype=np.float32)).pin_memory()
+    ctl.step_host(h_x0, h_v, 5)
+    assert np.array_equal(h_v.numpy(), d_v.cpu().numpy())
+    # pageable numpy memory works too
+    h_v2 = torch.tensor(np.asarray(p.v, dtype=np.float32))
+    ctl.step_host(torch.tensor(np.asarray(p.x0, dtype=np.float32)), h_v2, 5)
+    assert np.array_equal(h_v2.numpy(), d_v.cpu().numpy())
+
+
+def test_kernel_timing_hook(torch_cuda):
+    torch = torch_cuda
+    p = W.small(W.config3(), K=1024, M=128, T=50)
+    ctl = _ctl(p)
+    d_x0, d_v = ctl.tensor(p.x0), ctl.tensor(p.v)
+    ctl.enable_kernel_timing(True)
+    ctl.step(d_x0, d_v, 0)
+    ms = ctl.last_rollout_ms()
+    assert 0.0 < ms < 100.0
+    assert ctl.launches_per_step == 3
