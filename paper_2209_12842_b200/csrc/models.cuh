@@ -13,7 +13,10 @@ __device__ __forceinline__ float clampf(float x, float lo, float hi) { return fm
 // sin/cos by three-term Cody-Waite reduction to [-pi/4, pi/4] and FMA-pipe polynomials.
 // Valid (<= 2 ulp) for |x| < ~6000 rad; yaw angles here stay within a few turns.
 __device__ __forceinline__ void sincos_cw(float x, float& s, float& c) {
-  const float j = rintf(x * 0.636619747f);
+  // round-to-nearest by the 1.5*2^23 trick (FMA pipe; no FRND/F2I on the XU pipe): the low mantissa
+  // bits of jm hold the integer, valid for |x| < 2^21 quarter-turns
+  const float jm = fmaf(x, 0.636619747f, 12582912.0f);
+  const float j = jm - 12582912.0f;
   float r = fmaf(j, -1.5703125f, x);
   r = fmaf(j, -4.837512969970703e-4f, r);
   r = fmaf(j, -7.549790126404332e-8f, r);
@@ -28,7 +31,7 @@ __device__ __forceinline__ void sincos_cw(float x, float& s, float& c) {
   pc = fmaf(pc, r2, 4.16666667e-2f);    //  1/4!
   pc = fmaf(pc, r2, -0.5f);
   const float cr = fmaf(pc, r2, 1.0f);
-  const int q = (int)j;
+  const int q = __float_as_int(jm);
   const float cs = (q & 1) ? -sr : cr;
   const float sn = (q & 1) ? cr : sr;
   c = (q & 2) ? -cs : cs;
@@ -107,38 +110,39 @@ __device__ __forceinline__ float nominal_cost(const Params& p, float Xabs, float
   }
 }
 
-// Bilinear costmap lookup between cell centres with clamp-to-edge.  The grid coordinate is
-// split as (integer bias) + (fractional bias + X_rel / res) so the fraction keeps full
-// precision wherever the vehicle is on the map.
+// Bilinear costmap lookup between cell centres with clamp-to-edge (G26).
+// Layout: the context stores the map as a "quad" grid Q[(H+1)][(W+1)] of float4, where
+// Q[jy][jx] = (c[jy-1][jx-1], c[jy-1][jx], c[jy][jx-1], c[jy][jx]) with indices clamped to the map, so
+// one 16-byte load fetches the four texels of a lookup and clamp-to-edge is baked into the table;
+// only the coordinate is clamped (to [0, W] in the +1-shifted grid).  The grid coordinate is split as
+// (integer bias) + (fractional bias + X_rel / res) so the fraction keeps full precision wherever
+// the vehicle is on the map.
 struct MapFrame {
-  float bxf, byf;  // fractional part of (x0 - origin)/res - 1/2
-  int bxi, byi;    // integer part
+  float bxf, byf;            // fractional part of (x0 - origin)/res + 1/2
+  float lox, hix, loy, hiy;  // clamp bounds of the fractional-frame coordinate
+  int base;                  // (integer bias y) * (W+1) + (integer bias x)
 };
 
 __device__ __forceinline__ MapFrame make_map_frame(const Params& p, float x0X, float x0Y) {
   MapFrame f;
-  const float bx = fmaf(x0X - p.map_ox, p.map_inv_res, -0.5f);
-  const float by = fmaf(x0Y - p.map_oy, p.map_inv_res, -0.5f);
+  const float bx = fmaf(x0X - p.map_ox, p.map_inv_res, 0.5f);
+  const float by = fmaf(x0Y - p.map_oy, p.map_inv_res, 0.5f);
   const float fx = floorf(bx), fy = floorf(by);
   f.bxf = bx - fx; f.byf = by - fy;
-  f.bxi = (int)fx; f.byi = (int)fy;
+  f.lox = -fx; f.hix = (float)p.map_w - fx;
+  f.loy = -fy; f.hiy = (float)p.map_h - fy;
+  f.base = (int)fy * (p.map_w + 1) + (int)fx;
   return f;
 }
 
 __device__ __forceinline__ float bilinear(const Params& p, const MapFrame& f, float Xrel, float Yrel) {
-  const float gx = fmaf(Xrel, p.map_inv_res, f.bxf);
-  const float gy = fmaf(Yrel, p.map_inv_res, f.byf);
-  const float flx = floorf(gx), fly = floorf(gy);
-  const float tx = gx - flx, ty = gy - fly;
-  const int ix = (int)flx + f.bxi, iy = (int)fly + f.byi;
-  const int ix0 = min(max(ix, 0), p.map_w - 1), ix1 = min(max(ix + 1, 0), p.map_w - 1);
-  const int iy0 = min(max(iy, 0), p.map_h - 1), iy1 = min(max(iy + 1, 0), p.map_h - 1);
-  const float* r0 = p.costmap + (size_t)iy0 * p.map_w;
-  const float* r1 = p.costmap + (size_t)iy1 * p.map_w;
-  const float c00 = __ldg(r0 + ix0), c01 = __ldg(r0 + ix1);
-  const float c10 = __ldg(r1 + ix0), c11 = __ldg(r1 + ix1);
-  const float top = fmaf(tx, c01 - c00, c00);
-  const float bot = fmaf(tx, c11 - c10, c10);
+  const float gx = fminf(fmaxf(fmaf(Xrel, p.map_inv_res, f.bxf), f.lox), f.hix);
+  const float gy = fminf(fmaxf(fmaf(Yrel, p.map_inv_res, f.byf), f.loy), f.hiy);
+  const int ix = __float2int_rd(gx), iy = __float2int_rd(gy);
+  const float tx = gx - __int2float_rn(ix), ty = gy - __int2float_rn(iy);
+  const float4 q = __ldg(p.quadmap + (f.base + iy * (p.map_w + 1) + ix));
+  const float top = fmaf(tx, q.y - q.x, q.x);
+  const float bot = fmaf(tx, q.w - q.z, q.z);
   return fmaf(ty, bot - top, top);
 }
 

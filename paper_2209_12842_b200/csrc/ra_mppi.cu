@@ -26,7 +26,7 @@ struct ra_mppi_ctx {
   RolloutLaunchFn rollout = nullptr;
   // device allocations owned by the context
   float4* d_circles = nullptr;
-  float* d_costmap = nullptr;
+  float4* d_costmap = nullptr;  // quad-texel table
   float2* d_u_raw = nullptr;
   float4* d_ce = nullptr;
   double* d_S = nullptr;
@@ -211,11 +211,22 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
     p.circles = c->d_circles;
   }
   if (cfg->risk == RA_RISK_COSTMAP) {
-    const size_t n = (size_t)env->map_h * env->map_w;
+    // quad-texel table (models.cuh): Q[jy][jx] = the four texels around grid corner (jx-1/2, jy-1/2)
+    const int H = env->map_h, Wd = env->map_w;
+    const size_t n = (size_t)(H + 1) * (Wd + 1);
+    std::vector<float4> q(n);
+    auto at = [&](int iy, int ix) {
+      iy = iy < 0 ? 0 : (iy > H - 1 ? H - 1 : iy);
+      ix = ix < 0 ? 0 : (ix > Wd - 1 ? Wd - 1 : ix);
+      return env->costmap[(size_t)iy * Wd + ix];
+    };
+    for (int jy = 0; jy <= H; ++jy)
+      for (int jx = 0; jx <= Wd; ++jx)
+        q[(size_t)jy * (Wd + 1) + jx] = make_float4(at(jy - 1, jx - 1), at(jy - 1, jx), at(jy, jx - 1), at(jy, jx));
     if (cuda_fail(c, dev_alloc(&c->d_costmap, n), "alloc costmap")) return bail(RA_ENOMEM);
-    if (cudaMemcpy(c->d_costmap, env->costmap, n * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess)
+    if (cudaMemcpy(c->d_costmap, q.data(), n * sizeof(float4), cudaMemcpyHostToDevice) != cudaSuccess)
       return bail(RA_ECUDA);
-    p.costmap = c->d_costmap;
+    p.quadmap = c->d_costmap;
     p.map_h = env->map_h; p.map_w = env->map_w;
     p.map_inv_res = (float)(1.0 / (double)env->map_res);
     p.map_ox = env->map_ox; p.map_oy = env->map_oy;

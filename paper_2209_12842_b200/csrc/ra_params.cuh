@@ -36,7 +36,7 @@ struct Params {
   // environment (device copies owned by the context)
   const float4* circles;  // [n] absolute (cx, cy, r + margin, unused)
   int n_circles;
-  const float* costmap;
+  const float4* quadmap;  // [(map_h+1)][(map_w+1)] texel quads, clamp-to-edge baked in
   int map_h, map_w;
   float map_inv_res, map_ox, map_oy;
   // scratch owned by the context

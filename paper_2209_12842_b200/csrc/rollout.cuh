@@ -150,8 +150,14 @@ __device__ __forceinline__ void risk_accumulate(const Params& p, const float4* c
 // A3-A7.  HALF: two control samples per warp (G = 16 lanes each, M <= 16).
 // Dynamic shared memory: [n_circles] float4 obstacle records, then per warp R_total*32 keys.
 // ---------------------------------------------------------------------------------------
+#ifndef RA_MIN_CTAS_BICYCLE
+#define RA_MIN_CTAS_BICYCLE 4   // 64 registers / thread: 32 resident warps per SM
+#endif
+#ifndef RA_MIN_CTAS_SINGLE_TRACK
+#define RA_MIN_CTAS_SINGLE_TRACK 2
+#endif
 template <int DYN, int RISK, int NOISE, int RC, bool HALF>
-__global__ void __launch_bounds__(kRolloutThreads)
+__global__ void __launch_bounds__(kRolloutThreads, DYN == DYN_BICYCLE ? RA_MIN_CTAS_BICYCLE : RA_MIN_CTAS_SINGLE_TRACK)
 noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__ x0g,
                      float* __restrict__ L_out, float* __restrict__ xT_out) {
   constexpr int NX = StateDim<DYN>::value;

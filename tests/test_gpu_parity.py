@@ -64,8 +64,17 @@ def test_state_noise_draws(torch_cuda, cfg):
     ref = np.array([orc.state_noise(int(k), int(m), int(t), 1, 3) for k, m, t in kmt])
     sig = np.asarray(p.sigma_w)[: p.nx]
     z, zr = w / sig, ref / sig
-    err = np.abs(z - zr) / np.maximum(1.0, np.abs(zr))
-    assert err.max() < 2e-6, err.max()   # a few fp32 ulp on the normal (parity stage 2)
+    if cfg == "uniform":
+        assert np.abs(z - zr).max() < 2e-7            # exact uniforms, one rounding
+    elif cfg == "jump":
+        assert np.abs(z - zr).max() < 2e-5            # unit direction through the fast normals
+        assert np.array_equal(z == 0, zr == 0)        # same trigger decisions (exact uniform compare)
+    else:
+        # MUFU-based Box-Muller: |dz| <= 4e-6 max(1,|z|) + 4e-7 / max(rho, 1e-3)
+        rho = np.sqrt((zr.reshape(len(zr), -1, 2) ** 2).sum(-1, keepdims=True)).repeat(2, -1).reshape(zr.shape)
+        bound = 4e-6 * np.maximum(1.0, np.abs(zr)) + 4e-7 / np.maximum(rho, 1e-3)
+        assert (np.abs(z - zr) <= bound).all(), (np.abs(z - zr) / bound).max()
+        print(f"{cfg}: max |dz| = {np.abs(z - zr).max():.2e}, max |dz|/bound = {(np.abs(z - zr) / bound).max():.2f}")
 
 
 # ------------------------------------------------------------------ rollouts, costs, CVaR, update
