@@ -31,9 +31,9 @@ UNIT = "state-steps/s"
 # Algorithmic lane-operations per noisy state-step: the instructions the
 # method itself needs (Philox, normal transform, dynamics, risk cost), one per FP32-lane slot.
 #   Philox4x32-10 call 40 (20 mul-wide + 20 xor3); Box-Muller 14 per pair + 1 scale-add per normal;
-#   bicycle step 7; single-track step 75; circle test 5 per obstacle; bilinear lookup 21.
-ALGO_OPS = {"C0": 40 + 32 + 7 + 5 * 8, "C1": 40 + 32 + 7 + 5 * 32, "C2": 80 + 48 + 75 + 5 * 128,
-            "C3": 40 + 32 + 7 + 21, "C4": 40 + 32 + 7 + 5 * 64}
+#   bicycle step 7; single-track step 75; bilinear lookup 21.  Circle tests are NOT credited: far
+#   obstacles are culled exactly, and a culled test is not achieved work.
+ALGO_OPS = {"C0": 40 + 32 + 7, "C1": 40 + 32 + 7, "C2": 80 + 48 + 75, "C3": 40 + 32 + 7 + 21, "C4": 40 + 32 + 7}
 ALU_PEAK_LANE_OPS = 148 * 128 * 1.965e9  # 148 SMs x 128 FP32 lanes x 1.965 GHz (B200_PROFILING.md nominal)
 
 

@@ -111,22 +111,60 @@ __device__ __forceinline__ float cvar_select(const uint32_t* keys, int R_total, 
   return fmaf((float)k_rem, key_float(prefix), sum_gt) / (float)k_tail;
 }
 
+// Warp-wide float min / max in one instruction: redux.sync.{min,max}.f32 (sm_100a; SASS CREDUX).
+__device__ __forceinline__ float warp_min_f32(float v) {
+  float r;
+  asm volatile("redux.sync.min.f32 %0, %1, 0xffffffff;" : "=f"(r) : "f"(v));
+  return r;
+}
+__device__ __forceinline__ float warp_max_f32(float v) {
+  float r;
+  asm volatile("redux.sync.max.f32 %0, %1, 0xffffffff;" : "=f"(r) : "f"(v));
+  return r;
+}
+
 // Risk running cost l(x~) (9) PAPER.md:93 for RC interleaved realisations of one lane.
 template <int RISK, int RC, int NX>
 __device__ __forceinline__ void risk_accumulate(const Params& p, const float4* circ_s,
                                                 const MapFrame& mf, float x0X, float x0Y,
                                                 const float (&x)[RC][NX], float (&L)[RC]) {
   if constexpr (RISK == RISK_CIRCLES) {
+    // Exact culling: the lanes of a warp share u^k and start together, so they stay within a
+    // few metres.  Once per step the warp takes the bounding box of all its positions (four
+    // warp-wide CREDUX.F32), each lane tests one obstacle of a 32-obstacle batch against the box
+    // (inflated by 1e-4 so fp32 rounding can only add candidates), and every lane then evaluates
+    // only the balloted candidates.  A culled obstacle contributes exactly 0 to every lane.
     const float w = p.risk_p[0];
-    for (int i = 0; i < p.n_circles; ++i) {
-      const float4 c = circ_s[i];  // (cx - x0X, cy - x0Y, r + margin, (r + margin)^2), broadcast
+    float lox = x[0][0], hix = x[0][0], loy = x[0][1], hiy = x[0][1];
 #pragma unroll
-      for (int r = 0; r < RC; ++r) {
-        const float dx = x[r][0] - c.x, dy = x[r][1] - c.y;
-        const float d2 = fmaf(dx, dx, dy * dy);
-        if (d2 < c.w) {
-          const float pen = c.z - sqrtf(d2);
-          L[r] = fmaf(w * pen, pen, L[r]);
+    for (int r = 1; r < RC; ++r) {
+      lox = fminf(lox, x[r][0]); hix = fmaxf(hix, x[r][0]);
+      loy = fminf(loy, x[r][1]); hiy = fmaxf(hiy, x[r][1]);
+    }
+    lox = warp_min_f32(lox); hix = warp_max_f32(hix);
+    loy = warp_min_f32(loy); hiy = warp_max_f32(hiy);
+    const int lane = threadIdx.x & 31;
+    for (int base = 0; base < p.n_circles; base += 32) {
+      const int j = base + lane;
+      bool near = false;
+      if (j < p.n_circles) {
+        const float4 c = circ_s[j];  // (cx - x0X, cy - x0Y, r + margin, (r + margin)^2)
+        const float ddx = fmaxf(fmaxf(lox - c.x, c.x - hix), 0.0f);
+        const float ddy = fmaxf(fmaxf(loy - c.y, c.y - hiy), 0.0f);
+        near = fmaf(ddx, ddx, ddy * ddy) < c.w * 1.0001f;
+      }
+      uint32_t cand = __ballot_sync(0xFFFFFFFFu, near);
+      while (cand) {
+        const float4 c = circ_s[base + __ffs(cand) - 1];  // broadcast
+        cand &= cand - 1u;
+#pragma unroll
+        for (int r = 0; r < RC; ++r) {
+          const float dx = x[r][0] - c.x, dy = x[r][1] - c.y;
+          const float d2 = fmaf(dx, dx, dy * dy);
+          if (d2 < c.w) {
+            const float pen = c.z - sqrtf(d2);
+            L[r] = fmaf(w * pen, pen, L[r]);
+          }
         }
       }
     }
