@@ -38,6 +38,29 @@ __device__ __forceinline__ void sincos_cw(float x, float& s, float& c) {
   s = (q & 2) ? -sn : sn;
 }
 
+// atan2(y, x) for x > 0 (the single-track model floors vx at a positive value): one MUFU.RCP and
+// a degree-8 odd polynomial in z = min(|y|,x)/max(|y|,x) (max error 1.3e-7 rad in fp32, fitted on
+// Chebyshev nodes; the linear coefficient is exactly 1 so small slip angles keep relative accuracy).
+__device__ __forceinline__ float atan2_posx(float y, float x) {
+  const float ay = fabsf(y);
+  const float den = fmaxf(ay, x);
+  float inv;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(inv) : "f"(den));
+  const float z = fminf(ay, x) * inv;
+  const float s = z * z;
+  float p = 0.0028340641874819994f;
+  p = fmaf(p, s, -0.016005029901862144f);
+  p = fmaf(p, s, 0.042587608098983765f);
+  p = fmaf(p, s, -0.07495445758104324f);
+  p = fmaf(p, s, 0.10636754333972931f);
+  p = fmaf(p, s, -0.14202570915222168f);
+  p = fmaf(p, s, 0.19992484152317047f);
+  p = fmaf(p, s, -0.3333306610584259f);
+  p = fmaf(p * s, z, z);                       // z (1 + s P(s))
+  const float r = (ay > x) ? 1.57079632679489662f - p : p;
+  return copysignf(r, y);
+}
+
 // Control effects: everything F needs from u^k_t that is the same for all M realisations,
 // computed once per (k,t) by the sampling kernel.
 //   bicycle:       (dt tan(delta_c)/L, dt a_c, -, -)
@@ -70,11 +93,11 @@ __device__ __forceinline__ void dynamics_step(const Params& p, float (&x)[StateD
     x[2] = fmaf(x[3], ce.x, x[2]);
     x[3] = x[3] + ce.y;
   } else {
-    const float m_inv = 1.0f / p.dyn_p[0], iz_inv = 1.0f / p.dyn_p[1];
+    const float m_inv = p.dyn_q[0], iz_inv = p.dyn_q[1];  // 1/m, 1/Iz (host-computed)
     const float lf = p.dyn_p[2], lr = p.dyn_p[3], Cf = p.dyn_p[4], Cr = p.dyn_p[5];
     const float vx = x[3], vy = x[4], r = x[5];
-    const float alpha_f = ce.x - atan2f(fmaf(lf, r, vy), vx);
-    const float alpha_r = -atan2f(fmaf(-lr, r, vy), vx);
+    const float alpha_f = ce.x - atan2_posx(fmaf(lf, r, vy), vx);   // vx >= vx_floor > 0
+    const float alpha_r = -atan2_posx(fmaf(-lr, r, vy), vx);
     const float Fyf = Cf * alpha_f, Fyr = Cr * alpha_r;
     const float vx_dot = fmaf(vy, r, (ce.y - Fyf * ce.z) * m_inv);
     const float vy_dot = fmaf(-vx, r, fmaf(Fyf, ce.w, Fyr) * m_inv);

@@ -176,9 +176,16 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
   p.G = c->half ? 16 : 32;
   p.R_total = (cfg->M + p.G - 1) / p.G;
   c->rc = c->half ? 1 : (p.R_total % 4 == 0 ? 4 : (p.R_total % 2 == 0 ? 2 : 1));
+#ifdef RA_FORCE_RC  // tuning experiments only
+  if (!c->half && p.R_total % RA_FORCE_RC == 0) c->rc = RA_FORCE_RC;
+#endif
   p.nx = cfg->dyn == RA_DYN_SINGLE_TRACK ? 6 : 4;
   p.dt = cfg->dt;
   std::memcpy(p.dyn_p, cfg->dyn_p, sizeof p.dyn_p);
+  if (cfg->dyn == RA_DYN_SINGLE_TRACK) {
+    p.dyn_q[0] = (float)(1.0 / (double)cfg->dyn_p[0]);
+    p.dyn_q[1] = (float)(1.0 / (double)cfg->dyn_p[1]);
+  }
   std::memcpy(p.nom_p, cfg->nom_p, sizeof p.nom_p);
   std::memcpy(p.risk_p, cfg->risk_p, sizeof p.risk_p);
   std::memcpy(p.noise_p, cfg->noise_p, sizeof p.noise_p);

@@ -22,6 +22,7 @@ struct Params {
   int nx;
   float dt;
   float dyn_p[8];
+  float dyn_q[2];   // single-track: 1/m, 1/Iz
   float u_min[2], u_max[2];
   float sigma_eps[2];
   float ctrl_w[2];  // gamma / sigma_eps^2 (0 where sigma_eps == 0)   (3) PAPER.md:47

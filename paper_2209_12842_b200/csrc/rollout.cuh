@@ -162,7 +162,9 @@ __device__ __forceinline__ void risk_accumulate(const Params& p, const float4* c
           const float dx = x[r][0] - c.x, dy = x[r][1] - c.y;
           const float d2 = fmaf(dx, dx, dy * dy);
           if (d2 < c.w) {
-            const float pen = c.z - sqrtf(d2);
+            float d;
+            asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(d) : "f"(d2));  // 1 ulp; pen = R - d
+            const float pen = c.z - d;
             L[r] = fmaf(w * pen, pen, L[r]);
           }
         }
@@ -189,10 +191,10 @@ __device__ __forceinline__ void risk_accumulate(const Params& p, const float4* c
 // Dynamic shared memory: [n_circles] float4 obstacle records, then per warp R_total*32 keys.
 // ---------------------------------------------------------------------------------------
 #ifndef RA_MIN_CTAS_BICYCLE
-#define RA_MIN_CTAS_BICYCLE 4   // 64 registers / thread: 32 resident warps per SM
+#define RA_MIN_CTAS_BICYCLE 3   // measured: 3 CTAs (<= 80 regs) beats 4-6 (throughput-, not latency-bound)
 #endif
 #ifndef RA_MIN_CTAS_SINGLE_TRACK
-#define RA_MIN_CTAS_SINGLE_TRACK 2
+#define RA_MIN_CTAS_SINGLE_TRACK 3
 #endif
 template <int DYN, int RISK, int NOISE, int RC, bool HALF>
 __global__ void __launch_bounds__(kRolloutThreads, DYN == DYN_BICYCLE ? RA_MIN_CTAS_BICYCLE : RA_MIN_CTAS_SINGLE_TRACK)
