@@ -34,6 +34,8 @@ UNIT = "state-steps/s"
 #   bicycle step 7; single-track step 75; bilinear lookup 21.  Circle tests are NOT credited: far
 #   obstacles are culled exactly, and a culled test is not achieved work.
 ALGO_OPS = {"C0": 40 + 32 + 7, "C1": 40 + 32 + 7, "C2": 80 + 48 + 75, "C3": 40 + 32 + 7 + 21, "C4": 40 + 32 + 7}
+# DRAM bytes (read + write) of one noisy_rollout_kernel launch, from the committed `ncu --set full` captures
+TRAFFIC_BYTES = {"C3": 13.41e6, "C2": 7.97e6}   # profiles/r1b_c3_c2_optimised.md
 ALU_PEAK_LANE_OPS = 148 * 128 * 1.965e9  # 148 SMs x 128 FP32 lanes x 1.965 GHz (B200_PROFILING.md nominal)
 
 
@@ -95,12 +97,12 @@ class ClockSampler(threading.Thread):
                 "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
-def cpu_baseline(p: W.Problem, seconds_target: float = 15.0):
+def cpu_baseline(p: W.Problem, seconds_target: float = 20.0):
     """The oracle as it stands, timed on the host cores on a bounded slice of the same workload."""
     from oracle import oracle as O
     orc = O.Oracle(p)
     cores = os.cpu_count() or 1
-    per_step = 0.3e-6  # rough single-thread cost; only sizes the sample
+    per_step = 0.2e-6  # rough single-thread cost per state-step; only sizes the sample (CPU-seconds of work)
     n_k = int(min(p.K, max(cores, seconds_target / (per_step * p.M * p.T))))
     t0 = time.perf_counter()
     orc.rollout_costs(k_begin=0, k_end=n_k, n_threads=cores, want_L=False, want_xT=False)
@@ -109,6 +111,21 @@ def cpu_baseline(p: W.Problem, seconds_target: float = 15.0):
             "sample": f"samples k in [0,{n_k}) of {p.name} (K={p.K}, M={p.M}, T={p.T}): {n_k * p.M * p.T} "
                       f"state-steps of O1 (sampling, nominal + noisy rollouts, CVaR) in {dt:.2f} s wall",
             "seconds": dt}
+
+
+def max_over_ranks(values, world, device):
+    """Element-wise MAX of per-rank timings over the process group (a no-op for one rank)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t.cpu()]
+
+
+def aggregate_rate(units_per_step, steps, world, max_ms):
+    """Whole-job throughput of `world` replicas: all units processed / slowest rank's time."""
+    return world * units_per_step * steps / (max_ms * 1e-3)
 
 
 def run_reference(args):
@@ -222,14 +239,11 @@ def run_cuda(args):
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
 
-    # ---- max over ranks
-    t = torch.tensor([total_ms, e2e_s * 1e3, kernel_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms, e2e_ms, kernel_ms = (float(x) for x in t.cpu())
+    # ---- max over ranks; every rank is an independent replica of the same workload (weak scaling)
+    total_ms, e2e_ms, kernel_ms = max_over_ranks([total_ms, e2e_s * 1e3, kernel_ms], world, dev)
     units_step = p.state_steps
-    value = world * units_step * args.steps / (total_ms * 1e-3)
-    e2e_value = world * units_step * args.steps / (e2e_ms * 1e-3)
+    value = aggregate_rate(units_step, args.steps, world, total_ms)
+    e2e_value = aggregate_rate(units_step, args.steps, world, e2e_ms)
 
     if rank == 0:
         key = workload_key(args.workload)
@@ -251,7 +265,7 @@ def run_cuda(args):
             "gpu_launches": int(ctl.launches_per_step * args.steps),
             "roofline": {"bound": "alu", "kernel": "noisy_rollout_kernel", "achieved": achieved / 1e12,
                          "peak": ALU_PEAK_LANE_OPS / 1e12, "unit": "Tlane-op/s (FP32-lane issue slots; FFMA = 1)",
-                         "frac": achieved / ALU_PEAK_LANE_OPS, "traffic": None,
+                         "frac": achieved / ALU_PEAK_LANE_OPS, "traffic": TRAFFIC_BYTES.get(key),
                          "algorithmic_ops_per_state_step": ALGO_OPS[key], "kernel_ms": kernel_ms,
                          "kernel_share_of_step": kernel_ms / (total_ms / args.steps),
                          "peak_source": "derived: 148 SMs x 128 FP32 lanes x 1.965 GHz (DESIGN.md)"},
@@ -264,8 +278,88 @@ def run_cuda(args):
         dist.destroy_process_group()
 
 
+def quick_time(p, steps=50, warmup=5):
+    """Device-timed ra_mppi_step on problem p (events per step, L2 flushed between); small helper of --report."""
+    import torch
+
+    from paper_2209_12842_b200.controller import RaMppi
+    ctl = RaMppi(p, device=0)
+    d_x0, v_init = ctl.tensor(p.x0), ctl.tensor(p.v)
+    d_v = v_init.clone()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=ctl.device)
+    stream = torch.cuda.current_stream()
+    ctl.enable_kernel_timing(True)
+    ms, kms = [], []
+    for i in range(warmup + steps):
+        d_v.copy_(v_init)
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        ctl.step(d_x0, d_v, i)
+        b.record(stream)
+        b.synchronize()
+        if i >= warmup:
+            ms.append(a.elapsed_time(b))
+            kms.append(ctl.last_rollout_ms())
+    ctl.close()
+    step_ms = float(np.mean(ms))
+    return {"workload": f"{p.name} K={p.K} M={p.M} T={p.T}", "ms_per_step": step_ms, "iterations_per_s": 1e3 / step_ms,
+            "state_steps_per_s": p.state_steps / (step_ms * 1e-3), "rollout_kernel_ms": float(np.mean(kms))}
+
+
+def run_report(args):
+    """--report: all five BASELINE workloads, the C4 sweep, the materialised-noise (HBM) variant of C3 and the
+    500-iteration CUDA-graph closed loop.  One JSON object per line on stdout (not the driver's bench line)."""
+    import torch
+
+    from paper_2209_12842_b200.controller import RaMppi
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    for name in ("C0", "C1", "C2", "C3"):
+        print(json.dumps({"report": "workload", **quick_time(make_problem(name))}), flush=True)
+    for K in W.C4_SWEEP_K:
+        for M in W.C4_SWEEP_M:
+            steps = 20 if K * M >= 65536 * 64 else 50
+            print(json.dumps({"report": "C4 sweep", **quick_time(make_problem(f"C4-K{K}-M{M}"), steps=steps)}), flush=True)
+    # materialised-noise mode: w[K,T,n_x,M] written by the generator and streamed back by the rollout kernel
+    p = make_problem("C3").replace(noise_mode=W.NOISE_MATERIALISED)
+    r = quick_time(p, steps=30)
+    noise_bytes = 4.0 * p.nx * p.state_steps
+    r.update({"report": "materialised noise (HBM-bound variant)", "noise_tensor_GB": noise_bytes / 1e9,
+              "rollout_read_GBps": noise_bytes / (r["rollout_kernel_ms"] * 1e-3) / 1e9,
+              "hbm_peak_GBps": hbm_peak, "peak_source": "measured" if peaks else "fallback",
+              "rollout_frac_of_hbm_peak": noise_bytes / (r["rollout_kernel_ms"] * 1e-3) / 1e9 / hbm_peak})
+    print(json.dumps(r), flush=True)
+    # closed loop: config 4, K=8192, M=64, 500 receding-horizon iterations replayed from one CUDA graph
+    p = make_problem("C4-K8192-M64")
+    ctl = RaMppi(p, device=0)
+    d_x0, d_v = ctl.tensor(p.x0), ctl.tensor(np.zeros((p.T, 2)))
+    ctl.closed_loop(d_x0, d_v, 0, 20)                      # capture + warm-up
+    d_x0.copy_(ctl.tensor(p.x0)); d_v.zero_()
+    log, ms = ctl.closed_loop(d_x0, d_v, 0, 500)           # per-iteration events: p50/p99
+    d_x0.copy_(ctl.tensor(p.x0)); d_v.zero_()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(torch.cuda.current_stream())
+    ctl.closed_loop(d_x0, d_v, 0, 500, log=False, timing=False)   # sustained: no per-iteration events
+    b.record(torch.cuda.current_stream())
+    b.synchronize()
+    total = a.elapsed_time(b)
+    log = log.cpu().numpy()
+    print(json.dumps({"report": "closed loop (CUDA graph)", "workload": f"{p.name} K={p.K} M={p.M} T={p.T}",
+                      "iterations": 500, "sustained_hz": 500.0 / (total * 1e-3), "latency_ms_p50": float(np.percentile(ms, 50)),
+                      "latency_ms_p99": float(np.percentile(ms, 99)), "latency_ms_max": float(ms.max()),
+                      "final_state": [float(x) for x in log[-1, :p.nx]],
+                      "distance_travelled_m": float(np.hypot(np.diff(log[:, 0]), np.diff(log[:, 1])).sum())}), flush=True)
+    ctl.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--report", action="store_true", help="all workloads + sweep + closed loop (not the bench line)")
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
@@ -274,7 +368,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
-    if args.impl == "reference":
+    if args.report:
+        run_report(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_cuda(args)

@@ -1,0 +1,108 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (pytest -m gpu).
+
+C1 and C3 are compared against the oracle in full (the oracle's k-loop is split over the host
+cores; every k is independent).  C2 and the largest C4 sweep point are compared on sampled
+control samples the oracle computes one by one, plus properties that hold at any size.
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2209_12842_b200 import workloads as W
+
+from parity_utils import TOL_STATE_ABS, TOL_V_ABS, assert_costs_close
+
+pytestmark = pytest.mark.gpu
+CORES = O.host_cores()
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2209_12842_b200 import build
+    build.build()
+    return torch
+
+
+def _problem(name):
+    import bench
+    return bench.make_problem(name)      # exactly the problem bench.py times
+
+
+def _gpu_step_and_costs(torch, p):
+    from paper_2209_12842_b200.controller import RaMppi
+    ctl = RaMppi(p, device=0)
+    d_x0, d_v = ctl.tensor(p.x0), ctl.tensor(p.v)
+    g = ctl.rollout_costs(d_x0, d_v, 0, want_L=True, want_xT=True, want_u=True)
+    ctl.step(d_x0, d_v, 0)                # same launch path as bench.py
+    S64, St64 = ctl.costs_f64()
+    torch.cuda.synchronize()
+    out = {k: t.cpu().numpy() for k, t in g.items()}
+    out["v_plus"] = d_v.cpu().numpy()
+    out["S64"], out["St64"] = S64.cpu().numpy(), St64.cpu().numpy()
+    ctl.close()
+    return out
+
+
+def _check_slice(p, g, r, sl):
+    assert np.abs(g["u"][sl] - r["u"]).max() < 2e-6 * max(1.0, np.abs(r["u"]).max())
+    assert np.abs(g["xT"][sl] - r["xT"]).max() < TOL_STATE_ABS
+    assert_costs_close(g["L"][sl], r["L"], "L")
+    assert_costs_close(g["S"][sl], r["S"], "S")
+    assert_costs_close(g["cvar"][sl], r["cvar"], "CVaR")
+    assert_costs_close(g["S_tilde"][sl], r["S_tilde"], "S_tilde")
+
+
+def _check_any_size_properties(p, g):
+    K = p.K
+    assert np.isfinite(g["S_tilde"]).all() and np.isfinite(g["xT"]).all()
+    # S~ = S + A CVaR 1[CVaR > C_u]  (14)-(16), on the GPU's own outputs
+    pen = np.where(g["cvar"] > p.C_u, p.A * g["cvar"].astype(np.float64), 0.0)
+    assert np.abs(g["St64"] - (g["S64"] + pen)).max() < 1e-6 * np.abs(g["St64"]).max()
+    # CVaR of each sample equals the sort-based top-k mean of its own L (all K samples, numpy)
+    k_tail = O.tail_count(p.alpha, p.M)
+    top = np.sort(g["L"].astype(np.float64), axis=1)[:, -k_tail:].mean(axis=1)
+    Lbar = g["L"].astype(np.float64).mean(axis=1)
+    assert_costs_close(g["cvar"], p.B * (top - Lbar) + Lbar, "CVaR vs sort of own L", tol=2e-6)
+    assert (g["cvar"] >= Lbar - 1e-3 * np.abs(Lbar) - 1e-6).all()          # tail mean >= mean
+    # v+ is inside the clamps and equals the softmin-weighted mean of the GPU's own u under its own S~
+    assert (g["v_plus"] >= np.asarray(p.u_min) - 1e-7).all() and (g["v_plus"] <= np.asarray(p.u_max) + 1e-7).all()
+    w = np.exp(-(g["St64"] - g["St64"].min()) / p.lam)
+    vp = np.clip(np.einsum("k,kti->ti", w, g["u"].astype(np.float64)) / w.sum(), p.u_min, p.u_max)
+    assert np.abs(g["v_plus"] - vp).max() < TOL_V_ABS
+    assert 1.0 <= w.sum() <= K
+
+
+@pytest.mark.parametrize("name", ["C1", "C3"])
+def test_full_oracle_comparison(torch_cuda, name):
+    p = _problem(name)
+    g = _gpu_step_and_costs(torch_cuda, p)
+    orc = O.Oracle(p)
+    r = orc.rollout_costs(n_threads=CORES)
+    _check_slice(p, g, r, slice(0, p.K))
+    _check_any_size_properties(p, g)
+    frac = (r["cvar"] > 0).mean()
+    print(f"{name}: fraction of samples with CVaR>0 = {frac:.3f}")
+    ref = orc.weights_update(r["S_tilde"], r["u"])
+    err = np.abs(g["v_plus"] - ref["v_plus"]).max()
+    ref2 = orc.weights_update(g["St64"], r["u"])
+    err2 = np.abs(g["v_plus"] - ref2["v_plus"]).max()
+    ess = 1.0 / ((ref["w"] / ref["Z"]) ** 2).sum()
+    print(f"{name}: v+ end-to-end err {err:.2e}; with GPU S~ through the oracle update {err2:.2e}; ESS {ess:.2f}; "
+          f"max|dS~| {np.abs(g['St64'] - r['S_tilde']).max():.2e}")
+    assert err2 < TOL_V_ABS
+    assert int(np.argmin(g["St64"])) == int(np.argmin(r["S_tilde"])) or \
+        np.sort(r["S_tilde"])[1] - np.sort(r["S_tilde"])[0] < 2 * np.abs(g["St64"] - r["S_tilde"]).max()
+
+
+@pytest.mark.parametrize("name", ["C2", "C4-K8192-M64", "C4-K65536-M256", "C4-K65536-M16"])
+def test_sampled_oracle_comparison(torch_cuda, name):
+    p = _problem(name)
+    g = _gpu_step_and_costs(torch_cuda, p)
+    orc = O.Oracle(p)
+    n = 24 if p.M >= 128 else 96
+    for kb in (0, p.K // 2 - 7, p.K - n):          # first CTA, a middle one across a CTA boundary, the last
+        r = orc.rollout_costs(k_begin=kb, k_end=kb + n, n_threads=CORES)
+        _check_slice(p, g, r, slice(kb, kb + n))
+    _check_any_size_properties(p, g)
