@@ -280,8 +280,8 @@ namespace {
 
 cudaError_t launch_sample_nominal(const ra_mppi_ctx* c, const Params& p, const float* d_x0, const float* d_v,
                                   cudaStream_t s) {
-  const int threads = 128, grid = (p.K + threads - 1) / threads;
-  const size_t smem = (size_t)2 * p.T * sizeof(float);
+  const int threads = kSampleThreads, grid = (p.K + kSampleKB - 1) / kSampleKB;
+  const size_t smem = (size_t)p.T * kSampleKB * (sizeof(float4) + sizeof(float)) + (size_t)2 * p.T * sizeof(float);
   const int dyn = c->cfg.dyn, nom = c->cfg.nominal;
   if (dyn == 0 && nom == 0) sample_nominal_kernel<0, 0><<<grid, threads, smem, s>>>(p, d_x0, d_v);
   else if (dyn == 0 && nom == 1) sample_nominal_kernel<0, 1><<<grid, threads, smem, s>>>(p, d_x0, d_v);

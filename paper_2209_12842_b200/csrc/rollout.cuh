@@ -19,16 +19,44 @@ constexpr int NOISE_MATERIALISED = 3;  // rollout-kernel variant that reads w fr
 // (3) PAPER.md:47, Alg.1 l.11-15.  S is accumulated in fp64 (K*T adds only) because the
 // softmin weights of (17) are sensitive to absolute errors in S~.
 // ---------------------------------------------------------------------------------------
+constexpr int kSampleThreads = 128;
+constexpr int kSampleKB = 16;  // control samples per CTA
+
 template <int DYN, int NOM>
-__global__ void __launch_bounds__(128) sample_nominal_kernel(const __grid_constant__ Params p,
-                                                             const float* __restrict__ x0g,
-                                                             const float* __restrict__ v) {
+__global__ void __launch_bounds__(kSampleThreads) sample_nominal_kernel(const __grid_constant__ Params p,
+                                                                        const float* __restrict__ x0g,
+                                                                        const float* __restrict__ v) {
   constexpr int NX = StateDim<DYN>::value;
-  extern __shared__ float v_s[];  // [T][2]
+  // Phase 1 is parallel over (k, t): Philox + Box-Muller + tan/sincos of the clamped control are
+  // independent across the horizon, so the K*T sampling work is spread over all threads.
+  // Phase 2 is the only sequential chain: one thread per sample rolls the nominal state forward.
+  extern __shared__ float4 sn_smem[];
+  float4* ce_s = sn_smem;                                              // [T][KB]
+  float* ctrl_s = reinterpret_cast<float*>(ce_s + (size_t)p.T * kSampleKB);  // [T][KB]
+  float* v_s = ctrl_s + (size_t)p.T * kSampleKB;                        // [T][2]
   for (int i = threadIdx.x; i < 2 * p.T; i += blockDim.x) v_s[i] = v[i];
   __syncthreads();
-  const int k = blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= p.K) return;
+  const int k0 = blockIdx.x * kSampleKB;
+  const uint32_t c3 = iteration_field(p, STREAM_EPS);
+  for (int idx = threadIdx.x; idx < p.T * kSampleKB; idx += blockDim.x) {
+    const int t = idx / kSampleKB, kl = idx % kSampleKB, k = k0 + kl;
+    if (k >= p.K) continue;
+    const uint4 r = philox4x32_10((uint32_t)k, 0u, (uint32_t)t, c3, p.rk);
+    float z0, z1;
+    box_muller(r.x, r.y, z0, z1);
+    const bool with_mean = k < p.K0;
+    const float v0 = v_s[2 * t], v1 = v_s[2 * t + 1];
+    const float u0 = fmaf(p.sigma_eps[0], z0, with_mean ? v0 : 0.0f);
+    const float u1 = fmaf(p.sigma_eps[1], z1, with_mean ? v1 : 0.0f);
+    const float4 ce = control_effect<DYN>(p, u0, u1);
+    p.u_raw[(size_t)t * p.K + k] = make_float2(u0, u1);
+    p.ce[(size_t)t * p.K + k] = ce;
+    ce_s[idx] = ce;
+    ctrl_s[idx] = fmaf(p.ctrl_w[0] * v0, u0, p.ctrl_w[1] * v1 * u1);   // gamma v^T Sigma^-1 u  (3)
+  }
+  __syncthreads();
+  const int k = k0 + threadIdx.x;
+  if (threadIdx.x >= kSampleKB || k >= p.K) return;
 
   const float x0X = x0g[0], x0Y = x0g[1];
   float x[NX];
@@ -36,24 +64,11 @@ __global__ void __launch_bounds__(128) sample_nominal_kernel(const __grid_consta
 #pragma unroll
   for (int i = 2; i < NX; ++i) x[i] = x0g[i];
   if constexpr (DYN == DYN_SINGLE_TRACK) x[3] = fmaxf(x[3], p.dyn_p[6]);
-
-  const uint32_t c3 = iteration_field(p, STREAM_EPS);
-  const bool with_mean = k < p.K0;
   double S = 0.0;
   for (int t = 0; t < p.T; ++t) {
-    const uint4 r = philox4x32_10((uint32_t)k, 0u, (uint32_t)t, c3, p.rk);
-    float z0, z1;
-    box_muller(r.x, r.y, z0, z1);
-    const float v0 = v_s[2 * t], v1 = v_s[2 * t + 1];
-    const float u0 = fmaf(p.sigma_eps[0], z0, with_mean ? v0 : 0.0f);
-    const float u1 = fmaf(p.sigma_eps[1], z1, with_mean ? v1 : 0.0f);
-    const float4 ce = control_effect<DYN>(p, u0, u1);
-    p.u_raw[(size_t)t * p.K + k] = make_float2(u0, u1);
-    p.ce[(size_t)t * p.K + k] = ce;
     const float q = nominal_cost<NOM>(p, x0X + x[0], x0Y + x[1], x[3]);
-    const float ctrl = fmaf(p.ctrl_w[0] * v0, u0, p.ctrl_w[1] * v1 * u1);
-    S += (double)q + (double)ctrl;
-    dynamics_step<DYN>(p, x, ce);
+    S += (double)q + (double)ctrl_s[t * kSampleKB + threadIdx.x];
+    dynamics_step<DYN>(p, x, ce_s[t * kSampleKB + threadIdx.x]);
   }
   const float w_phi = (NOM == NOM_GOAL) ? p.nom_p[3] : p.nom_p[7];
   S += (double)(w_phi * nominal_cost<NOM>(p, x0X + x[0], x0Y + x[1], x[3]));

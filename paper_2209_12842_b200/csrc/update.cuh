@@ -37,7 +37,7 @@ weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S
                       float* __restrict__ v_out, float* __restrict__ w_out,
                       float* __restrict__ stats) {
   __shared__ ST red_s[32];
-  __shared__ float red_f[32];
+  __shared__ float red_f[96];
   const int t = blockIdx.x;
   ST bmin = (ST)INFINITY;
   for (int k = threadIdx.x; k < p.K; k += blockDim.x) bmin = min(bmin, S_tilde[k]);
@@ -51,10 +51,27 @@ weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S
     n0 = fmaf(w, uk.x, n0);
     n1 = fmaf(w, uk.y, n1);
   }
-  auto add = [](float a, float b) { return a + b; };
-  Z = block_reduce<float>(Z, red_f, add, 0.0f);
-  n0 = block_reduce<float>(n0, red_f, add, 0.0f);
-  n1 = block_reduce<float>(n1, red_f, add, 0.0f);
+  // one fixed-order tree for the three sums (a single shared-memory exchange)
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    Z += __shfl_xor_sync(0xFFFFFFFFu, Z, o);
+    n0 += __shfl_xor_sync(0xFFFFFFFFu, n0, o);
+    n1 += __shfl_xor_sync(0xFFFFFFFFu, n1, o);
+  }
+  {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    if (lane == 0) { red_f[warp] = Z; red_f[32 + warp] = n0; red_f[64 + warp] = n1; }
+    __syncthreads();
+    Z = lane < nw ? red_f[lane] : 0.0f;
+    n0 = lane < nw ? red_f[32 + lane] : 0.0f;
+    n1 = lane < nw ? red_f[64 + lane] : 0.0f;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      Z += __shfl_xor_sync(0xFFFFFFFFu, Z, o);
+      n0 += __shfl_xor_sync(0xFFFFFFFFu, n0, o);
+      n1 += __shfl_xor_sync(0xFFFFFFFFu, n1, o);
+    }
+  }
   if (threadIdx.x == 0) {
     v_out[2 * t] = clampf(n0 / Z, p.u_min[0], p.u_max[0]);
     v_out[2 * t + 1] = clampf(n1 / Z, p.u_min[1], p.u_max[1]);
