@@ -9,7 +9,10 @@
 
 namespace ra {
 
-constexpr int kRolloutThreads = 256;
+#ifndef RA_ROLLOUT_THREADS
+#define RA_ROLLOUT_THREADS 256
+#endif
+constexpr int kRolloutThreads = RA_ROLLOUT_THREADS;
 constexpr int kRolloutWarps = kRolloutThreads / 32;
 constexpr int NOISE_MATERIALISED = 3;  // rollout-kernel variant that reads w from HBM
 
