@@ -148,6 +148,12 @@ ra_status ra_mppi_philox(ra_mppi_ctx* ctx, const uint32_t* d_ctr, int32_t n, uin
 ra_status ra_mppi_state_noise(ra_mppi_ctx* ctx, const int32_t* d_kmt, int32_t n,
                               uint64_t iteration, float* d_w, void* cuda_stream);
 
+/* Measured issue rates of the plain SM pipes on `device`, in 1e12 lane-operations per second:
+ * h_tera_lane_ops[4] (HOST) = {FFMA, IMAD.WIDE.U32 each paired with one LOP3 (the Philox round
+ * pattern), LOP3, MUFU.LG2}.  Runs four short
+ * microbenchmark kernels on the NULL stream and synchronises.  Roofline denominators only.   */
+ra_status ra_mppi_measure_pipe_peaks(int32_t device, float* h_tera_lane_ops);
+
 /* Number of kernels one ra_mppi_step launches (for launch accounting).                   */
 int32_t ra_mppi_launches_per_step(const ra_mppi_ctx* ctx);
 /* Last error text, owned by the context (valid until the next call on it).               */

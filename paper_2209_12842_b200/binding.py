@@ -55,7 +55,7 @@ EXPORTS = (
     "ra_mppi_create", "ra_mppi_step", "ra_mppi_rollout_costs", "ra_mppi_weights_update",
     "ra_mppi_step_host", "ra_mppi_enable_kernel_timing", "ra_mppi_last_rollout_ms",
     "ra_mppi_export_costs_f64", "ra_mppi_plant_shift", "ra_mppi_closed_loop", "ra_mppi_philox", "ra_mppi_state_noise",
-    "ra_mppi_launches_per_step", "ra_mppi_last_error", "ra_mppi_destroy",
+    "ra_mppi_measure_pipe_peaks", "ra_mppi_launches_per_step", "ra_mppi_last_error", "ra_mppi_destroy",
 )
 
 _lib = None
@@ -84,6 +84,7 @@ def load():
     L.ra_mppi_closed_loop.argtypes = [vp, fp, fp, u64, i32, fp, C.POINTER(C.c_float), vp]
     L.ra_mppi_philox.argtypes = [vp, vp, i32, vp, vp]
     L.ra_mppi_state_noise.argtypes = [vp, vp, i32, u64, fp, vp]
+    L.ra_mppi_measure_pipe_peaks.argtypes = [i32, C.POINTER(C.c_float)]
     L.ra_mppi_launches_per_step.argtypes = [vp]
     L.ra_mppi_launches_per_step.restype = i32
     L.ra_mppi_last_error.argtypes = [vp]
@@ -207,6 +208,13 @@ def ra_mppi_philox(ctx, d_ctr, n, d_out, stream=0):
 def ra_mppi_state_noise(ctx, d_kmt, n, iteration, d_w, stream=0):
     _check(ctx, load().ra_mppi_state_noise(ctx, d_kmt, int(n), int(iteration), d_w, stream),
            "ra_mppi_state_noise")
+
+
+def ra_mppi_measure_pipe_peaks(device=0):
+    """{pipe: 1e12 lane-ops/s} measured by the library's microbenchmark kernels."""
+    out = (C.c_float * 4)()
+    _check(None, load().ra_mppi_measure_pipe_peaks(int(device), out), "ra_mppi_measure_pipe_peaks")
+    return dict(zip(("ffma", "imad_wide", "lop3", "mufu"), (float(x) for x in out)))
 
 
 def ra_mppi_launches_per_step(ctx):

@@ -484,7 +484,8 @@ ra_status ra_mppi_closed_loop(ra_mppi_ctx* c, float* d_x0, float* d_v, uint64_t 
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   cudaStream_t own = nullptr;
   if (s == nullptr) {  // the legacy default stream cannot be captured
-    RA_CUDA(c, cudaStreamCreateWithFlags(&own, cudaStreamNonBlocking));
+    // a blocking stream: ordered after (and before) the work the caller put on the NULL stream
+    RA_CUDA(c, cudaStreamCreate(&own));
     s = own;
   }
   ra_status st = RA_OK;
