@@ -24,7 +24,7 @@ class OrcProblem(C.Structure):
         ("sigma_eps", C.c_double * 2), ("sigma_w", C.c_double * 6),
         ("alpha", C.c_double), ("lam", C.c_double), ("gamma", C.c_double),
         ("A", C.c_double), ("B", C.c_double), ("C_u", C.c_double), ("eta", C.c_double),
-        ("nominal", C.c_int32), ("nom_p", C.c_double * 8),
+        ("nominal", C.c_int32), ("nom_p", C.c_double * 12),
         ("risk", C.c_int32), ("risk_p", C.c_double * 4),
         ("noise_kind", C.c_int32), ("noise_p", C.c_double * 4),
         ("seed", C.c_uint64),
@@ -50,8 +50,13 @@ def lib():
                                       C.c_uint32, C.c_uint64, _DP]
         L.orc_nx.argtypes = [C.c_int32]
         L.orc_dynamics.argtypes = [C.POINTER(OrcProblem), _DP, _DP, _DP]
-        for f in (L.orc_q, L.orc_phi, L.orc_l):
+        for f in (L.orc_q, L.orc_l):
             f.argtypes = [C.POINTER(OrcProblem), _DP]
+            f.restype = C.c_double
+        L.orc_phi.argtypes = [C.POINTER(OrcProblem), _DP, _DP]
+        L.orc_phi.restype = C.c_double
+        for f in (L.orc_racing_offset, L.orc_racing_arclength, L.orc_indicator_margin):
+            f.argtypes = [C.POINTER(OrcProblem), C.c_double, C.c_double]
             f.restype = C.c_double
         L.orc_ellipse_offset.argtypes = [C.c_double] * 4
         L.orc_ellipse_offset.restype = C.c_double
@@ -65,7 +70,7 @@ def lib():
         L.orc_cvar_literal12.restype = C.c_double
         L.orc_sensitivity_scale.argtypes = [_DP, C.c_int32, C.c_double, _DP]
         L.orc_rollout_costs.argtypes = [C.POINTER(OrcProblem), _DP, _DP, C.c_uint64, C.c_int32,
-                                        C.c_int32, C.c_int32] + [_DP] * 7
+                                        C.c_int32, C.c_int32] + [_DP] * 8
         L.orc_rollout_costs.restype = C.c_int
         L.orc_weights_update.argtypes = [C.POINTER(OrcProblem), _DP, _DP, _DP, _DP, _DP, _DP]
         L.orc_weights_update.restype = C.c_int
@@ -127,9 +132,19 @@ class Oracle:
         x = np.ascontiguousarray(x, dtype=np.float64)
         return lib().orc_q(C.byref(self.s), _dp(x))
 
-    def phi(self, x):
+    def phi(self, x, x0=None):
         x = np.ascontiguousarray(x, dtype=np.float64)
-        return lib().orc_phi(C.byref(self.s), _dp(x))
+        x0 = np.ascontiguousarray(self.p.x0 if x0 is None else x0, dtype=np.float64)
+        return lib().orc_phi(C.byref(self.s), _dp(x), _dp(x0))
+
+    def racing_offset(self, X, Y):
+        return lib().orc_racing_offset(C.byref(self.s), float(X), float(Y))
+
+    def racing_arclength(self, X, Y):
+        return lib().orc_racing_arclength(C.byref(self.s), float(X), float(Y))
+
+    def indicator_margin(self, X, Y):
+        return lib().orc_indicator_margin(C.byref(self.s), float(X), float(Y))
 
     def l(self, x):
         x = np.ascontiguousarray(x, dtype=np.float64)
@@ -145,7 +160,7 @@ class Oracle:
 
     # ---- iteration
     def rollout_costs(self, x0=None, v=None, iteration=0, k_begin=0, k_end=None, n_threads=1,
-                      want_L=True, want_xT=True):
+                      want_L=True, want_xT=True, want_margin=False):
         p, s = self.p, self.s
         x0 = np.ascontiguousarray(p.x0 if x0 is None else x0, dtype=np.float64)
         v = np.ascontiguousarray(p.v if v is None else v, dtype=np.float64)
@@ -156,11 +171,12 @@ class Oracle:
             L=np.zeros((n, s.M)) if want_L else None,
             xT=np.zeros((n, s.M, self.nx)) if want_xT else None,
             x_nom=np.zeros((n, self.nx)),
+            margin=np.zeros((n, s.M + 1)) if want_margin else None,
         )
         rc = lib().orc_rollout_costs(C.byref(s), _dp(x0), _dp(v), int(iteration), k_begin, k_end,
                                      int(n_threads), _dp(out["u"]), _dp(out["S"]), _dp(out["cvar"]),
                                      _dp(out["S_tilde"]), _dp(out["L"]), _dp(out["xT"]),
-                                     _dp(out["x_nom"]))
+                                     _dp(out["x_nom"]), _dp(out["margin"]))
         if rc:
             raise RuntimeError(f"orc_rollout_costs failed: {rc}")
         return out

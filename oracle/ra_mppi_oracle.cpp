@@ -169,9 +169,61 @@ double orc_ellipse_offset(double a, double b, double X, double Y) {
   return f / (2.0 * std::max(g, 1e-12));
 }
 
+/* Rounded-rectangle track (synthetic stand-in for the paper's track: 0.6 m wide, 10.9 m
+ * centreline, corner radius 0.3 m; its layout figure P:257 is missing).  The centreline is the set
+ * of points at distance rc from the box B = [-ax,ax] x [-ay,ay].  e = signed distance to the
+ * centreline, + outward ("lateral deviation e(x)"). */
+double orc_racing_offset(const orc_problem* p, double X, double Y) {
+  const double ax = p->nom_p[0], ay = p->nom_p[1], rc = p->nom_p[2];
+  const double qx = std::fabs(X) - ax, qy = std::fabs(Y) - ay;
+  const double ox = std::max(qx, 0.0), oy = std::max(qy, 0.0);
+  const double sd = std::sqrt(ox * ox + oy * oy) + std::min(std::max(qx, qy), 0.0);  /* signed distance to B */
+  return sd - rc;
+}
+
+/* Arc length s(x) of the projection onto the centreline (Fig. 2), measured counter-clockwise
+ * from (ax+rc, 0); one quadrant is folded onto the first by symmetry. */
+double orc_racing_arclength(const orc_problem* p, double X, double Y) {
+  const double ax = p->nom_p[0], ay = p->nom_p[1], rc = p->nom_p[2];
+  const double Xa = std::fabs(X), Ya = std::fabs(Y);
+  const double dx = std::max(Xa - ax, 0.0), dy = std::max(Ya - ay, 0.0);
+  const double Pq = ay + rc * (kPi / 2.0) + ax;  /* quarter perimeter */
+  double sq;
+  if (dx > 0.0 && dy > 0.0) sq = ay + rc * std::atan2(dy, dx);             /* corner arc       */
+  else if (dx > 0.0) sq = Ya;                                               /* right straight   */
+  else if (dy > 0.0) sq = ay + rc * (kPi / 2.0) + (ax - Xa);                /* top straight     */
+  else sq = ((ax - Xa) < (ay - Ya)) ? Ya : ay + rc * (kPi / 2.0) + (ax - Xa); /* inside B: nearest side */
+  if (X >= 0.0 && Y >= 0.0) return sq;
+  if (X < 0.0 && Y >= 0.0) return 2.0 * Pq - sq;
+  if (X < 0.0 && Y < 0.0) return 2.0 * Pq + sq;
+  return 4.0 * Pq - sq;
+}
+
+double orc_indicator_margin(const orc_problem* p, double X, double Y) {
+  double m = std::numeric_limits<double>::infinity();
+  for (int i = 0; i < p->n_circles; ++i) {
+    const double dx = X - p->circles[3 * i + 0], dy = Y - p->circles[3 * i + 1];
+    m = std::min(m, std::fabs(std::sqrt(dx * dx + dy * dy) - p->circles[3 * i + 2]));
+  }
+  return m;
+}
+
 namespace {
 /* state part of the nominal running cost; q "can take an arbitrary form" P:45 */
 double q_state(const orc_problem* p, const double* x) {
+  if (p->nominal == ORC_NOM_RACING) {
+    /* (20) P:164: q = c1 mu_bdry + c2 mu_obs + c3 q_dev, q_dev = e^2 */
+    const double hw = p->nom_p[3], c1 = p->nom_p[4], c2 = p->nom_p[5], c3 = p->nom_p[6];
+    const double e = orc_racing_offset(p, x[0], x[1]);
+    const double d = hw - std::fabs(e);      /* signed distance from the nearest boundary, + on track */
+    const double mu_bdry = std::max(0.0, std::atan(-100.0 * d) / kPi + 0.5);                 /* (21) P:227 */
+    double mu_obs = 0.0;                                                                      /* (22) P:232 */
+    for (int i = 0; i < p->n_circles; ++i) {
+      const double dx = x[0] - p->circles[3 * i + 0], dy = x[1] - p->circles[3 * i + 1];
+      if (std::sqrt(dx * dx + dy * dy) < p->circles[3 * i + 2]) mu_obs += 1.0;
+    }
+    return c1 * mu_bdry + c2 * mu_obs + c3 * e * e;
+  }
   if (p->nominal == ORC_NOM_GOAL) {
     const double w = p->nom_p[0], gx = p->nom_p[1], gy = p->nom_p[2];
     return w * ((x[0] - gx) * (x[0] - gx) + (x[1] - gy) * (x[1] - gy));
@@ -187,8 +239,16 @@ double q_state(const orc_problem* p, const double* x) {
 
 double orc_q(const orc_problem* p, const double* x) { return q_state(p, x); }
 
-/* phi(x) = w_phi * q_state(x)  (D:G18; the paper's own (23) P:239 needs a centreline) */
-double orc_phi(const orc_problem* p, const double* x) {
+/* phi(x) = w_phi * q_state(x)  (D:G18); racing: (23) P:239 phi = c4 - c5 s(x), s = distance travelled
+ * along the centreline by the end of the horizon, i.e. s(x_T) - s(x_0) wrapped to (-P/2, P/2]. */
+double orc_phi(const orc_problem* p, const double* x, const double* x0) {
+  if (p->nominal == ORC_NOM_RACING) {
+    const double P = 4.0 * (p->nom_p[1] + p->nom_p[2] * (kPi / 2.0) + p->nom_p[0]);
+    double ds = orc_racing_arclength(p, x[0], x[1]) - orc_racing_arclength(p, x0[0], x0[1]);
+    if (ds > 0.5 * P) ds -= P;
+    if (ds < -0.5 * P) ds += P;
+    return p->nom_p[7] - p->nom_p[8] * ds;
+  }
   const double w_phi = p->nominal == ORC_NOM_GOAL ? p->nom_p[3] : p->nom_p[7];
   return w_phi * q_state(p, x);
 }
@@ -225,6 +285,7 @@ double orc_l(const orc_problem* p, const double* x) {
     return l;
   }
   if (p->risk == ORC_RISK_COSTMAP) return p->risk_p[0] * orc_bilinear(p, x[0], x[1]);
+  if (p->risk == ORC_RISK_NOMINAL) return q_state(p, x);   /* "l(x~) = q(x~)" P:247 */
   /* test-only: weight * x[index] */
   return p->risk_p[0] * x[(int)p->risk_p[1]];
 }
@@ -277,7 +338,7 @@ namespace {
 void one_sample(const orc_problem* p, const double* x0_in, const double* v, uint64_t iteration,
                 int32_t k, int32_t k_tail, int32_t K0,
                 double* u_out, double* S_out, double* cvar_out, double* Stil_out,
-                double* L_out, double* xT_out, double* xnom_out) {
+                double* L_out, double* xT_out, double* xnom_out, double* margin_out) {
   const int nx = orc_nx(p->dyn);
   const int T = p->T, M = p->M;
   const uint32_t key[2] = {(uint32_t)(p->seed & 0xFFFFFFFFull), (uint32_t)(p->seed >> 32)};
@@ -306,7 +367,10 @@ void one_sample(const orc_problem* p, const double* x0_in, const double* v, uint
   double x[6], xn[6];
   for (int i = 0; i < nx; ++i) x[i] = x0[i];
   double S = 0.0;
+  const bool want_margin = margin_out && p->nominal == ORC_NOM_RACING;
+  double mg = std::numeric_limits<double>::infinity();
   for (int t = 0; t < T; ++t) {
+    if (want_margin) mg = std::min(mg, orc_indicator_margin(p, x[0], x[1]));
     double ctrl = 0.0;
     for (int i = 0; i < 2; ++i)
       if (p->sigma_eps[i] > 0.0)
@@ -315,7 +379,8 @@ void one_sample(const orc_problem* p, const double* x0_in, const double* v, uint
     orc_dynamics(p, x, &u[2 * t], xn);
     for (int i = 0; i < nx; ++i) x[i] = xn[i];
   }
-  S += orc_phi(p, x);
+  S += orc_phi(p, x, x0);
+  if (margin_out) margin_out[0] = mg;
 
   /* O1c: M noisy rollouts (6) P:63 from x~_0 = x_0 P:109, risk cost (9) P:93,
    * Alg.1 l.16-21 P:194-199; driven by the sampled u^k (D:G6) */
@@ -324,7 +389,10 @@ void one_sample(const orc_problem* p, const double* x0_in, const double* v, uint
     double xt[6];
     for (int i = 0; i < nx; ++i) xt[i] = x0[i];
     double L = 0.0;
+    double mgm = std::numeric_limits<double>::infinity();
     for (int t = 0; t < T; ++t) {
+      if (margin_out && p->risk == ORC_RISK_NOMINAL && p->nominal == ORC_NOM_RACING)
+        mgm = std::min(mgm, orc_indicator_margin(p, xt[0], xt[1]));
       L += orc_l(p, xt);
       double w[6];
       orc_state_noise(p, (uint32_t)k, (uint32_t)m, (uint32_t)t, ORC_STREAM_W, iteration, w);
@@ -333,6 +401,7 @@ void one_sample(const orc_problem* p, const double* x0_in, const double* v, uint
       if (p->dyn == ORC_DYN_SINGLE_TRACK) xt[3] = std::max(xt[3], p->dyn_p[6]);
     }
     Lk[m] = L;
+    if (margin_out) margin_out[1 + m] = mgm;
     if (L_out) L_out[m] = L;
     if (xT_out) for (int i = 0; i < nx; ++i) xT_out[(size_t)m * nx + i] = xt[i];
   }
@@ -356,7 +425,7 @@ void one_sample(const orc_problem* p, const double* x0_in, const double* v, uint
 int orc_rollout_costs(const orc_problem* p, const double* x0, const double* v,
                       uint64_t iteration, int32_t k_begin, int32_t k_end, int32_t n_threads,
                       double* u, double* S, double* cvar, double* S_tilde, double* L, double* xT,
-                      double* x_nom) {
+                      double* x_nom, double* margin) {
   if (!p || !x0 || !v || k_begin < 0 || k_end > p->K || k_begin > k_end) return 1;
   const int nx = orc_nx(p->dyn);
   const int32_t k_tail = orc_tail_count(p->alpha, p->M);                       /* O0 */
@@ -368,7 +437,8 @@ int orc_rollout_costs(const orc_problem* p, const double* x0, const double* v,
       one_sample(p, x0, v, iteration, k, k_tail, K0,
                  u ? u + i * T * 2 : nullptr, S ? S + i : nullptr, cvar ? cvar + i : nullptr,
                  S_tilde ? S_tilde + i : nullptr, L ? L + i * M : nullptr,
-                 xT ? xT + i * M * nx : nullptr, x_nom ? x_nom + i * nx : nullptr);
+                 xT ? xT + i * M * nx : nullptr, x_nom ? x_nom + i * nx : nullptr,
+                 margin ? margin + i * (M + 1) : nullptr);
     }
   };
   const int32_t n = k_end - k_begin;
@@ -412,7 +482,7 @@ int orc_step(const orc_problem* p, const double* x0, const double* v, uint64_t i
              int32_t n_threads, double* v_plus) {
   std::vector<double> u((size_t)p->K * p->T * 2), Stil((size_t)p->K);
   int rc = orc_rollout_costs(p, x0, v, iteration, 0, p->K, n_threads, u.data(), nullptr, nullptr,
-                             Stil.data(), nullptr, nullptr, nullptr);
+                             Stil.data(), nullptr, nullptr, nullptr, nullptr);
   if (rc) return rc;
   return orc_weights_update(p, Stil.data(), u.data(), v_plus, nullptr, nullptr, nullptr);
 }

@@ -37,8 +37,8 @@ extern "C" {
 #endif
 
 enum { ORC_DYN_BICYCLE = 0, ORC_DYN_SINGLE_TRACK = 1 };
-enum { ORC_NOM_GOAL = 0, ORC_NOM_ELLIPSE_TRACK = 1 };
-enum { ORC_RISK_CIRCLES = 0, ORC_RISK_COSTMAP = 1, ORC_RISK_LINEAR_STATE = 2 };
+enum { ORC_NOM_GOAL = 0, ORC_NOM_ELLIPSE_TRACK = 1, ORC_NOM_RACING = 2 };
+enum { ORC_RISK_CIRCLES = 0, ORC_RISK_COSTMAP = 1, ORC_RISK_LINEAR_STATE = 2, ORC_RISK_NOMINAL = 3 /* l = q */ };
 enum { ORC_NOISE_GAUSSIAN = 0, ORC_NOISE_UNIFORM = 1, ORC_NOISE_JUMP = 2 };
 enum { ORC_STREAM_EPS = 0, ORC_STREAM_W = 1, ORC_STREAM_PLANT = 2 };
 
@@ -53,7 +53,8 @@ typedef struct {
   double  alpha, lambda, gamma;     /* (8b) :81, (5)/(17) :55/:134, (3) :47            */
   double  A, B, C_u, eta;           /* (14) :120, (18) :144, (15) :124, Alg.1 l.7 :183 */
   int32_t nominal;          /* ORC_NOM_*                                               */
-  double  nom_p[8];         /* goal {w,gx,gy,w_phi}; track {a,b,half_w,w_lat,w_v,v_ref,w_bdry,w_phi} */
+  double  nom_p[12];        /* goal {w,gx,gy,w_phi}; track {a,b,half_w,w_lat,w_v,v_ref,w_bdry,w_phi};
+                               racing {ax,ay,rc,half_w,c1,c2,c3,c4,c5} (20)-(23) PAPER.md:164-241 */
   int32_t risk;             /* ORC_RISK_*                                              */
   double  risk_p[4];        /* circles {weight,margin}; costmap {weight}; linear {weight,index} */
   int32_t noise_kind;       /* ORC_NOISE_*                                             */
@@ -78,10 +79,15 @@ void   orc_state_noise(const orc_problem* p, uint32_t k, uint32_t m, uint32_t t,
 int    orc_nx(int32_t dyn);
 void   orc_dynamics(const orc_problem* p, const double* x, const double u[2], double* x_next);
 double orc_q(const orc_problem* p, const double* x);     /* nominal running cost */
-double orc_phi(const orc_problem* p, const double* x);   /* terminal cost        */
+double orc_phi(const orc_problem* p, const double* x, const double* x0);   /* terminal cost (x0: racing progress) */
 double orc_l(const orc_problem* p, const double* x);     /* risk running cost    */
 double orc_ellipse_offset(double a, double b, double X, double Y);
 double orc_bilinear(const orc_problem* p, double X, double Y);
+/* rounded-rectangle race track: lateral deviation e (+ outward) and centreline arc length s  */
+double orc_racing_offset(const orc_problem* p, double X, double Y);
+double orc_racing_arclength(const orc_problem* p, double X, double Y);
+/* smallest |d_i - r_i| over the obstacles at (X,Y): distance of the indicator (22) from its jump */
+double orc_indicator_margin(const orc_problem* p, double X, double Y);
 
 /* ---- CVaR -------------------------------------------------------------- */
 int32_t orc_tail_count(double alpha, int32_t M);
@@ -97,7 +103,8 @@ int orc_rollout_costs(const orc_problem* p, const double* x0, const double* v,
                       uint64_t iteration, int32_t k_begin, int32_t k_end, int32_t n_threads,
                       double* u /*[n,T,2]*/, double* S /*[n]*/, double* cvar /*[n]*/,
                       double* S_tilde /*[n]*/, double* L /*[n,M]*/, double* xT /*[n,M,nx]*/,
-                      double* x_nom /*[n,nx] nominal terminal state*/);
+                      double* x_nom /*[n,nx] nominal terminal state*/,
+                      double* margin /*[n,M+1] min indicator margin: col 0 nominal, 1..M noisy; or NULL*/);
 /* O2-O3: weights and update from S_tilde[K] and u[K,T,2].                   */
 int orc_weights_update(const orc_problem* p, const double* S_tilde, const double* u,
                        double* v_plus /*[T,2]*/, double* w /*[K]*/, double* Z, double* beta);

@@ -21,8 +21,8 @@ from typing import Optional
 import numpy as np
 
 DYN_BICYCLE, DYN_SINGLE_TRACK = 0, 1
-NOM_GOAL, NOM_ELLIPSE_TRACK = 0, 1
-RISK_CIRCLES, RISK_COSTMAP, RISK_LINEAR_STATE = 0, 1, 2
+NOM_GOAL, NOM_ELLIPSE_TRACK, NOM_RACING = 0, 1, 2
+RISK_CIRCLES, RISK_COSTMAP, RISK_LINEAR_STATE, RISK_NOMINAL = 0, 1, 2, 3
 NOISE_GAUSSIAN, NOISE_UNIFORM, NOISE_JUMP = 0, 1, 2
 NOISE_FUSED, NOISE_MATERIALISED = 0, 1
 
@@ -185,6 +185,54 @@ def config4(K=8192, M=64, T=50) -> Problem:
     """Config-1 track with 64 obstacles; sweep points and the closed loop vary K, M."""
     p = config1(K=K, M=M, T=T, n_obs=64, seed=4)
     return p.replace(name=f"C4-K{K}-M{M}")
+
+
+def rounded_rect_points(ax, ay, rc, s_values):
+    """Centreline points and outward unit normals of the rounded-rectangle track at arc lengths s
+    (counter-clockwise from (ax+rc, 0)).  Scene geometry only (obstacle placement, start pose)."""
+    seg = [2 * ay, rc * math.pi / 2, 2 * ax, rc * math.pi / 2] * 2          # straight, corner, ... from (ax+rc, -ay)
+    P = sum(seg)
+    pts = []
+    for s in np.atleast_1d(s_values):
+        u = (s + ay) % P                                                     # shift origin to the corner (ax+rc, -ay)
+        corners = [(ax, ay), (-ax, ay), (-ax, -ay), (ax, -ay)]
+        k = 0
+        while u > seg[k]:
+            u -= seg[k]; k += 1
+        side, is_corner = k // 2, k % 2 == 1
+        a0 = side * math.pi / 2                                              # outward normal angle of this side
+        if not is_corner:
+            n = (math.cos(a0), math.sin(a0)); t = (-math.sin(a0), math.cos(a0))
+            start = [(ax + rc, -ay), (ax, ay + rc), (-ax - rc, ay), (-ax, -ay - rc)][side]
+            pts.append((start[0] + u * t[0], start[1] + u * t[1], n[0], n[1]))
+        else:
+            c = corners[side]; ang = a0 + u / rc
+            pts.append((c[0] + rc * math.cos(ang), c[1] + rc * math.sin(ang), math.cos(ang), math.sin(ang)))
+    return np.array(pts), P
+
+
+def paper_racing(K=1024, M=300, T=30, seed=5) -> Problem:
+    """The paper's own controller set-up: costs (20)-(23) with c1..c5 = 2, 1, 0.1, 0.6, 2,
+    l = q, horizon 30, lambda 0.35, eta 0.2, A 10, 1024 samples x 300 realisations, on a synthetic
+    rounded-rectangle track with the published dimensions (0.6 m wide, 10.9 m centreline, 0.3 m corners, ten
+    r = 0.1 m obstacles) because the paper's layout figure is missing.  Vehicle: kinematic bicycle
+    at 1/28 scale (the paper's own model is not given)."""
+    rc, hw = 0.3, 0.3
+    ax = 1.5
+    ay = (10.9 - 2 * math.pi * rc) / 4 - ax
+    rng = np.random.default_rng(seed)
+    P = 4 * (ax + ay) + 2 * math.pi * rc
+    s_obs = (np.arange(10) + rng.uniform(0.2, 0.8, size=10)) * P / 10
+    pts, _ = rounded_rect_points(ax, ay, rc, s_obs)
+    off = rng.uniform(-0.18, 0.18, size=10)
+    circles = _f32(np.stack([pts[:, 0] + off * pts[:, 2], pts[:, 1] + off * pts[:, 3], np.full(10, 0.1)], axis=1))
+    start, _ = rounded_rect_points(ax, ay, rc, [P - ay - rc * math.pi / 2 - 0.6 * ax])   # on the bottom straight
+    x0 = _f32([start[0, 0], start[0, 1], 0.0, 1.5])                                      # heading +x (counter-clockwise)
+    return Problem(name="paper-racing", K=K, M=M, T=T, dt=0.02, dyn=DYN_BICYCLE, dyn_p=[0.093],
+                   u_min=[-0.4, -4.0], u_max=[0.4, 4.0], sigma_eps=[0.15, 1.0],
+                   sigma_w=[0.004, 0.004, 0.01, 0.03], alpha=0.9, lam=0.35, gamma=0.35, A=10.0, B=1.0, C_u=0.5,
+                   eta=0.2, nominal=NOM_RACING, nom_p=[ax, float(_f32(ay)), rc, hw, 2.0, 1.0, 0.1, 0.6, 2.0],
+                   risk=RISK_NOMINAL, risk_p=[0.0], seed=seed, x0=x0, v=np.zeros((T, 2)), circles=circles)
 
 
 C4_SWEEP_K = (1024, 4096, 16384, 65536)
