@@ -39,8 +39,11 @@ typedef enum {
 } ra_status;
 
 typedef enum { RA_DYN_KINEMATIC_BICYCLE = 0, RA_DYN_SINGLE_TRACK = 1 } ra_dyn;
-typedef enum { RA_NOM_GOAL = 0, RA_NOM_ELLIPSE_TRACK = 1 } ra_nominal;
-typedef enum { RA_RISK_CIRCLES = 0, RA_RISK_COSTMAP = 1, RA_RISK_LINEAR_STATE = 2 /* test-only */ } ra_risk;
+typedef enum { RA_NOM_GOAL = 0, RA_NOM_ELLIPSE_TRACK = 1, RA_NOM_RACING = 2 /* (20)-(23) PAPER.md:164-241 */ } ra_nominal;
+typedef enum {
+  RA_RISK_CIRCLES = 0, RA_RISK_COSTMAP = 1, RA_RISK_LINEAR_STATE = 2 /* test-only */,
+  RA_RISK_NOMINAL = 3 /* l = q; with RA_NOM_RACING */
+} ra_risk;
 typedef enum { RA_NOISE_GAUSSIAN = 0, RA_NOISE_UNIFORM = 1, RA_NOISE_JUMP = 2 } ra_noise_kind;
 typedef enum { RA_NOISE_FUSED = 0, RA_NOISE_MATERIALISED = 1 } ra_noise_mode;
 
@@ -65,7 +68,8 @@ typedef struct {
   float C_u;            /* CVaR bound (8b)/(15) PAPER.md:81,:124                              */
   float eta;            /* fraction of zero-mean samples, Alg.1 l.7 PAPER.md:183,:247; [0,1)  */
   int32_t nominal;      /* ra_nominal: q(x), phi(x) of (3)                                    */
-  float nom_p[8];       /* goal {w,gx,gy,w_phi}; track {a,b,half_w,w_lat,w_v,v_ref,w_bdry,w_phi} */
+  float nom_p[12];      /* goal {w,gx,gy,w_phi}; track {a,b,half_w,w_lat,w_v,v_ref,w_bdry,w_phi};
+                           racing {ax,ay,rc,half_w,c1,c2,c3,c4,c5}: rounded-rectangle track, costs (20)-(23) */
   int32_t risk;         /* ra_risk: l(x~) of (9) PAPER.md:93                                  */
   float risk_p[4];      /* circles {weight,margin}; costmap {weight}; linear {weight,index}   */
   int32_t noise_kind;   /* ra_noise_kind                                       */

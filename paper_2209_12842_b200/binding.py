@@ -34,7 +34,7 @@ class ra_mppi_config(C.Structure):
         ("sigma_eps", C.c_float * 2), ("sigma_w", C.c_float * 6),
         ("alpha", C.c_float), ("lam", C.c_float), ("gamma", C.c_float),
         ("A", C.c_float), ("B", C.c_float), ("C_u", C.c_float), ("eta", C.c_float),
-        ("nominal", C.c_int32), ("nom_p", C.c_float * 8),
+        ("nominal", C.c_int32), ("nom_p", C.c_float * 12),
         ("risk", C.c_int32), ("risk_p", C.c_float * 4),
         ("noise_kind", C.c_int32), ("noise_p", C.c_float * 4),
         ("noise_mode", C.c_int32),

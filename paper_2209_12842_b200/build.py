@@ -30,7 +30,7 @@ def _jobs():
     jobs = [(os.path.join(CSRC, "ra_mppi.cu"), os.path.join(OBJ, "ra_mppi.o"), []),
             (os.path.join(CSRC, "pipe_peaks.cu"), os.path.join(OBJ, "pipe_peaks.o"), [])]
     for d in (0, 1):
-        for r in (0, 1, 2):
+        for r in (0, 1, 2, 3):
             jobs.append((os.path.join(CSRC, "rollout_inst.cu"), os.path.join(OBJ, f"rollout_{d}_{r}.o"),
                          [f"-DRA_INST_DYN={d}", f"-DRA_INST_RISK={r}"]))
     return jobs

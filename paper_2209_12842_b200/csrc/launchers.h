@@ -19,9 +19,11 @@ using RolloutLaunchFn = cudaError_t (*)(const Params& p, int noise, int rc, bool
 RA_DECLARE_ROLLOUT(0, 0)
 RA_DECLARE_ROLLOUT(0, 1)
 RA_DECLARE_ROLLOUT(0, 2)
+RA_DECLARE_ROLLOUT(0, 3)
 RA_DECLARE_ROLLOUT(1, 0)
 RA_DECLARE_ROLLOUT(1, 1)
 RA_DECLARE_ROLLOUT(1, 2)
+RA_DECLARE_ROLLOUT(1, 3)
 #undef RA_DECLARE_ROLLOUT
 
 }  // namespace ra

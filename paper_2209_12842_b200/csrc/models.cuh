@@ -113,6 +113,41 @@ __device__ __forceinline__ void dynamics_step(const Params& p, float (&x)[StateD
   }
 }
 
+// ---- the paper's own racing costs (20)-(23), on a rounded-rectangle track -------
+// nom_p = {ax, ay, rc, half_w, c1, c2, c3, c4, c5}; centreline = points at distance rc from the box
+// [-ax,ax] x [-ay,ay].  e = lateral deviation (+ outward), d = half_w - |e| (+ on the track).
+__device__ __forceinline__ float racing_offset(const Params& p, float X, float Y) {
+  const float qx = fabsf(X) - p.nom_p[0], qy = fabsf(Y) - p.nom_p[1];
+  const float ox = fmaxf(qx, 0.0f), oy = fmaxf(qy, 0.0f);
+  float outside;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(outside) : "f"(fmaf(ox, ox, oy * oy)));
+  return outside + fminf(fmaxf(qx, qy), 0.0f) - p.nom_p[2];
+}
+
+// c1 mu_bdry + c3 e^2 : the smooth part of (20); mu_bdry = max(0, atan(-100 d)/pi + 1/2)  (21)
+__device__ __forceinline__ float racing_smooth_cost(const Params& p, float X, float Y) {
+  const float e = racing_offset(p, X, Y);
+  const float d = p.nom_p[3] - fabsf(e);
+  const float mu = fmaxf(0.0f, fmaf(atan2_posx(-100.0f * d, 1.0f), 0.318309886183790672f, 0.5f));
+  return fmaf(p.nom_p[4], mu, p.nom_p[6] * e * e);
+}
+
+// s(x): arc length of the projection onto the centreline, counter-clockwise from (ax+rc, 0)
+__device__ __forceinline__ float racing_arclength(const Params& p, float X, float Y) {
+  const float ax = p.nom_p[0], ay = p.nom_p[1], rc = p.nom_p[2];
+  const float Xa = fabsf(X), Ya = fabsf(Y);
+  const float dx = fmaxf(Xa - ax, 0.0f), dy = fmaxf(Ya - ay, 0.0f);
+  const float quarter_arc = rc * 1.57079632679489662f;
+  const float Pq = ay + quarter_arc + ax;
+  float sq;
+  if (dx > 0.0f && dy > 0.0f) sq = fmaf(rc, atan2_posx(dy, dx), ay);
+  else if (dx > 0.0f) sq = Ya;
+  else if (dy > 0.0f) sq = ay + quarter_arc + (ax - Xa);
+  else sq = ((ax - Xa) < (ay - Ya)) ? Ya : ay + quarter_arc + (ax - Xa);
+  if (X >= 0.0f) return Y >= 0.0f ? sq : 4.0f * Pq - sq;
+  return Y >= 0.0f ? 2.0f * Pq - sq : 2.0f * Pq + sq;
+}
+
 // Nominal running cost q(x) (state part; "arbitrary form" PAPER.md:45) at absolute position
 // (X, Y) = frame origin + x[0..1]; v = x[3].  BASELINE configs 0/3 (goal) and 1/2/4 (track).
 template <int NOM>
@@ -120,6 +155,15 @@ __device__ __forceinline__ float nominal_cost(const Params& p, float Xabs, float
   if constexpr (NOM == NOM_GOAL) {
     const float dx = Xabs - p.nom_p[1], dy = Yabs - p.nom_p[2];
     return p.nom_p[0] * fmaf(dx, dx, dy * dy);
+  } else if constexpr (NOM == NOM_RACING) {
+    // (20): c1 mu_bdry + c2 mu_obs + c3 e^2 with the indicator obstacle cost (22) (K*T evaluations only)
+    float q = racing_smooth_cost(p, Xabs, Yabs);
+    for (int i = 0; i < p.n_circles; ++i) {
+      const float4 c = __ldg(p.circles + i);
+      const float dx = Xabs - c.x, dy = Yabs - c.y;
+      if (fmaf(dx, dx, dy * dy) < c.z * c.z) q += p.nom_p[5];
+    }
+    return q;
   } else {
     const float a = p.nom_p[0], b = p.nom_p[1];
     const float xa = Xabs / a, yb = Yabs / b;
@@ -130,6 +174,23 @@ __device__ __forceinline__ float nominal_cost(const Params& p, float Xabs, float
     const float over = fmaxf(0.0f, fabsf(e) - p.nom_p[2]);
     const float dv = v - p.nom_p[5];
     return fmaf(p.nom_p[3] * e, e, fmaf(p.nom_p[4] * dv, dv, p.nom_p[6] * over * over));
+  }
+}
+
+// Terminal cost phi(x_T): w_phi * q_state (G18), or the paper's (23) phi = c4 - c5 s with
+// s = distance travelled along the centreline since x_0, wrapped to (-P/2, P/2].
+template <int NOM>
+__device__ __forceinline__ float terminal_cost(const Params& p, float Xabs, float Yabs, float v, float x0X,
+                                               float x0Y) {
+  if constexpr (NOM == NOM_RACING) {
+    const float P = 4.0f * (p.nom_p[1] + p.nom_p[2] * 1.57079632679489662f + p.nom_p[0]);
+    float ds = racing_arclength(p, Xabs, Yabs) - racing_arclength(p, x0X, x0Y);
+    if (ds > 0.5f * P) ds -= P;
+    if (ds < -0.5f * P) ds += P;
+    return fmaf(-p.nom_p[8], ds, p.nom_p[7]);
+  } else {
+    const float w_phi = (NOM == NOM_GOAL) ? p.nom_p[3] : p.nom_p[7];
+    return w_phi * nominal_cost<NOM>(p, Xabs, Yabs, v);
   }
 }
 

@@ -78,8 +78,8 @@ const char* validate(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_statu
   if (cfg->K <= 0 || cfg->M <= 0 || cfg->T <= 0) return "K, M, T must be positive";
   if (!(cfg->dt > 0.0f) || !std::isfinite(cfg->dt)) return "dt must be positive";
   if (cfg->dyn != RA_DYN_KINEMATIC_BICYCLE && cfg->dyn != RA_DYN_SINGLE_TRACK) return "unknown dyn";
-  if (cfg->nominal != RA_NOM_GOAL && cfg->nominal != RA_NOM_ELLIPSE_TRACK) return "unknown nominal cost";
-  if (cfg->risk < RA_RISK_CIRCLES || cfg->risk > RA_RISK_LINEAR_STATE) return "unknown risk cost";
+  if (cfg->nominal < RA_NOM_GOAL || cfg->nominal > RA_NOM_RACING) return "unknown nominal cost";
+  if (cfg->risk < RA_RISK_CIRCLES || cfg->risk > RA_RISK_NOMINAL) return "unknown risk cost";
   if (cfg->noise_kind < RA_NOISE_GAUSSIAN || cfg->noise_kind > RA_NOISE_JUMP) return "unknown noise kind";
   if (cfg->noise_mode != RA_NOISE_FUSED && cfg->noise_mode != RA_NOISE_MATERIALISED) return "unknown noise mode";
   if (!(cfg->alpha > 0.0f && cfg->alpha < 1.0f)) return "alpha must be in (0,1) (PAPER.md:87)";
@@ -99,9 +99,12 @@ const char* validate(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_statu
     return "single-track needs m, Iz, vx_floor > 0";
   if (cfg->nominal == RA_NOM_ELLIPSE_TRACK && (!(cfg->nom_p[0] > 0.0f) || !(cfg->nom_p[1] > 0.0f)))
     return "track semi-axes must be positive";
-  if (cfg->risk == RA_RISK_CIRCLES) {
-    if (!env || env->n_circles < 0 || (env->n_circles > 0 && !env->circles)) return "circle risk needs env->circles";
+  const bool uses_circles = cfg->risk == RA_RISK_CIRCLES || cfg->nominal == RA_NOM_RACING;
+  if (uses_circles) {
+    if (!env || env->n_circles < 0 || (env->n_circles > 0 && !env->circles)) return "circle costs need env->circles";
   }
+  if (cfg->nominal == RA_NOM_RACING && (!(cfg->nom_p[0] > 0.0f) || !(cfg->nom_p[1] > 0.0f) || !(cfg->nom_p[2] > 0.0f)))
+    return "racing track needs ax, ay, rc > 0";
   if (cfg->risk == RA_RISK_COSTMAP) {
     if (!env || !env->costmap || env->map_h < 1 || env->map_w < 1 || !(env->map_res > 0.0f))
       return "costmap risk needs env->costmap";
@@ -115,15 +118,16 @@ const char* validate(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_statu
   *st = RA_EUNSUPPORTED;
   if (cfg->M > RA_MAX_M) return "M above RA_MAX_M";
   if (cfg->T > RA_MAX_T) return "T above RA_MAX_T";
-  if (cfg->risk == RA_RISK_CIRCLES && env->n_circles > kMaxCirclesSmem) return "too many circles";
+  if (uses_circles && env->n_circles > kMaxCirclesSmem) return "too many circles";
+  if (cfg->risk == RA_RISK_NOMINAL && cfg->nominal != RA_NOM_RACING) return "l = q is built for the racing costs only";
   *st = RA_OK;
   return nullptr;
 }
 
 RolloutLaunchFn pick_rollout(int dyn, int risk) {
-  static const RolloutLaunchFn table[2][3] = {
-      {launch_rollout_0_0, launch_rollout_0_1, launch_rollout_0_2},
-      {launch_rollout_1_0, launch_rollout_1_1, launch_rollout_1_2}};
+  static const RolloutLaunchFn table[2][4] = {
+      {launch_rollout_0_0, launch_rollout_0_1, launch_rollout_0_2, launch_rollout_0_3},
+      {launch_rollout_1_0, launch_rollout_1_1, launch_rollout_1_2, launch_rollout_1_3}};
   return table[dyn][risk];
 }
 
@@ -207,11 +211,12 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
   c->rollout = pick_rollout(cfg->dyn, cfg->risk);
 
   // environment copies
-  if (cfg->risk == RA_RISK_CIRCLES) {
+  if (cfg->risk == RA_RISK_CIRCLES || cfg->nominal == RA_NOM_RACING) {
+    const float margin = cfg->risk == RA_RISK_CIRCLES ? cfg->risk_p[1] : 0.0f;   // (22) has no margin
     p.n_circles = env->n_circles;
     std::vector<float4> h((size_t)std::max(env->n_circles, 1));
     for (int i = 0; i < env->n_circles; ++i)
-      h[i] = make_float4(env->circles[3 * i], env->circles[3 * i + 1], env->circles[3 * i + 2] + cfg->risk_p[1], 0.0f);
+      h[i] = make_float4(env->circles[3 * i], env->circles[3 * i + 1], env->circles[3 * i + 2] + margin, 0.0f);
     if (cuda_fail(c, dev_alloc(&c->d_circles, h.size()), "alloc circles")) return bail(RA_ENOMEM);
     if (cudaMemcpy(c->d_circles, h.data(), h.size() * sizeof(float4), cudaMemcpyHostToDevice) != cudaSuccess)
       return bail(RA_ECUDA);
@@ -283,10 +288,10 @@ cudaError_t launch_sample_nominal(const ra_mppi_ctx* c, const Params& p, const f
   const int threads = kSampleThreads, grid = (p.K + kSampleKB - 1) / kSampleKB;
   const size_t smem = (size_t)p.T * kSampleKB * (sizeof(float4) + sizeof(float)) + (size_t)2 * p.T * sizeof(float);
   const int dyn = c->cfg.dyn, nom = c->cfg.nominal;
-  if (dyn == 0 && nom == 0) sample_nominal_kernel<0, 0><<<grid, threads, smem, s>>>(p, d_x0, d_v);
-  else if (dyn == 0 && nom == 1) sample_nominal_kernel<0, 1><<<grid, threads, smem, s>>>(p, d_x0, d_v);
-  else if (dyn == 1 && nom == 0) sample_nominal_kernel<1, 0><<<grid, threads, smem, s>>>(p, d_x0, d_v);
-  else sample_nominal_kernel<1, 1><<<grid, threads, smem, s>>>(p, d_x0, d_v);
+#define RA_SN(D, N) sample_nominal_kernel<D, N><<<grid, threads, smem, s>>>(p, d_x0, d_v)
+  if (dyn == 0) { if (nom == 0) RA_SN(0, 0); else if (nom == 1) RA_SN(0, 1); else RA_SN(0, 2); }
+  else { if (nom == 0) RA_SN(1, 0); else if (nom == 1) RA_SN(1, 1); else RA_SN(1, 2); }
+#undef RA_SN
   return cudaGetLastError();
 }
 

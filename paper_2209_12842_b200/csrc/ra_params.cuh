@@ -6,8 +6,8 @@
 namespace ra {
 
 enum : int { DYN_BICYCLE = 0, DYN_SINGLE_TRACK = 1 };
-enum : int { NOM_GOAL = 0, NOM_TRACK = 1 };
-enum : int { RISK_CIRCLES = 0, RISK_COSTMAP = 1, RISK_LINEAR = 2 };
+enum : int { NOM_GOAL = 0, NOM_TRACK = 1, NOM_RACING = 2 };
+enum : int { RISK_CIRCLES = 0, RISK_COSTMAP = 1, RISK_LINEAR = 2, RISK_NOMINAL = 3 };
 enum : int { NOISE_GAUSSIAN = 0, NOISE_UNIFORM = 1, NOISE_JUMP = 2 };
 enum : uint32_t { STREAM_EPS = 0u, STREAM_W = 1u, STREAM_PLANT = 2u };
 
@@ -29,7 +29,7 @@ struct Params {
   float sigma_w[6];
   float neg_log2e_over_lambda;  // weights (17) PAPER.md:134 as exp2
   float A, B, C_u;
-  float nom_p[8];
+  float nom_p[12];
   float risk_p[4];
   float noise_p[4];
   int Jc;           // Philox calls per state step (counter stride)

@@ -73,8 +73,7 @@ __global__ void __launch_bounds__(kSampleThreads) sample_nominal_kernel(const __
     S += (double)q + (double)ctrl_s[t * kSampleKB + threadIdx.x];
     dynamics_step<DYN>(p, x, ce_s[t * kSampleKB + threadIdx.x]);
   }
-  const float w_phi = (NOM == NOM_GOAL) ? p.nom_p[3] : p.nom_p[7];
-  S += (double)(w_phi * nominal_cost<NOM>(p, x0X + x[0], x0Y + x[1], x[3]));
+  S += (double)terminal_cost<NOM>(p, x0X + x[0], x0Y + x[1], x[3], x0X, x0Y);
   p.S[k] = S;
 }
 
@@ -146,7 +145,13 @@ template <int RISK, int RC, int NX>
 __device__ __forceinline__ void risk_accumulate(const Params& p, const float4* circ_s,
                                                 const MapFrame& mf, float x0X, float x0Y,
                                                 const float (&x)[RC][NX], float (&L)[RC]) {
-  if constexpr (RISK == RISK_CIRCLES) {
+  if constexpr (RISK == RISK_CIRCLES || RISK == RISK_NOMINAL) {
+    // RISK_NOMINAL: l = q of the paper's racing costs: smooth part per lane, then the
+    // indicator obstacle cost (22) through the same culled candidate loop as the hinge cost.
+    if constexpr (RISK == RISK_NOMINAL) {
+#pragma unroll
+      for (int r = 0; r < RC; ++r) L[r] += racing_smooth_cost(p, x0X + x[r][0], x0Y + x[r][1]);
+    }
     // Exact culling: the lanes of a warp share u^k and start together, so they stay within a
     // few metres.  Once per step the warp takes the bounding box of all its positions (four
     // warp-wide CREDUX.F32), each lane tests one obstacle of a 32-obstacle batch against the box
@@ -180,10 +185,14 @@ __device__ __forceinline__ void risk_accumulate(const Params& p, const float4* c
           const float dx = x[r][0] - c.x, dy = x[r][1] - c.y;
           const float d2 = fmaf(dx, dx, dy * dy);
           if (d2 < c.w) {
-            float d;
-            asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(d) : "f"(d2));  // 1 ulp; pen = R - d
-            const float pen = c.z - d;
-            L[r] = fmaf(w * pen, pen, L[r]);
+            if constexpr (RISK == RISK_NOMINAL) {
+              L[r] += p.nom_p[5];                                      // c2 * 1[d_i < r_i]  (22)
+            } else {
+              float d;
+              asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(d) : "f"(d2));  // 1 ulp; pen = R - d
+              const float pen = c.z - d;
+              L[r] = fmaf(w * pen, pen, L[r]);
+            }
           }
         }
       }
@@ -222,12 +231,13 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
   constexpr int G = HALF ? 16 : 32;
   extern __shared__ float4 smem4[];
   float4* circ_s = smem4;
-  const int n_circ_s = (RISK == RISK_CIRCLES) ? p.n_circles : 0;
+  constexpr bool kUsesCircles = (RISK == RISK_CIRCLES || RISK == RISK_NOMINAL);
+  const int n_circ_s = kUsesCircles ? p.n_circles : 0;
   uint32_t* keys_all = reinterpret_cast<uint32_t*>(smem4 + n_circ_s);
 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const float x0X = x0g[0], x0Y = x0g[1];
-  if constexpr (RISK == RISK_CIRCLES) {
+  if constexpr (kUsesCircles) {
     for (int i = threadIdx.x; i < p.n_circles; i += blockDim.x) {
       const float4 c = p.circles[i];
       circ_s[i] = make_float4(c.x - x0X, c.y - x0Y, c.z, c.z * c.z);

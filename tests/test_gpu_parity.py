@@ -211,3 +211,52 @@ def test_single_track_floor_and_x0_floor(torch_cuda):
     ctl, orc = _ctl(p), O.Oracle(p)
     g, r = check_rollout_parity(p, ctl, orc)
     assert (g["xT"][..., 3] >= 0.5).all() and (g["xT"][..., 3] == 0.5).any()
+
+
+# ------------------------------------------------------------------ the paper's own racing costs (NEXT row 2)
+def _racing_compare(p, g, r, sl):
+    """Indicator obstacle cost (22) is a float decision: exclude rollouts whose distance to some
+    obstacle rim comes within 1e-5 m of the jump (both answers are then correct), compare the rest."""
+    tie = r["margin"] < 1e-5                       # [n, M+1]: col 0 nominal, 1.. noisy
+    ok_L = ~tie[:, 1:]
+    assert ok_L.mean() > 0.99
+    assert np.abs(g["xT"][sl] - r["xT"]).max() < TOL_STATE_ABS
+    assert np.abs(g["u"][sl] - r["u"]).max() < 2e-6 * max(1.0, np.abs(r["u"]).max())
+    from parity_utils import rel_err
+    assert rel_err(g["L"][sl], r["L"])[ok_L].max() < 1e-4
+    clean = ~tie.any(axis=1)
+    assert clean.mean() > 0.5
+    assert rel_err(g["S"][sl], r["S"])[~tie[:, 0]].max() < 1e-4
+    assert rel_err(g["cvar"][sl], r["cvar"])[clean].max() < 1e-4
+    assert rel_err(g["S_tilde"][sl], r["S_tilde"])[clean].max() < 1e-4
+    return clean
+
+
+def test_paper_racing_costs_l_equals_q(torch_cuda):
+    p = W.paper_racing(K=96, M=300, T=30)          # the paper's M = 300: ragged over 32 lanes
+    p = p.replace(v=W.random_mean_control(p, 4, (0.1, 0.5)))
+    ctl, orc = _ctl(p), O.Oracle(p)
+    g = gpu_outputs(ctl, p)
+    r = orc.rollout_costs(n_threads=8, want_margin=True)
+    clean = _racing_compare(p, g, r, slice(0, p.K))
+    assert (r["cvar"] > p.C_u).mean() > 0.05 and (r["L"] > 1.0).mean() > 0.01      # obstacles / boundary are hit
+    # CVaR select isolated on the GPU's own L, and the update stage isolated
+    k_tail = O.tail_count(p.alpha, p.M)
+    iso = np.array([O.cvar_topk(g["L"][i].astype(np.float64), k_tail) for i in range(p.K)])
+    assert_costs_close(g["cvar"], iso, "CVaR vs sort of GPU L", tol=2e-6)
+    check_update_parity(p, ctl, orc, r)
+    if clean.all():
+        verdict, err = check_step_parity(p, ctl, orc, r)
+        print(f"paper-racing: end-to-end v+ {verdict}")
+    ctl.close()
+
+
+def test_paper_racing_full_size_sampled(torch_cuda):
+    p = W.paper_racing()                           # 1024 x 300 x 30 = the paper's 3.072e5 trajectories
+    p = p.replace(v=W.random_mean_control(p, 5, (0.1, 0.5)))
+    ctl, orc = _ctl(p), O.Oracle(p)
+    g = gpu_outputs(ctl, p)
+    for kb in (0, 800, p.K - 48):                  # 800..848 straddles K0 = ceil(0.8 K) = 820 (eta = 0.2)
+        r = orc.rollout_costs(k_begin=kb, k_end=kb + 48, n_threads=8, want_margin=True)
+        _racing_compare(p, g, r, slice(kb, kb + 48))
+    ctl.close()
