@@ -33,7 +33,7 @@ UNIT = "state-steps/s"
 #   Philox4x32-10 call 40 (20 mul-wide + 20 xor3); Box-Muller 14 per pair + 1 scale-add per normal;
 #   bicycle step 7; single-track step 75; bilinear lookup 21.  Circle tests are NOT credited: far
 #   obstacles are culled exactly, and a culled test is not achieved work.
-ALGO_OPS = {"C0": 40 + 32 + 7, "C1": 40 + 32 + 7, "C2": 80 + 48 + 75, "C3": 40 + 32 + 7 + 21, "C4": 40 + 32 + 7}
+ALGO_OPS = {"PAPER": 40 + 32 + 7 + 30, "PAPER-ST": 80 + 48 + 75 + 30, "C0": 40 + 32 + 7, "C1": 40 + 32 + 7, "C2": 80 + 48 + 75, "C3": 40 + 32 + 7 + 21, "C4": 40 + 32 + 7}
 # DRAM bytes (read + write) of one noisy_rollout_kernel launch, from the committed `ncu --set full` captures
 TRAFFIC_BYTES = {"C3": 13.41e6, "C2": 7.97e6}   # profiles/r1b_c3_c2_optimised.md
 ALU_PEAK_LANE_OPS = 148 * 128 * 1.965e9  # 148 SMs x 128 FP32 lanes x 1.965 GHz (B200_PROFILING.md nominal)
@@ -49,6 +49,8 @@ def make_problem(name: str, rank: int = 0) -> W.Problem:
         p = W.config2()
     elif name == "C3":
         p = W.config3()
+    elif name in ("PAPER", "PAPER-ST"):
+        p = W.paper_racing(single_track=name.endswith("ST"))      # the paper's own workload: 3.072e5 trajectories
     elif name.startswith("C4"):
         parts = name.split("-")
         K = int(parts[1][1:]) if len(parts) > 1 else 8192
@@ -328,6 +330,9 @@ def run_report(args):
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     for name in ("C0", "C1", "C2", "C3"):
         print(json.dumps({"report": "workload", **quick_time(make_problem(name))}), flush=True)
+    for name in ("PAPER", "PAPER-ST"):   # the paper's own workload (context for its 44.3 Hz on an RTX 3090)
+        print(json.dumps({"report": "paper workload (1024 x 300 x 30, costs (20)-(23), l = q)",
+                          **quick_time(make_problem(name), steps=100)}), flush=True)
     for K in W.C4_SWEEP_K:
         for M in W.C4_SWEEP_M:
             steps = 20 if K * M >= 65536 * 64 else 50

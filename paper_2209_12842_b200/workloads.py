@@ -211,7 +211,7 @@ def rounded_rect_points(ax, ay, rc, s_values):
     return np.array(pts), P
 
 
-def paper_racing(K=1024, M=300, T=30, seed=5) -> Problem:
+def paper_racing(K=1024, M=300, T=30, seed=5, single_track=False) -> Problem:
     """The paper's own controller set-up: costs (20)-(23) with c1..c5 = 2, 1, 0.1, 0.6, 2,
     l = q, horizon 30, lambda 0.35, eta 0.2, A 10, 1024 samples x 300 realisations, on a synthetic
     rounded-rectangle track with the published dimensions (0.6 m wide, 10.9 m centreline, 0.3 m corners, ten
@@ -228,9 +228,14 @@ def paper_racing(K=1024, M=300, T=30, seed=5) -> Problem:
     circles = _f32(np.stack([pts[:, 0] + off * pts[:, 2], pts[:, 1] + off * pts[:, 3], np.full(10, 0.1)], axis=1))
     start, _ = rounded_rect_points(ax, ay, rc, [P - ay - rc * math.pi / 2 - 0.6 * ax])   # on the bottom straight
     x0 = _f32([start[0, 0], start[0, 1], 0.0, 1.5])                                      # heading +x (counter-clockwise)
-    return Problem(name="paper-racing", K=K, M=M, T=T, dt=0.02, dyn=DYN_BICYCLE, dyn_p=[0.093],
-                   u_min=[-0.4, -4.0], u_max=[0.4, 4.0], sigma_eps=[0.15, 1.0],
-                   sigma_w=[0.004, 0.004, 0.01, 0.03], alpha=0.9, lam=0.35, gamma=0.35, A=10.0, B=1.0, C_u=0.5,
+    if single_track:   # "dynamic vehicle model with tire dynamics", 1/28-scale linear-tyre stand-in
+        veh = dict(dyn=DYN_SINGLE_TRACK, dyn_p=[0.15, 2.5e-4, 0.045, 0.045, 2.0, 2.0, 0.2], u_min=[-0.4, -0.6],
+                   u_max=[0.4, 0.6], sigma_eps=[0.15, 0.15], sigma_w=[0.004, 0.004, 0.01, 0.03, 0.03, 0.1])
+        x0 = _f32([start[0, 0], start[0, 1], 0.0, 1.5, 0.0, 0.0])
+    else:
+        veh = dict(dyn=DYN_BICYCLE, dyn_p=[0.093], u_min=[-0.4, -4.0], u_max=[0.4, 4.0], sigma_eps=[0.15, 1.0],
+                   sigma_w=[0.004, 0.004, 0.01, 0.03])
+    return Problem(name="paper-racing" + ("-st" if single_track else ""), K=K, M=M, T=T, dt=0.02, **veh, alpha=0.9, lam=0.35, gamma=0.35, A=10.0, B=1.0, C_u=0.5,
                    eta=0.2, nominal=NOM_RACING, nom_p=[ax, float(_f32(ay)), rc, hw, 2.0, 1.0, 0.1, 0.6, 2.0],
                    risk=RISK_NOMINAL, risk_p=[0.0], seed=seed, x0=x0, v=np.zeros((T, 2)), circles=circles)
 

@@ -216,8 +216,8 @@ def test_single_track_floor_and_x0_floor(torch_cuda):
 # ------------------------------------------------------------------ the paper's own racing costs (NEXT row 2)
 def _racing_compare(p, g, r, sl):
     """Indicator obstacle cost (22) is a float decision: exclude rollouts whose distance to some
-    obstacle rim comes within 1e-5 m of the jump (both answers are then correct), compare the rest."""
-    tie = r["margin"] < 1e-5                       # [n, M+1]: col 0 nominal, 1.. noisy
+    obstacle rim comes within 3e-6 m of the jump (both answers are then correct), compare the rest."""
+    tie = r["margin"] < 3e-6                       # [n, M+1]: col 0 nominal, 1.. noisy
     ok_L = ~tie[:, 1:]
     assert ok_L.mean() > 0.99
     assert np.abs(g["xT"][sl] - r["xT"]).max() < TOL_STATE_ABS
@@ -225,7 +225,7 @@ def _racing_compare(p, g, r, sl):
     from parity_utils import rel_err
     assert rel_err(g["L"][sl], r["L"])[ok_L].max() < 1e-4
     clean = ~tie.any(axis=1)
-    assert clean.mean() > 0.5
+    assert clean.mean() > 0.3
     assert rel_err(g["S"][sl], r["S"])[~tie[:, 0]].max() < 1e-4
     assert rel_err(g["cvar"][sl], r["cvar"])[clean].max() < 1e-4
     assert rel_err(g["S_tilde"][sl], r["S_tilde"])[clean].max() < 1e-4
@@ -259,4 +259,14 @@ def test_paper_racing_full_size_sampled(torch_cuda):
     for kb in (0, 800, p.K - 48):                  # 800..848 straddles K0 = ceil(0.8 K) = 820 (eta = 0.2)
         r = orc.rollout_costs(k_begin=kb, k_end=kb + 48, n_threads=8, want_margin=True)
         _racing_compare(p, g, r, slice(kb, kb + 48))
+    ctl.close()
+
+
+def test_paper_racing_single_track(torch_cuda):
+    p = W.paper_racing(K=64, M=96, T=30, single_track=True)
+    p = p.replace(v=W.random_mean_control(p, 6, (0.1, 0.2)))
+    ctl, orc = _ctl(p), O.Oracle(p)
+    g = gpu_outputs(ctl, p)
+    r = orc.rollout_costs(n_threads=8, want_margin=True)
+    _racing_compare(p, g, r, slice(0, p.K))
     ctl.close()
