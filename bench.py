@@ -259,7 +259,7 @@ def run_cuda(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"{p.name} K={p.K} M={p.M} T={p.T}", "baseline_config_index": int(key[1]),
+            "config": {"workload": f"{p.name} K={p.K} M={p.M} T={p.T}", "baseline_config_index": int(key[1]) if key[1:].isdigit() else None,
                        "l2_flush_between_steps": True, "parallelism": "replicas only" if world > 1 else "single GPU",
                        "noise_mode": "fused"},
             "iterations_per_s": world * args.steps / (total_ms * 1e-3),
