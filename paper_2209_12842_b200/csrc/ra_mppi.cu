@@ -179,9 +179,23 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
   c->half = cfg->M <= 16;
   p.G = c->half ? 16 : 32;
   p.R_total = (cfg->M + p.G - 1) / p.G;
-  c->rc = c->half ? 1 : (p.R_total % 4 == 0 ? 4 : (p.R_total % 2 == 0 ? 2 : 1));
+  // Work split of the rollout kernel (measured on B200, profiles/r1c): a warp interleaves RC slots
+  // of 32 realisations per lane (RC = 4 when the slot count divides by 4, else 2), and the
+  // ceil(R_total / RC) groups of one control sample go to as many warps (wps, a power of two <= 8),
+  // so every warp runs one group: shorter CTAs fill the SMs at small K (the paper's 1024 x 300
+  // workload: 5 groups -> 8 warps) and cut the wave tail at large K.
+  p.wps = 1;
+  c->rc = 1;
+  if (!c->half) {
+    c->rc = (p.R_total >= 4 && p.R_total % 4 == 0) ? 4 : (p.R_total >= 2 ? 2 : 1);
+    const int groups = (p.R_total + c->rc - 1) / c->rc;
+    while (p.wps < 8 && p.wps < groups) p.wps *= 2;
+  }
 #ifdef RA_FORCE_RC  // tuning experiments only
-  if (!c->half && p.R_total % RA_FORCE_RC == 0) c->rc = RA_FORCE_RC;
+  if (!c->half) c->rc = RA_FORCE_RC;
+#endif
+#ifdef RA_FORCE_WPS
+  if (!c->half) p.wps = RA_FORCE_WPS;
 #endif
   p.nx = cfg->dyn == RA_DYN_SINGLE_TRACK ? 6 : 4;
   p.dt = cfg->dt;

@@ -18,7 +18,8 @@ struct Params {
   int K0;       // samples k < K0 use u = v + eps, the rest u = eps   (Alg.1 l.7-10)
   int k_tail;   // ceil((1-alpha) M)                                  (Alg.1 l.25)
   int G;        // lanes per control sample: 32, or 16 when M <= 16
-  int R_total;  // realisations per lane = ceil(M / G)
+  int R_total;  // realisation slots of G lanes per sample = ceil(M / G)
+  int wps;      // warps per control sample in the rollout kernel (1, 2, 4 or 8)
   int nx;
   float dt;
   float dyn_p[8];

@@ -247,13 +247,18 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
   MapFrame mf{};
   if constexpr (RISK == RISK_COSTMAP) mf = make_map_frame(p, x0X, x0Y);
 
-  const int gwarp = blockIdx.x * kRolloutWarps + warp;
-  const int k_raw = HALF ? gwarp * 2 + (lane >> 4) : gwarp;
+  // wps warps share one control sample when K alone cannot fill the GPU (small K, large M):
+  // warp ws of the sample takes the realisation chunks ws, ws + wps, ...; the CVaR select runs in
+  // warp 0 of the sample after a CTA barrier.  HALF (two samples per warp) always has wps = 1.
+  const int wps = HALF ? 1 : p.wps;
+  const int sample_in_cta = warp / wps, ws = warp - sample_in_cta * wps;
+  const int sample = blockIdx.x * (kRolloutWarps / wps) + sample_in_cta;
+  const int k_raw = HALF ? sample * 2 + (lane >> 4) : sample;
   const int sub = HALF ? (lane & 15) : lane;
   const uint32_t mask = HALF ? (0xFFFFu << (lane & 16)) : 0xFFFFFFFFu;
   const bool k_valid = k_raw < p.K;
   const int k = k_valid ? k_raw : p.K - 1;
-  uint32_t* keys = keys_all + (size_t)warp * p.R_total * 32;
+  uint32_t* keys = keys_all + (size_t)sample_in_cta * p.R_total * 32;
 
   float x_init[NX];
   x_init[0] = 0.0f; x_init[1] = 0.0f;
@@ -264,7 +269,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
   const uint32_t c3 = iteration_field(p, STREAM_W);
   const float4* ce_k = p.ce + k;
 
-  for (int chunk = 0; chunk < p.R_total; chunk += RC) {
+  for (int chunk = ws * RC; chunk < p.R_total; chunk += wps * RC) {
     float x[RC][NX], L[RC];
     uint32_t m[RC];
 #pragma unroll
@@ -312,7 +317,12 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
       }
     }
   }
-  __syncwarp();
+  if (wps > 1) {
+    __syncthreads();          // every warp of the CTA reaches this exactly once (trip counts may differ)
+    if (ws != 0) return;      // warp 0 of the sample reduces
+  } else {
+    __syncwarp();
+  }
 
   float Lbar;
   float cvar = cvar_select<G>(keys, p.R_total, lane, p.k_tail, p.M, mask, &Lbar);

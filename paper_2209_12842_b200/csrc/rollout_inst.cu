@@ -15,7 +15,7 @@ namespace {
 
 template <int NOISE, int RC, bool HALF>
 cudaError_t launch(const Params& p, const float* d_x0, float* d_L, float* d_xT, cudaStream_t stream) {
-  const int samples_per_cta = HALF ? 2 * kRolloutWarps : kRolloutWarps;
+  const int samples_per_cta = HALF ? 2 * kRolloutWarps : kRolloutWarps / p.wps;
   const int grid = (p.K + samples_per_cta - 1) / samples_per_cta;
   const size_t smem = ((RA_INST_RISK == RISK_CIRCLES || RA_INST_RISK == RISK_NOMINAL) ? (size_t)p.n_circles * sizeof(float4) : 0) +
                       (size_t)kRolloutWarps * p.R_total * 32 * sizeof(uint32_t);
