@@ -323,7 +323,15 @@ cudaError_t launch_materialise(const ra_mppi_ctx* c, const Params& p, cudaStream
 
 // Alg.1 l.3-29: sampling, nominal and noisy rollouts, CVaR, soft filter -> context scratch.
 ra_status enqueue_costs(ra_mppi_ctx* c, const Params& p, const float* d_x0, const float* d_v, float* d_L,
-                        float* d_xT, cudaStream_t s) {
+                        float* d_xT, cudaStream_t s, bool diagnostics) {
+  // A = 0 is the baseline MPPI of section II: S~ = S by (14)-(16), so unless the caller
+  // asks for the risk diagnostics the M noisy rollouts are not needed at all.
+  if (c->cfg.A == 0.0f && !diagnostics) {
+    RA_CUDA(c, launch_sample_nominal(c, p, d_x0, d_v, s));
+    RA_CUDA(c, cudaMemsetAsync(c->d_cvar, 0, (size_t)p.K * sizeof(float), s));
+    RA_CUDA(c, cudaMemcpyAsync(c->d_S_tilde, c->d_S, (size_t)p.K * sizeof(double), cudaMemcpyDeviceToDevice, s));
+    return RA_OK;
+  }
   if (c->cfg.noise_mode == RA_NOISE_MATERIALISED)
     RA_CUDA(c, p.nx == 4 ? launch_materialise<4>(c, p, s) : launch_materialise<6>(c, p, s));
   RA_CUDA(c, launch_sample_nominal(c, p, d_x0, d_v, s));
@@ -367,7 +375,7 @@ ra_status ra_mppi_step(ra_mppi_ctx* c, const float* d_x0, float* d_v, uint64_t i
   if (!d_x0 || !d_v) return fail(c, RA_EINVAL, "null device pointer");
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const Params p = with_iteration(c, iteration);
-  if (ra_status st = enqueue_costs(c, p, d_x0, d_v, nullptr, nullptr, s)) return st;
+  if (ra_status st = enqueue_costs(c, p, d_x0, d_v, nullptr, nullptr, s, false)) return st;
   return enqueue_update(c, p, d_v, s);
 }
 
@@ -378,7 +386,7 @@ ra_status ra_mppi_rollout_costs(ra_mppi_ctx* c, const float* d_x0, const float* 
   if (!d_x0 || !d_v) return fail(c, RA_EINVAL, "null device pointer");
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const Params p = with_iteration(c, iteration);
-  if (ra_status st = enqueue_costs(c, p, d_x0, d_v, d_L, d_xT, s)) return st;
+  if (ra_status st = enqueue_costs(c, p, d_x0, d_v, d_L, d_xT, s, true)) return st;
   if (d_S || d_cvar || d_S_tilde) {
     export_costs_kernel<<<(p.K + 255) / 256, 256, 0, s>>>(p, d_S, d_cvar, d_S_tilde);
     RA_CUDA(c, cudaGetLastError());
@@ -455,6 +463,7 @@ ra_status ra_mppi_export_costs_f64(ra_mppi_ctx* c, double* d_S64, double* d_S_ti
 
 int32_t ra_mppi_launches_per_step(const ra_mppi_ctx* c) {
   if (!c) return 0;
+  if (c->cfg.A == 0.0f) return 2;   // baseline MPPI: sampling/nominal + weights/update
   return 3 + (c->cfg.noise_mode == RA_NOISE_MATERIALISED ? 1 : 0);
 }
 
@@ -518,7 +527,7 @@ ra_status ra_mppi_closed_loop(ra_mppi_ctx* c, float* d_x0, float* d_v, uint64_t 
       p.iter_imm = 0;
       cudaGraph_t graph = nullptr;
       if (cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { st = fail(c, RA_ECUDA, "begin capture"); break; }
-      st = enqueue_costs(c, p, d_x0, d_v, nullptr, nullptr, s);
+      st = enqueue_costs(c, p, d_x0, d_v, nullptr, nullptr, s, false);
       if (st == RA_OK) st = enqueue_update(c, p, d_v, s);
       if (st == RA_OK) st = cuda_fail(c, launch_plant(c, p, d_x0, d_v, nullptr, d_log, c->d_loop, s), "plant");
       cudaError_t e = cudaStreamEndCapture(s, &graph);

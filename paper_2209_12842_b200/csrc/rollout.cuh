@@ -13,6 +13,13 @@ namespace ra {
 #define RA_ROLLOUT_THREADS 256
 #endif
 constexpr int kRolloutThreads = RA_ROLLOUT_THREADS;
+#define RA_PRAGMA_(x) _Pragma(#x)
+#define RA_PRAGMA(x) RA_PRAGMA_(x)
+#ifdef RA_T_UNROLL
+#define RA_T_LOOP_UNROLL RA_PRAGMA(unroll RA_T_UNROLL)
+#else
+#define RA_T_LOOP_UNROLL
+#endif
 constexpr int kRolloutWarps = kRolloutThreads / 32;
 constexpr int NOISE_MATERIALISED = 3;  // rollout-kernel variant that reads w from HBM
 
@@ -280,6 +287,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
       for (int i = 0; i < NX; ++i) x[r][i] = x_init[i];
     }
     float4 ce = __ldg(ce_k);
+    RA_T_LOOP_UNROLL
     for (int t = 0; t < p.T; ++t) {
       const float4 ce_next = __ldg(ce_k + (size_t)min(t + 1, p.T - 1) * p.K);  // prefetch
       risk_accumulate<RISK, RC, NX>(p, circ_s, mf, x0X, x0Y, x, L);            // l(x~_t), pre-step

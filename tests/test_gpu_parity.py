@@ -270,3 +270,22 @@ def test_paper_racing_single_track(torch_cuda):
     r = orc.rollout_costs(n_threads=8, want_margin=True)
     _racing_compare(p, g, r, slice(0, p.K))
     ctl.close()
+
+
+def test_baseline_mppi_mode_skips_the_noisy_rollouts(torch_cuda):
+    """A = 0 is the MPPI of section II: S~ = S, and ra_mppi_step needs no noisy rollout."""
+    torch = torch_cuda
+    p = _with_v(W.small(W.config1(), K=300, M=64, T=25)).replace(A=0.0, lam=50.0)
+    ctl, orc = _ctl(p), O.Oracle(p)
+    assert ctl.launches_per_step == 2
+    d_x0, d_v = ctl.tensor(p.x0), ctl.tensor(p.v)
+    ctl.step(d_x0, d_v, 3)
+    S64, St64 = ctl.costs_f64()
+    torch.cuda.synchronize()
+    assert np.array_equal(S64.cpu().numpy(), St64.cpu().numpy())
+    ref = orc.step(iteration=3, n_threads=8)
+    assert np.abs(d_v.cpu().numpy() - ref).max() < 1e-4
+    # the diagnostic call still runs the risk path and reports CVaR, with S~ = S
+    g, r = check_rollout_parity(p, ctl, orc, iteration=3)
+    assert (g["cvar"] > 0).any() and np.array_equal(g["S"], g["S_tilde"])
+    assert _ctl(p.replace(A=1.0)).launches_per_step == 3
