@@ -28,12 +28,17 @@ from paper_2209_12842_b200 import workloads as W  # noqa: E402
 METRIC = "noisy_state_steps_per_s"
 UNIT = "state-steps/s"
 
-# Algorithmic lane-operations per noisy state-step: the instructions the
-# method itself needs (Philox, normal transform, dynamics, risk cost), one per FP32-lane slot.
-#   Philox4x32-10 call 40 (20 mul-wide + 20 xor3); Box-Muller 14 per pair + 1 scale-add per normal;
-#   bicycle step 7; single-track step 75; bilinear lookup 21.  Circle tests are NOT credited: far
-#   obstacles are culled exactly, and a culled test is not achieved work.
-ALGO_OPS = {"PAPER": 40 + 32 + 7 + 30, "PAPER-ST": 80 + 48 + 75 + 30, "C0": 40 + 32 + 7, "C1": 40 + 32 + 7, "C2": 80 + 48 + 75, "C3": 40 + 32 + 7 + 21, "C4": 40 + 32 + 7}
+# Algorithmic lane-operations per noisy state-step ("What bounds it"): the instructions
+# the method itself needs in its leanest known formulation, one per FP32-lane slot (FFMA = 1).
+#   Philox4x32-10 call 40 (20 mul-wide + 20 xor3); Box-Muller pair 11 (2 exact uniforms at 2 each, lg2, sqrt,
+#   angle FMA, sin, cos, 2 products) => 22 for n_x = 4, 33 for n_x = 6; noise add 1 FMA per component;
+#   bicycle step 7 (sin, cos, 5 FMA-class); single-track step 75; bilinear lookup 18; racing smooth cost 30.
+#   NOT credited: range reductions, address arithmetic, loop control, the CVaR select, and every circle test
+#   (far obstacles are culled exactly, and a culled test is not achieved work).
+_BICYCLE = 40 + 22 + 4 + 7
+_SINGLE_TRACK = 80 + 33 + 6 + 75
+ALGO_OPS = {"PAPER": _BICYCLE + 30, "PAPER-ST": _SINGLE_TRACK + 30, "C0": _BICYCLE, "C1": _BICYCLE, "C2": _SINGLE_TRACK,
+            "C3": _BICYCLE + 18, "C4": _BICYCLE}
 # DRAM bytes (read + write) of one noisy_rollout_kernel launch, from the committed `ncu --set full` captures
 TRAFFIC_BYTES = {"C3": 13.41e6, "C2": 7.97e6}   # profiles/r1b_c3_c2_optimised.md
 ALU_PEAK_LANE_OPS = 148 * 128 * 1.965e9  # 148 SMs x 128 FP32 lanes x 1.965 GHz (B200_PROFILING.md nominal)

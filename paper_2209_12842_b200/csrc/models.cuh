@@ -38,6 +38,23 @@ __device__ __forceinline__ void sincos_cw(float x, float& s, float& c) {
   s = (q & 2) ? -sn : sn;
 }
 
+// sin/cos of the yaw angle inside the K*M*T noisy rollouts: two-term Cody-Waite reduction to
+// [-pi, pi] (exact for |x| < pi, where j = 0) and MUFU.SIN / MUFU.COS (max abs error 2^-21.4 there).
+// Per Euler step that is <= dt v 4e-7 ~ 1e-7 m of position, below the half-ulp rounding (2.4e-7 m at
+// |X| in [4,8) m) that the fp32 position sum makes anyway; 7 instructions instead of 25.
+// The K*T nominal rollout and the plant keep sincos_cw.
+#ifndef RA_DYN_SINCOS_MUFU
+#define RA_DYN_SINCOS_MUFU 1
+#endif
+__device__ __forceinline__ void sincos_mufu(float x, float& s, float& c) {
+  const float jm = fmaf(x, 0.159154943f, 12582912.0f);
+  const float j = jm - 12582912.0f;
+  float r = fmaf(j, -6.28125f, x);
+  r = fmaf(j, -1.9353071795864769e-3f, r);
+  s = __sinf(r);
+  c = __cosf(r);
+}
+
 // atan2(y, x) for x > 0 (the single-track model floors vx at a positive value): one MUFU.RCP and
 // a degree-8 odd polynomial in z = min(|y|,x)/max(|y|,x) (max error 1.3e-7 rad in fp32, fitted on
 // Chebyshev nodes; the linear coefficient is exactly 1 so small slip angles keep relative accuracy).
@@ -81,11 +98,12 @@ __device__ __forceinline__ float4 control_effect(const Params& p, float u0, floa
 template <int DYN> struct StateDim { static constexpr int value = DYN == DYN_SINGLE_TRACK ? 6 : 4; };
 
 // One Euler step in the x0-centred frame.  x: (X,Y,psi,v) or (X,Y,psi,vx,vy,r).
-template <int DYN>
+template <int DYN, bool FAST = false>
 __device__ __forceinline__ void dynamics_step(const Params& p, float (&x)[StateDim<DYN>::value],
                                               const float4 ce) {
   float s, c;
-  sincos_cw(x[2], s, c);
+  if constexpr (FAST && RA_DYN_SINCOS_MUFU) sincos_mufu(x[2], s, c);
+  else sincos_cw(x[2], s, c);
   if constexpr (DYN == DYN_BICYCLE) {
     const float dv = p.dt * x[3];
     x[0] = fmaf(dv, c, x[0]);
@@ -194,18 +212,24 @@ __device__ __forceinline__ float terminal_cost(const Params& p, float Xabs, floa
   }
 }
 
-// Bilinear costmap lookup between cell centres with clamp-to-edge (G26).
-// Layout: the context stores the map as a "quad" grid Q[(H+1)][(W+1)] of float4, where
-// Q[jy][jx] = (c[jy-1][jx-1], c[jy-1][jx], c[jy][jx-1], c[jy][jx]) with indices clamped to the map, so
-// one 16-byte load fetches the four texels of a lookup and clamp-to-edge is baked into the table;
-// only the coordinate is clamped (to [0, W] in the +1-shifted grid).  The grid coordinate is split as
-// (integer bias) + (fractional bias + X_rel / res) so the fraction keeps full precision wherever
-// the vehicle is on the map.
+// Risk-weighted bilinear costmap lookup between cell centres with clamp-to-edge (G26).
+// Layout: the context stores the map as a coefficient grid Q[(H+1)][(W+1)] of float4: with
+// (c00, c01, c10, c11) = (c[jy-1][jx-1], c[jy-1][jx], c[jy][jx-1], c[jy][jx]) (indices clamped to the
+// map, so clamp-to-edge is baked into the table) and w = risk weight,
+//   Q[jy][jx] = w (c00, c01 - c00, c10 - c00, c11 - c10 - c01 + c00)
+// so w * bilinear = a + b tx + c ty + d tx ty is one 16-byte load and three FFMA.  Only the coordinate
+// is clamped (to [0, W] in the +1-shifted grid).  The grid coordinate is split as (integer bias) +
+// (fractional bias + X_rel / res) so the fraction keeps full precision wherever the vehicle is on the
+// map.  floor() is taken on the FMA pipe: gx + 1.5*2^23 rounded down has floor(gx) in its low mantissa
+// bits (valid for |gx| < 2^22; map sizes are validated), so no F2I/I2F touches the XU pipe.
 struct MapFrame {
   float bxf, byf;            // fractional part of (x0 - origin)/res + 1/2
   float lox, hix, loy, hiy;  // clamp bounds of the fractional-frame coordinate
-  int base;                  // (integer bias y) * (W+1) + (integer bias x)
+  uint32_t base;             // (integer bias y) * (W+1) + (integer bias x), less the magic-number bits (mod 2^32)
 };
+
+constexpr float kFloorMagic = 12582912.0f;     // 1.5 * 2^23
+constexpr uint32_t kFloorMagicBits = 0x4B400000u;
 
 __device__ __forceinline__ MapFrame make_map_frame(const Params& p, float x0X, float x0Y) {
   MapFrame f;
@@ -215,19 +239,20 @@ __device__ __forceinline__ MapFrame make_map_frame(const Params& p, float x0X, f
   f.bxf = bx - fx; f.byf = by - fy;
   f.lox = -fx; f.hix = (float)p.map_w - fx;
   f.loy = -fy; f.hiy = (float)p.map_h - fy;
-  f.base = (int)fy * (p.map_w + 1) + (int)fx;
+  const uint32_t stride = (uint32_t)(p.map_w + 1);
+  f.base = (uint32_t)(int)fy * stride + (uint32_t)(int)fx - ((uint32_t)kFloorMagicBits * stride + (uint32_t)kFloorMagicBits);
   return f;
 }
 
-__device__ __forceinline__ float bilinear(const Params& p, const MapFrame& f, float Xrel, float Yrel) {
+__device__ __forceinline__ float bilinear_weighted(const Params& p, const MapFrame& f, float Xrel, float Yrel) {
   const float gx = fminf(fmaxf(fmaf(Xrel, p.map_inv_res, f.bxf), f.lox), f.hix);
   const float gy = fminf(fmaxf(fmaf(Yrel, p.map_inv_res, f.byf), f.loy), f.hiy);
-  const int ix = __float2int_rd(gx), iy = __float2int_rd(gy);
-  const float tx = gx - __int2float_rn(ix), ty = gy - __int2float_rn(iy);
-  const float4 q = __ldg(p.quadmap + (f.base + iy * (p.map_w + 1) + ix));
-  const float top = fmaf(tx, q.y - q.x, q.x);
-  const float bot = fmaf(tx, q.w - q.z, q.z);
-  return fmaf(ty, bot - top, top);
+  const float jx = __fadd_rd(gx, kFloorMagic), jy = __fadd_rd(gy, kFloorMagic);
+  const float tx = gx - (jx - kFloorMagic), ty = gy - (jy - kFloorMagic);
+  // all index arithmetic is mod 2^32; the sum is the absolute table index in [0, (H+1)(W+1))
+  const uint32_t idx = __float_as_uint(jy) * (uint32_t)(p.map_w + 1) + __float_as_uint(jx) + f.base;
+  const float4 q = __ldg(p.quadmap + idx);
+  return fmaf(ty, fmaf(tx, q.w, q.z), fmaf(tx, q.y, q.x));
 }
 
 }  // namespace ra

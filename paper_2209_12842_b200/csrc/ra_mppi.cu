@@ -108,6 +108,7 @@ const char* validate(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_statu
   if (cfg->risk == RA_RISK_COSTMAP) {
     if (!env || !env->costmap || env->map_h < 1 || env->map_w < 1 || !(env->map_res > 0.0f))
       return "costmap risk needs env->costmap";
+    if (env->map_h > (1 << 20) || env->map_w > (1 << 20)) return "costmap side above 2^20 cells";
   }
   if (cfg->risk == RA_RISK_LINEAR_STATE) {
     const int nx = cfg->dyn == RA_DYN_SINGLE_TRACK ? 6 : 4;
@@ -208,6 +209,13 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
   std::memcpy(p.risk_p, cfg->risk_p, sizeof p.risk_p);
   std::memcpy(p.noise_p, cfg->noise_p, sizeof p.noise_p);
   std::memcpy(p.sigma_w, cfg->sigma_w, sizeof p.sigma_w);
+  {
+    // rng.cuh: Gaussian a = sqrt(-log2 u1)(cos, sin)(2 pi (u2 - 1/2)) = -z / sqrt(2 ln 2); uniform a = z;
+    // jump a = -(unit direction)
+    const double c = cfg->noise_kind == RA_NOISE_GAUSSIAN ? -std::sqrt(2.0 * std::log(2.0))
+                     : (cfg->noise_kind == RA_NOISE_JUMP ? -1.0 : 1.0);
+    for (int i = 0; i < 6; ++i) p.wscale[i] = (float)(c * (double)cfg->sigma_w[i]);
+  }
   for (int i = 0; i < 2; ++i) {
     p.u_min[i] = cfg->u_min[i]; p.u_max[i] = cfg->u_max[i];
     p.sigma_eps[i] = cfg->sigma_eps[i];
@@ -237,18 +245,22 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
     p.circles = c->d_circles;
   }
   if (cfg->risk == RA_RISK_COSTMAP) {
-    // quad-texel table (models.cuh): Q[jy][jx] = the four texels around grid corner (jx-1/2, jy-1/2)
+    // risk-weighted bilinear coefficient table (models.cuh) around grid corner (jx-1/2, jy-1/2)
     const int H = env->map_h, Wd = env->map_w;
     const size_t n = (size_t)(H + 1) * (Wd + 1);
     std::vector<float4> q(n);
     auto at = [&](int iy, int ix) {
       iy = iy < 0 ? 0 : (iy > H - 1 ? H - 1 : iy);
       ix = ix < 0 ? 0 : (ix > Wd - 1 ? Wd - 1 : ix);
-      return env->costmap[(size_t)iy * Wd + ix];
+      return (double)env->costmap[(size_t)iy * Wd + ix];
     };
+    const double w = (double)cfg->risk_p[0];
     for (int jy = 0; jy <= H; ++jy)
-      for (int jx = 0; jx <= Wd; ++jx)
-        q[(size_t)jy * (Wd + 1) + jx] = make_float4(at(jy - 1, jx - 1), at(jy - 1, jx), at(jy, jx - 1), at(jy, jx));
+      for (int jx = 0; jx <= Wd; ++jx) {
+        const double c00 = at(jy - 1, jx - 1), c01 = at(jy - 1, jx), c10 = at(jy, jx - 1), c11 = at(jy, jx);
+        q[(size_t)jy * (Wd + 1) + jx] = make_float4((float)(w * c00), (float)(w * (c01 - c00)), (float)(w * (c10 - c00)),
+                                                    (float)(w * (c11 - c10 - c01 + c00)));
+      }
     if (cuda_fail(c, dev_alloc(&c->d_costmap, n), "alloc costmap")) return bail(RA_ENOMEM);
     if (cudaMemcpy(c->d_costmap, q.data(), n * sizeof(float4), cudaMemcpyHostToDevice) != cudaSuccess)
       return bail(RA_ECUDA);

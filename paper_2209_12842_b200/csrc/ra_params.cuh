@@ -28,6 +28,7 @@ struct Params {
   float sigma_eps[2];
   float ctrl_w[2];  // gamma / sigma_eps^2 (0 where sigma_eps == 0)   (3) PAPER.md:47
   float sigma_w[6];
+  float wscale[6];   // additive noise of (6): w_i = wscale[i] * a_i, a = state_noise() (rng.cuh)
   float neg_log2e_over_lambda;  // weights (17) PAPER.md:134 as exp2
   float A, B, C_u;
   float nom_p[12];

@@ -74,16 +74,19 @@ __device__ __forceinline__ void box_muller(uint32_t ra, uint32_t rb, float& z0, 
 // cos.approx).  Error budget: |dz| <= ~2e-6 |z| + 2e-7 / max(rho, 1e-3); scaled by
 // sigma_w <= 0.05 that is <= 1e-7 m per step, below the fp32 rounding of the positions themselves.
 //   u1 = as_float(0x3F800000 | n1) - (1 - 2^-23) = (n1 + 1) 2^-23      (one funnel shift + one FADD)
-//   angle = 2 pi (u2 - 1/2) in [-pi, pi) where MUFU.SIN/COS are most accurate; the half-turn offset
-//   flips both signs, folded into rho.
-__device__ __forceinline__ void box_muller_fast(uint32_t ra, uint32_t rb, float& z0, float& z1) {
+//   angle = 2 pi (u2 - 1/2) in [-pi, pi) where MUFU.SIN/COS are most accurate (one funnel shift + one
+//   FFMA); the half-turn offset flips both signs.
+// Returns the UNSCALED pair (a0, a1) = sqrt(-log2 u1) (cos, sin)(angle); the normals are
+// z = -sqrt(2 ln 2) a, and that constant is folded into Params::wscale together with sigma_w, so the
+// caller's x += wscale * a is one FFMA per component (12 instructions per pair, 4 of them MUFU).
+__device__ __forceinline__ void box_muller_fast(uint32_t ra, uint32_t rb, float& a0, float& a1) {
   const float u1 = __uint_as_float(__funnelshift_r(ra, 0x7Fu, 9)) - 0.99999988079071044921875f;
-  float lg, rho;
+  float lg, s;
   asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lg) : "f"(u1));
-  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(rho) : "f"(lg * -1.3862943611198906f));  // sqrt(-2 ln u1)
-  const float th = (__uint_as_float(__funnelshift_r(rb, 0x7Fu, 9)) - 1.5f) * 6.283185307179586f;
-  z0 = -rho * __cosf(th);
-  z1 = -rho * __sinf(th);
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(s) : "f"(-lg));
+  const float th = fmaf(__uint_as_float(__funnelshift_r(rb, 0x7Fu, 9)), 6.283185307179586f, -9.42477796076938f);
+  a0 = s * __cosf(th);
+  a1 = s * __sinf(th);
 }
 
 // Uniform on (-1,1): (2 (r>>9) + 1) 2^-23 - 1, exact.
@@ -91,8 +94,9 @@ __device__ __forceinline__ float sym_uniform(uint32_t r) {
   return fmaf(__uint2float_rn(2u * (r >> 9) + 1u), 1.1920928955078125e-07f, -1.0f);
 }
 
-// The n_x per-step state-noise values z (before the sigma_w scale) of realisation (k,m) at
-// step t.  NX = 4 -> one Philox call, NX = 6 -> two.  Jump noise makes one more call.
+// The n_x per-step state-noise factors a of realisation (k,m) at step t; the additive noise of (6)
+// PAPER.md:63 is w_i = Params::wscale[i] * a[i] (wscale = sigma_w times the constant of the noise
+// kind, built by ra_mppi_create).  NX = 4 -> one Philox call, NX = 6 -> two.  Jump noise makes one more.
 template <int NX, int NOISE>
 __device__ __forceinline__ void state_noise(const Params& p, uint32_t k, uint32_t m, uint32_t t,
                                             uint32_t c3, float (&z)[NX]) {
@@ -115,6 +119,8 @@ __device__ __forceinline__ void state_noise(const Params& p, uint32_t k, uint32_
     }
   }
   if constexpr (NOISE == NOISE_JUMP) {
+    // jump of unit length in a uniformly random direction z/|z| (the common factor of the Gaussian
+    // draws cancels; its sign is in wscale), with probability noise_p[0]  (G29)
     const uint4 jr = philox4x32_10(k, m, c2 + (uint32_t)J, c3, p.rk);
     const float uj = __uint2float_rn(jr.x >> 9) * 1.1920928955078125e-07f;
     float n2 = 0.0f;

@@ -206,7 +206,7 @@ __device__ __forceinline__ void risk_accumulate(const Params& p, const float4* c
     }
   } else if constexpr (RISK == RISK_COSTMAP) {
 #pragma unroll
-    for (int r = 0; r < RC; ++r) L[r] = fmaf(p.risk_p[0], bilinear(p, mf, x[r][0], x[r][1]), L[r]);
+    for (int r = 0; r < RC; ++r) L[r] += bilinear_weighted(p, mf, x[r][0], x[r][1]);
   } else {  // test-only linear risk: weight * x[index]
     const int idx = (int)p.risk_p[1];
 #pragma unroll
@@ -300,12 +300,11 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
           for (int i = 0; i < NX; ++i) z[i] = __ldg(wp + (size_t)i * p.M_pad);
         } else {
           state_noise<NX, NOISE>(p, (uint32_t)k, m[r], (uint32_t)t, c3, z);
-#pragma unroll
-          for (int i = 0; i < NX; ++i) z[i] *= p.sigma_w[i];
         }
-        dynamics_step<DYN>(p, x[r], ce);   // x~_{t+1} = F(x~_t, u_t) + w_t   (6) PAPER.md:63
+        dynamics_step<DYN, true>(p, x[r], ce);   // x~_{t+1} = F(x~_t, u_t) + w_t   (6) PAPER.md:63
 #pragma unroll
-        for (int i = 0; i < NX; ++i) x[r][i] += z[i];
+        for (int i = 0; i < NX; ++i)
+          x[r][i] = (NOISE == NOISE_MATERIALISED) ? x[r][i] + z[i] : fmaf(p.wscale[i], z[i], x[r][i]);
         if constexpr (DYN == DYN_SINGLE_TRACK) x[r][3] = fmaxf(x[r][3], p.dyn_p[6]);
       }
       ce = ce_next;

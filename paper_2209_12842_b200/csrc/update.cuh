@@ -141,7 +141,7 @@ __global__ void __launch_bounds__(128) plant_shift_kernel(const __grid_constant_
     state_noise<NX, NOISE>(p, 0u, 0u, 0u, iteration_field(p, STREAM_PLANT), z);
     dynamics_step<DYN>(p, x, ce);
 #pragma unroll
-    for (int i = 0; i < NX; ++i) x[i] = fmaf(p.sigma_w[i], z[i], x[i]);
+    for (int i = 0; i < NX; ++i) x[i] = fmaf(p.wscale[i], z[i], x[i]);
     if constexpr (DYN == DYN_SINGLE_TRACK) x[3] = fmaxf(x[3], p.dyn_p[6]);
     x[0] += x0X; x[1] += x0Y;
 #pragma unroll
@@ -173,7 +173,7 @@ __global__ void noise_probe_kernel(const __grid_constant__ Params p, const int* 
   state_noise<NX, NOISE>(p, (uint32_t)kmt[3 * i], (uint32_t)kmt[3 * i + 1], (uint32_t)kmt[3 * i + 2],
                          iteration_field(p, STREAM_W), z);
 #pragma unroll
-  for (int j = 0; j < NX; ++j) w[(size_t)i * NX + j] = z[j] * p.sigma_w[j];
+  for (int j = 0; j < NX; ++j) w[(size_t)i * NX + j] = z[j] * p.wscale[j];
 }
 
 // Materialised-noise generator: w[K][T][NX][M_pad] = sigma_w (.) z, the same draws the fused
@@ -192,7 +192,7 @@ __global__ void __launch_bounds__(256) materialise_noise_kernel(const __grid_con
     state_noise<NX, NOISE>(p, (uint32_t)k, (uint32_t)m, (uint32_t)t, c3, z);
     float* o = w + (size_t)kt * NX * p.M_pad + m;
 #pragma unroll
-    for (int j = 0; j < NX; ++j) o[(size_t)j * p.M_pad] = z[j] * p.sigma_w[j];
+    for (int j = 0; j < NX; ++j) o[(size_t)j * p.M_pad] = z[j] * p.wscale[j];
   }
 }
 
