@@ -44,7 +44,7 @@ struct Params {
   float map_inv_res, map_ox, map_oy;
   // scratch owned by the context
   float2* u_raw;   // [T][K] sampled controls u^k_t (unclamped)
-  float4* ce;      // [T][K] control effects consumed by the rollout kernels
+  float4* ce;      // [K][T] control effects consumed by the rollout kernels
   double* S;        // [K] nominal cost (3), fp64 so weight errors come from q, not from the sum
   float* cvar;      // [K]
   double* S_tilde;  // [K] modified cost (16)

@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(kSampleThreads) sample_nominal_kernel(const __
     const float u1 = fmaf(p.sigma_eps[1], z1, with_mean ? v1 : 0.0f);
     const float4 ce = control_effect<DYN>(p, u0, u1);
     p.u_raw[(size_t)t * p.K + k] = make_float2(u0, u1);
-    p.ce[(size_t)t * p.K + k] = ce;
+    p.ce[(size_t)k * p.T + t] = ce;
     ce_s[idx] = ce;
     ctrl_s[idx] = fmaf(p.ctrl_w[0] * v0, u0, p.ctrl_w[1] * v1 * u1);   // gamma v^T Sigma^-1 u  (3)
   }
@@ -222,7 +222,8 @@ __device__ __forceinline__ void risk_accumulate(const Params& p, const float4* c
 
 // ---------------------------------------------------------------------------------------
 // A3-A7.  HALF: two control samples per warp (G = 16 lanes each, M <= 16).
-// Dynamic shared memory: [n_circles] float4 obstacle records, then per warp R_total*32 keys.
+// Dynamic shared memory: [n_circles] float4 obstacle records, [samples per CTA][T] float4 control
+// effects, then per warp R_total*32 keys.
 // ---------------------------------------------------------------------------------------
 #ifndef RA_MIN_CTAS_BICYCLE
 #define RA_MIN_CTAS_BICYCLE 3   // measured: 3 CTAs (<= 80 regs) beats 4-6 (throughput-, not latency-bound)
@@ -240,7 +241,14 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
   float4* circ_s = smem4;
   constexpr bool kUsesCircles = (RISK == RISK_CIRCLES || RISK == RISK_NOMINAL);
   const int n_circ_s = kUsesCircles ? p.n_circles : 0;
-  uint32_t* keys_all = reinterpret_cast<uint32_t*>(smem4 + n_circ_s);
+  // wps warps share one control sample when K alone cannot fill the GPU (small K, large M):
+  // warp ws of the sample takes the realisation chunks ws, ws + wps, ...; the CVaR select runs in
+  // warp 0 of the sample after a CTA barrier.  HALF (two samples per warp) always has wps = 1.
+  const int wps = HALF ? 1 : p.wps;
+  constexpr int kCeSlotsMax = HALF ? 2 * kRolloutWarps : kRolloutWarps;
+  const int ce_slots = HALF ? kCeSlotsMax : kRolloutWarps / wps;
+  float4* ce_all = smem4 + n_circ_s;                                   // [ce_slots][T] control effects
+  uint32_t* keys_all = reinterpret_cast<uint32_t*>(ce_all + (size_t)ce_slots * p.T);
 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const float x0X = x0g[0], x0Y = x0g[1];
@@ -249,15 +257,10 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
       const float4 c = p.circles[i];
       circ_s[i] = make_float4(c.x - x0X, c.y - x0Y, c.z, c.z * c.z);
     }
-    __syncthreads();
   }
   MapFrame mf{};
   if constexpr (RISK == RISK_COSTMAP) mf = make_map_frame(p, x0X, x0Y);
 
-  // wps warps share one control sample when K alone cannot fill the GPU (small K, large M):
-  // warp ws of the sample takes the realisation chunks ws, ws + wps, ...; the CVaR select runs in
-  // warp 0 of the sample after a CTA barrier.  HALF (two samples per warp) always has wps = 1.
-  const int wps = HALF ? 1 : p.wps;
   const int sample_in_cta = warp / wps, ws = warp - sample_in_cta * wps;
   const int sample = blockIdx.x * (kRolloutWarps / wps) + sample_in_cta;
   const int k_raw = HALF ? sample * 2 + (lane >> 4) : sample;
@@ -267,6 +270,16 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
   const int k = k_valid ? k_raw : p.K - 1;
   uint32_t* keys = keys_all + (size_t)sample_in_cta * p.R_total * 32;
 
+  // The T control effects of sample k (one contiguous row of ce[K][T]) go to shared memory once, so the
+  // step loop reads them with a broadcast LDS instead of a dependent L2 load per step.
+  const float4* ce_s = ce_all + (size_t)(HALF ? warp * 2 + (lane >> 4) : sample_in_cta) * p.T;
+  if (ws == 0) {
+    float4* dst = const_cast<float4*>(ce_s);
+    const float4* src = p.ce + (size_t)k * p.T;
+    for (int t = sub; t < p.T; t += G) dst[t] = __ldg(src + t);
+  }
+  __syncthreads();
+
   float x_init[NX];
   x_init[0] = 0.0f; x_init[1] = 0.0f;
 #pragma unroll
@@ -274,7 +287,6 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
   if constexpr (DYN == DYN_SINGLE_TRACK) x_init[3] = fmaxf(x_init[3], p.dyn_p[6]);
 
   const uint32_t c3 = iteration_field(p, STREAM_W);
-  const float4* ce_k = p.ce + k;
 
   for (int chunk = ws * RC; chunk < p.R_total; chunk += wps * RC) {
     float x[RC][NX], L[RC];
@@ -286,10 +298,9 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
 #pragma unroll
       for (int i = 0; i < NX; ++i) x[r][i] = x_init[i];
     }
-    float4 ce = __ldg(ce_k);
     RA_T_LOOP_UNROLL
     for (int t = 0; t < p.T; ++t) {
-      const float4 ce_next = __ldg(ce_k + (size_t)min(t + 1, p.T - 1) * p.K);  // prefetch
+      const float4 ce = ce_s[t];
       risk_accumulate<RISK, RC, NX>(p, circ_s, mf, x0X, x0Y, x, L);            // l(x~_t), pre-step
 #pragma unroll
       for (int r = 0; r < RC; ++r) {
@@ -307,7 +318,6 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
           x[r][i] = (NOISE == NOISE_MATERIALISED) ? x[r][i] + z[i] : fmaf(p.wscale[i], z[i], x[r][i]);
         if constexpr (DYN == DYN_SINGLE_TRACK) x[r][3] = fmaxf(x[r][3], p.dyn_p[6]);
       }
-      ce = ce_next;
     }
 #pragma unroll
     for (int r = 0; r < RC; ++r) {
