@@ -102,16 +102,16 @@ __device__ __forceinline__ float group_sum(float v, uint32_t mask) {
 
 // ---------------------------------------------------------------------------------------
 // A6: CVaR_k = mean of the k_tail largest of the M risk costs (Alg.1 l.25-26 PAPER.md:204-207,
-// (12) :107), by a bitwise radix select on order-preserving keys: 32 rounds of
-// (compare, warp REDUX) find the k_tail-th largest value exactly; the tail sum is then
-// sum(values above it) + (k_tail - count above) * it, which does not depend on which of
-// several tied values are "picked".  keys: R_total slots per lane in shared memory
-// (slot r of lane l at keys[r*32 + l]; key 0 marks an unused slot).
-// Returns CVaR of the raw costs; *mean_out = (1/M) sum (for (18)-(19)).
+// (12) :107) on order-preserving keys.  keys: R_total slots per lane in shared memory (slot r of
+// lane l at keys[r*32 + l]; key 0 marks an unused slot).  Both selectors work on VALUES, so the
+// result does not depend on which of several tied realisations are "picked".
+//   radix: 32 rounds of (compare, warp REDUX) find the k_tail-th largest value exactly; the tail sum is
+//          sum(values above it) + (k_tail - count above) * it.  Any k_tail, any R_total.
+// Returns CVaR of the raw costs; *mean_out = (1/M) sum (for (18)-(19)) when want_mean.
 // ---------------------------------------------------------------------------------------
 template <int G>
-__device__ __forceinline__ float cvar_select(const uint32_t* keys, int R_total, int lane, int k_tail,
-                                             int M, uint32_t mask, float* mean_out) {
+__device__ __forceinline__ float cvar_select_radix(const uint32_t* keys, int R_total, int lane, int k_tail,
+                                                   uint32_t mask) {
   uint32_t prefix = 0u;
   int k_rem = k_tail;
   for (int bit = 31; bit >= 0; --bit) {
@@ -122,17 +122,62 @@ __device__ __forceinline__ float cvar_select(const uint32_t* keys, int R_total, 
     if (cnt >= k_rem) prefix |= (1u << bit); else k_rem -= cnt;
   }
   // prefix = key of the k_tail-th largest; k_rem = how many copies of it belong to the tail
-  float sum_gt = 0.0f, sum_all = 0.0f;
+  float sum_gt = 0.0f;
   for (int r = 0; r < R_total; ++r) {
     const uint32_t key = keys[r * 32 + lane];
-    const float val = key ? key_float(key) : 0.0f;
-    sum_all += val;
-    sum_gt += (key > prefix) ? val : 0.0f;
+    sum_gt += (key > prefix) ? key_float(key) : 0.0f;
   }
   sum_gt = group_sum<G>(sum_gt, mask);
-  sum_all = group_sum<G>(sum_all, mask);
-  *mean_out = sum_all / (float)M;
   return fmaf((float)k_rem, key_float(prefix), sum_gt) / (float)k_tail;
+}
+
+// Small tails (k_tail <= kTopkMaxTail, at most kTopkSlots slots per lane: every BASELINE config):
+// repeated max extraction on keys held in registers.  Each round takes the largest remaining value
+// with one REDUX.MAX, counts its copies with one REDUX.ADD, adds min(copies, k_rem) of it to the tail sum
+// and clears them -- at most k_tail rounds of ~4 instructions per slot, instead of 32 radix rounds.
+constexpr int kTopkSlots = 8;       // M <= 256 with 32 lanes per sample
+constexpr int kTopkMaxTail = 40;
+template <int G>
+__device__ __forceinline__ float cvar_select_topk(const uint32_t* keys, int R_total, int lane, int k_tail,
+                                                  uint32_t mask) {
+  uint32_t key[kTopkSlots];
+#pragma unroll
+  for (int r = 0; r < kTopkSlots; ++r) key[r] = (r < R_total) ? keys[r * 32 + lane] : 0u;
+  float sum = 0.0f;
+  int k_rem = k_tail;
+  while (k_rem > 0) {
+    uint32_t top = key[0];
+#pragma unroll
+    for (int r = 1; r < kTopkSlots; ++r) top = max(top, key[r]);
+    top = __reduce_max_sync(mask, top);
+    int cnt = 0;
+#pragma unroll
+    for (int r = 0; r < kTopkSlots; ++r) {
+      const bool is_top = key[r] == top;
+      cnt += is_top ? 1 : 0;
+      key[r] = is_top ? 0u : key[r];
+    }
+    cnt = __reduce_add_sync(mask, cnt);
+    const int take = min(cnt, k_rem);
+    sum = fmaf((float)take, key_float(top), sum);
+    k_rem -= take;
+  }
+  return sum / (float)k_tail;
+}
+
+template <int G>
+__device__ __forceinline__ float cvar_select(const uint32_t* keys, int R_total, int lane, int k_tail,
+                                             int M, uint32_t mask, bool want_mean, float* mean_out) {
+  if (want_mean) {   // (18)-(19) need the sample mean only when B != 1
+    float sum_all = 0.0f;
+    for (int r = 0; r < R_total; ++r) {
+      const uint32_t key = keys[r * 32 + lane];
+      sum_all += key ? key_float(key) : 0.0f;
+    }
+    *mean_out = group_sum<G>(sum_all, mask) / (float)M;
+  }
+  if (R_total <= kTopkSlots && k_tail <= kTopkMaxTail) return cvar_select_topk<G>(keys, R_total, lane, k_tail, mask);
+  return cvar_select_radix<G>(keys, R_total, lane, k_tail, mask);
 }
 
 // Warp-wide float min / max in one instruction: redux.sync.{min,max}.f32 (sm_100a; SASS CREDUX).
@@ -148,8 +193,10 @@ __device__ __forceinline__ float warp_max_f32(float v) {
 }
 
 // Risk running cost l(x~) (9) PAPER.md:93 for RC interleaved realisations of one lane.
+// RISK_CIRCLES accumulates the UNWEIGHTED sum of squared penetrations; the kernel applies the weight
+// risk_p[0] once after the horizon loop.
 template <int RISK, int RC, int NX>
-__device__ __forceinline__ void risk_accumulate(const Params& p, const float4* circ_s,
+__device__ __forceinline__ void risk_accumulate(const Params& p, const float4* circ_s, int n_circ_pad, int lane,
                                                 const MapFrame& mf, float x0X, float x0Y,
                                                 const float (&x)[RC][NX], float (&L)[RC]) {
   if constexpr (RISK == RISK_CIRCLES || RISK == RISK_NOMINAL) {
@@ -161,10 +208,11 @@ __device__ __forceinline__ void risk_accumulate(const Params& p, const float4* c
     }
     // Exact culling: the lanes of a warp share u^k and start together, so they stay within a
     // few metres.  Once per step the warp takes the bounding box of all its positions (four
-    // warp-wide CREDUX.F32), each lane tests one obstacle of a 32-obstacle batch against the box
-    // (inflated by 1e-4 so fp32 rounding can only add candidates), and every lane then evaluates
-    // only the balloted candidates.  A culled obstacle contributes exactly 0 to every lane.
-    const float w = p.risk_p[0];
+    // warp-wide CREDUX.F32), each lane tests one obstacle of a 32-obstacle batch against the box, and
+    // every lane then evaluates only the balloted candidates.  The box distance uses the same
+    // subtract / FMA structure as the per-lane distance below and fp32 rounding is monotone, so
+    // box_d2 <= d2 holds exactly for every lane: a culled obstacle contributes exactly 0.  The staged
+    // list is padded to a multiple of 32 with records of R^2 = 0, which are never near.
     float lox = x[0][0], hix = x[0][0], loy = x[0][1], hiy = x[0][1];
 #pragma unroll
     for (int r = 1; r < RC; ++r) {
@@ -173,32 +221,34 @@ __device__ __forceinline__ void risk_accumulate(const Params& p, const float4* c
     }
     lox = warp_min_f32(lox); hix = warp_max_f32(hix);
     loy = warp_min_f32(loy); hiy = warp_max_f32(hiy);
-    const int lane = threadIdx.x & 31;
-    for (int base = 0; base < p.n_circles; base += 32) {
-      const int j = base + lane;
-      bool near = false;
-      if (j < p.n_circles) {
-        const float4 c = circ_s[j];  // (cx - x0X, cy - x0Y, r + margin, (r + margin)^2)
-        const float ddx = fmaxf(fmaxf(lox - c.x, c.x - hix), 0.0f);
-        const float ddy = fmaxf(fmaxf(loy - c.y, c.y - hiy), 0.0f);
-        near = fmaf(ddx, ddx, ddy * ddy) < c.w * 1.0001f;
-      }
-      uint32_t cand = __ballot_sync(0xFFFFFFFFu, near);
+    for (int base = 0; base < n_circ_pad; base += 32) {
+      const float4 cb = circ_s[base + lane];  // (cx - x0X, cy - x0Y, r + margin, (r + margin)^2)
+      const float ddx = fmaxf(fmaxf(lox - cb.x, cb.x - hix), 0.0f);
+      const float ddy = fmaxf(fmaxf(loy - cb.y, cb.y - hiy), 0.0f);
+      uint32_t cand = __ballot_sync(0xFFFFFFFFu, fmaf(ddx, ddx, ddy * ddy) < cb.w);
       while (cand) {
         const float4 c = circ_s[base + __ffs(cand) - 1];  // broadcast
         cand &= cand - 1u;
+        float d2[RC];
+        bool hit = false;
 #pragma unroll
         for (int r = 0; r < RC; ++r) {
           const float dx = x[r][0] - c.x, dy = x[r][1] - c.y;
-          const float d2 = fmaf(dx, dx, dy * dy);
-          if (d2 < c.w) {
-            if constexpr (RISK == RISK_NOMINAL) {
-              L[r] += p.nom_p[5];                                      // c2 * 1[d_i < r_i]  (22)
-            } else {
-              float d;
-              asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(d) : "f"(d2));  // 1 ulp; pen = R - d
-              const float pen = c.z - d;
-              L[r] = fmaf(w * pen, pen, L[r]);
+          d2[r] = fmaf(dx, dx, dy * dy);
+          hit = hit || (d2[r] < c.w);
+        }
+        if (__any_sync(0xFFFFFFFFu, hit)) {   // most candidates of the box touch no realisation
+#pragma unroll
+          for (int r = 0; r < RC; ++r) {
+            if (d2[r] < c.w) {
+              if constexpr (RISK == RISK_NOMINAL) {
+                L[r] += p.nom_p[5];                                      // c2 * 1[d_i < r_i]  (22)
+              } else {
+                float d;
+                asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(d) : "f"(d2[r]));  // 1 ulp; pen = R - d
+                const float pen = c.z - d;
+                L[r] = fmaf(pen, pen, L[r]);
+              }
             }
           }
         }
@@ -240,7 +290,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
   extern __shared__ float4 smem4[];
   float4* circ_s = smem4;
   constexpr bool kUsesCircles = (RISK == RISK_CIRCLES || RISK == RISK_NOMINAL);
-  const int n_circ_s = kUsesCircles ? p.n_circles : 0;
+  const int n_circ_s = kUsesCircles ? ((p.n_circles + 31) & ~31) : 0;   // padded to whole 32-obstacle batches
   // wps warps share one control sample when K alone cannot fill the GPU (small K, large M):
   // warp ws of the sample takes the realisation chunks ws, ws + wps, ...; the CVaR select runs in
   // warp 0 of the sample after a CTA barrier.  HALF (two samples per warp) always has wps = 1.
@@ -253,9 +303,13 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const float x0X = x0g[0], x0Y = x0g[1];
   if constexpr (kUsesCircles) {
-    for (int i = threadIdx.x; i < p.n_circles; i += blockDim.x) {
-      const float4 c = p.circles[i];
-      circ_s[i] = make_float4(c.x - x0X, c.y - x0Y, c.z, c.z * c.z);
+    for (int i = threadIdx.x; i < n_circ_s; i += blockDim.x) {
+      float4 c = make_float4(0.0f, 0.0f, 0.0f, 0.0f);   // padding: R^2 = 0 is never near
+      if (i < p.n_circles) {
+        c = p.circles[i];
+        c = make_float4(c.x - x0X, c.y - x0Y, c.z, c.z * c.z);
+      }
+      circ_s[i] = c;
     }
   }
   MapFrame mf{};
@@ -301,7 +355,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
     RA_T_LOOP_UNROLL
     for (int t = 0; t < p.T; ++t) {
       const float4 ce = ce_s[t];
-      risk_accumulate<RISK, RC, NX>(p, circ_s, mf, x0X, x0Y, x, L);            // l(x~_t), pre-step
+      risk_accumulate<RISK, RC, NX>(p, circ_s, n_circ_s, lane, mf, x0X, x0Y, x, L);            // l(x~_t), pre-step
 #pragma unroll
       for (int r = 0; r < RC; ++r) {
         float z[NX];
@@ -322,6 +376,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
 #pragma unroll
     for (int r = 0; r < RC; ++r) {
       const bool valid = (chunk + r) < p.R_total && (int)m[r] < p.M;
+      if constexpr (RISK == RISK_CIRCLES) L[r] *= p.risk_p[0];   // risk_accumulate sums unweighted penetrations
       if (chunk + r < p.R_total) keys[(chunk + r) * 32 + lane] = valid ? float_key(L[r]) : 0u;
       if (valid && k_valid) {
         if (L_out) L_out[(size_t)k * p.M + m[r]] = L[r];
@@ -341,8 +396,8 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
     __syncwarp();
   }
 
-  float Lbar;
-  float cvar = cvar_select<G>(keys, p.R_total, lane, p.k_tail, p.M, mask, &Lbar);
+  float Lbar = 0.0f;
+  float cvar = cvar_select<G>(keys, p.R_total, lane, p.k_tail, p.M, mask, p.B != 1.0f, &Lbar);
   // (18)-(19) PAPER.md:144-148: L_a = B (L - Lbar) + Lbar is affine-monotone for B > 0, so
   // CVaR(L_a) = B (CVaR(L) - Lbar) + Lbar.
   if (p.B != 1.0f) cvar = fmaf(p.B, cvar - Lbar, Lbar);

@@ -18,7 +18,7 @@ cudaError_t launch(const Params& p, const float* d_x0, float* d_L, float* d_xT, 
   const int samples_per_cta = HALF ? 2 * kRolloutWarps : kRolloutWarps / p.wps;
   const int grid = (p.K + samples_per_cta - 1) / samples_per_cta;
   const int ce_slots = HALF ? 2 * kRolloutWarps : kRolloutWarps / p.wps;
-  const size_t smem = ((RA_INST_RISK == RISK_CIRCLES || RA_INST_RISK == RISK_NOMINAL) ? (size_t)p.n_circles * sizeof(float4) : 0) +
+  const size_t smem = ((RA_INST_RISK == RISK_CIRCLES || RA_INST_RISK == RISK_NOMINAL) ? (size_t)((p.n_circles + 31) & ~31) * sizeof(float4) : 0) +
                       (size_t)ce_slots * p.T * sizeof(float4) + (size_t)kRolloutWarps * p.R_total * 32 * sizeof(uint32_t);
   auto kernel = noisy_rollout_kernel<RA_INST_DYN, RA_INST_RISK, NOISE, RC, HALF>;
   if (smem > 48 * 1024) {   // worst case (1024 circles, T = 128, M = 512) is 65 KB

@@ -144,7 +144,8 @@ def test_paper_sized_workload_M300(torch_cuda):
 def test_parameters_eta_B_Cu_A(torch_cuda):
     base = _with_v(W.small(W.config1(), K=96, M=64, T=20))
     for kw in (dict(eta=0.25), dict(B=3.0), dict(C_u=50.0, A=10.0), dict(A=0.0), dict(gamma=0.0),
-               dict(alpha=0.5), dict(alpha=0.99), dict(lam=100.0)):
+               dict(alpha=0.5), dict(alpha=0.99), dict(lam=100.0),
+               dict(alpha=0.3)):   # k_tail = 45: the radix selector with two slots per lane
         p = base.replace(**kw)
         ctl, orc = _ctl(p), O.Oracle(p)
         g, r = check_rollout_parity(p, ctl, orc)
