@@ -292,6 +292,87 @@ def run_cuda(args):
         dist.destroy_process_group()
 
 
+def run_sharded(args):
+    """--sharded: ONE controller whose K samples are split over the N ranks (strong scaling).
+    Every step = local rollouts + partial reduction, one NCCL all-gather of 2+2T doubles per rank, combine."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_2209_12842_b200.sharded import ShardedRaMppi
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    p = make_problem(args.workload, 0)              # the same problem on every rank; each takes its K-shard
+    sc = ShardedRaMppi(p, device=local)
+    dev = sc.ctl.device
+    d_x0, v_init = sc.ctl.tensor(p.x0), sc.ctl.tensor(p.v)
+    d_v = v_init.clone()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for i in range(args.warmup):
+        d_v.copy_(v_init)
+        sc.step(d_x0, d_v, i)
+    sampler = ClockSampler(local)
+    sampler.start()
+    starts = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    stops = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    barrier()
+    for i in range(args.steps):
+        d_v.copy_(v_init)
+        flush.zero_()
+        starts[i].record(stream)
+        sc.step(d_x0, d_v, args.warmup + i)
+        stops[i].record(stream)
+    barrier()
+    sampler.stop_flag = True
+    sampler.join()
+    total_ms = float(sum(s.elapsed_time(e) for s, e in zip(starts, stops)))
+    # end to end: pinned host x0, v -> device, sharded step, v+ -> host, every step
+    h_x0 = torch.tensor(np.asarray(p.x0, dtype=np.float32)).pin_memory()
+    h_v0 = torch.tensor(np.asarray(p.v, dtype=np.float32)).pin_memory()
+    h_v = h_v0.clone().pin_memory()
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        d_x0.copy_(h_x0, non_blocking=True)
+        d_v.copy_(h_v0, non_blocking=True)
+        sc.step(d_x0, d_v, args.warmup + i)
+        h_v.copy_(d_v, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    total_ms, e2e_ms = max_over_ranks([total_ms, e2e_ms], world, dev)
+    if rank == 0:
+        units = p.state_steps                       # the whole problem, once: strong scaling
+        print(json.dumps({
+            "metric": METRIC, "value": units * args.steps / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{p.name} K={p.K} M={p.M} T={p.T}", "l2_flush_between_steps": True,
+                       "parallelism": f"K-sharded over {world} GPU(s): {sc.ctl.K} samples on rank 0, "
+                                      f"one all-gather of {8 * (2 + 2 * p.T)} B per rank per step"},
+            "iterations_per_s": args.steps / (total_ms * 1e-3), "clocks": sampler.summary(),
+            "e2e": {"value": units * args.steps / (e2e_ms * 1e-3), "unit": UNIT,
+                    "h2d_bytes_per_step": int(4 * (p.nx + 2 * p.T)), "d2h_bytes_per_step": int(4 * 2 * p.T),
+                    "ms_per_step": e2e_ms / args.steps, "api": "ShardedRaMppi.step (pinned host x0, v -> v+)"},
+            "gpu_launches": int((sc.ctl.launches_per_step + 1) * args.steps),
+        }))
+    sc.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def quick_time(p, steps=50, warmup=5):
     """Device-timed ra_mppi_step on problem p (events per step, L2 flushed between); small helper of --report."""
     import torch
@@ -383,12 +464,16 @@ def main():
     ap.add_argument("--workload", default="C3")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sharded", action="store_true",
+                    help="one controller, K split over the ranks (strong scaling) instead of N independent replicas")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
     if args.report:
         run_report(args)
     elif args.impl == "reference":
         run_reference(args)
+    elif args.sharded:
+        run_sharded(args)
     else:
         run_cuda(args)
 

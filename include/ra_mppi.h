@@ -77,6 +77,12 @@ typedef struct {
   int32_t noise_mode;   /* ra_noise_mode: fused = Philox in registers; materialised = w[K,T,M,nx] in HBM */
   uint64_t seed;        /* Philox4x32-10 key                                                  */
   int32_t device;       /* CUDA device ordinal                                                */
+  /* K-sharding over several contexts / GPUs (not in the paper): this context
+   * holds the K samples with global indices k_offset .. k_offset+K-1 of K_total.  Philox counters and
+   * the eta split (Alg.1 l.7) use the global index, so results do not depend on the partition.
+   * K_total = 0 means "not sharded" (K_total = K, k_offset must be 0).                             */
+  int32_t k_offset;
+  int32_t K_total;
 } ra_mppi_config;
 
 /* Environment; HOST pointers, copied at create (caller keeps ownership). */
@@ -106,6 +112,17 @@ ra_status ra_mppi_step(ra_mppi_ctx* ctx, const float* d_x0, float* d_v, uint64_t
 ra_status ra_mppi_rollout_costs(ra_mppi_ctx* ctx, const float* d_x0, const float* d_v,
                                 uint64_t iteration, float* d_S, float* d_cvar, float* d_S_tilde,
                                 float* d_L, float* d_xT, float* d_u, void* cuda_stream);
+
+/* K-sharded iteration, local part: Alg.1 l.3-29 on this context's samples, then the shard's share of
+ * (17)/(4): d_partial [2+2T] fp64 (device) = { beta_g = min_k S~_k, Z_g = sum_k exp(-(S~_k-beta_g)/lambda),
+ * N_g[T][2] = sum_k exp(-(S~_k-beta_g)/lambda) u^k_t } over the local k.  d_v is read only.           */
+ra_status ra_mppi_step_partial(ra_mppi_ctx* ctx, const float* d_x0, const float* d_v, uint64_t iteration,
+                               double* d_partial, void* cuda_stream);
+/* K-sharded iteration, exchange step: d_partials [n_parts][2+2T] fp64 (device; the shards' partials,
+ * e.g. after an NCCL all-gather, any order) -> d_v_plus [T,2] = clamp(sum_g s_g N_g / sum_g s_g Z_g),
+ * s_g = exp(-(beta_g - min_g beta_g)/lambda): exactly (17)/(4) over the union of the shards.        */
+ra_status ra_mppi_combine_partials(ra_mppi_ctx* ctx, const double* d_partials, int32_t n_parts,
+                                   float* d_v_plus, void* cuda_stream);
 
 /* The fp64 cost scratch of the most recent step / rollout_costs on this context: d_S64 [K],
  * d_S_tilde64 [K] (device, fp64, either may be NULL).  The weights (17) are formed from these

@@ -264,3 +264,27 @@ def shift(v_plus):
 
 def host_cores():
     return os.cpu_count() or 1
+
+
+# ---- K-sharded update (not in the paper): (17) PAPER.md:134 and (4) :51 written per shard.
+# Factor exp(-(beta_g - beta)/lambda) out of every weight of shard g: sum_k w_k u_k = sum_g s_g N_g, Z = sum_g s_g Z_g.
+def shard_partial(S_tilde, u, lam):
+    """{beta_g, Z_g, N_g[T,2]} (flat [2+2T]) of the samples of one shard: S_tilde [K_g], u [K_g,T,2]."""
+    S_tilde = np.asarray(S_tilde, dtype=np.float64)
+    u = np.asarray(u, dtype=np.float64)
+    beta = S_tilde.min()
+    w = np.exp(-(S_tilde - beta) / lam)
+    N = np.zeros(u.shape[1:])
+    for k in range(u.shape[0]):
+        N += w[k] * u[k]
+    return np.concatenate([[beta, w.sum()], N.ravel()])
+
+
+def combine_partials(parts, lam, u_min, u_max):
+    """v+ [T,2] from the shards' partials [G, 2+2T] (any order)."""
+    parts = np.asarray(parts, dtype=np.float64)
+    beta = parts[:, 0].min()
+    s = np.exp(-(parts[:, 0] - beta) / lam)
+    Z = float((s * parts[:, 1]).sum())
+    N = (s[:, None] * parts[:, 2:]).sum(axis=0).reshape(-1, 2)
+    return np.clip(N / Z, np.asarray(u_min, dtype=np.float64), np.asarray(u_max, dtype=np.float64))

@@ -40,6 +40,7 @@ class ra_mppi_config(C.Structure):
         ("noise_mode", C.c_int32),
         ("seed", C.c_uint64),
         ("device", C.c_int32),
+        ("k_offset", C.c_int32), ("K_total", C.c_int32),
     ]
 
 
@@ -53,6 +54,7 @@ class ra_mppi_env(C.Structure):
 
 EXPORTS = (
     "ra_mppi_create", "ra_mppi_step", "ra_mppi_rollout_costs", "ra_mppi_weights_update",
+    "ra_mppi_step_partial", "ra_mppi_combine_partials",
     "ra_mppi_step_host", "ra_mppi_enable_kernel_timing", "ra_mppi_last_rollout_ms",
     "ra_mppi_export_costs_f64", "ra_mppi_plant_shift", "ra_mppi_closed_loop", "ra_mppi_philox", "ra_mppi_state_noise",
     "ra_mppi_measure_pipe_peaks", "ra_mppi_launches_per_step", "ra_mppi_last_error", "ra_mppi_destroy",
@@ -75,6 +77,8 @@ def load():
     L.ra_mppi_create.argtypes = [C.POINTER(ra_mppi_config), C.POINTER(ra_mppi_env), C.POINTER(vp)]
     L.ra_mppi_step.argtypes = [vp, fp, fp, u64, vp]
     L.ra_mppi_rollout_costs.argtypes = [vp, fp, fp, u64, fp, fp, fp, fp, fp, fp, vp]
+    L.ra_mppi_step_partial.argtypes = [vp, fp, fp, u64, vp, vp]
+    L.ra_mppi_combine_partials.argtypes = [vp, vp, i32, fp, vp]
     L.ra_mppi_weights_update.argtypes = [vp, fp, fp, fp, fp, fp, vp]
     L.ra_mppi_export_costs_f64.argtypes = [vp, vp, vp, vp]
     L.ra_mppi_step_host.argtypes = [vp, vp, vp, u64, vp]
@@ -119,6 +123,8 @@ def make_config(p, device=0) -> ra_mppi_config:
     c.noise_mode = int(getattr(p, "noise_mode", 0))
     c.seed = int(p.seed)
     c.device = int(device)
+    c.k_offset = int(getattr(p, "k_offset", 0))
+    c.K_total = int(getattr(p, "K_total", 0))
     return c
 
 
@@ -164,6 +170,15 @@ def ra_mppi_rollout_costs(ctx, d_x0, d_v, iteration, d_S=None, d_cvar=None, d_S_
                           d_xT=None, d_u=None, stream=0):
     _check(ctx, load().ra_mppi_rollout_costs(ctx, d_x0, d_v, int(iteration), d_S, d_cvar, d_S_tilde, d_L,
                                              d_xT, d_u, stream), "ra_mppi_rollout_costs")
+
+
+def ra_mppi_step_partial(ctx, d_x0, d_v, iteration, d_partial, stream=0):
+    _check(ctx, load().ra_mppi_step_partial(ctx, d_x0, d_v, int(iteration), d_partial, stream), "ra_mppi_step_partial")
+
+
+def ra_mppi_combine_partials(ctx, d_partials, n_parts, d_v_plus, stream=0):
+    _check(ctx, load().ra_mppi_combine_partials(ctx, d_partials, int(n_parts), d_v_plus, stream),
+           "ra_mppi_combine_partials")
 
 
 def ra_mppi_weights_update(ctx, d_S_tilde, d_u, d_v_plus, d_w=None, d_stats=None, stream=0):

@@ -59,6 +59,24 @@ class RaMppi:
                                 ptr(out["u"]), self._stream())
         return out
 
+    def step_partial(self, d_x0, d_v, iteration: int = 0, out: torch.Tensor = None):
+        """ra_mppi_step_partial: this context's share {beta_g, Z_g, N_g[T,2]} of (17)/(4) as fp64 [2+2T]."""
+        if out is None:
+            out = torch.empty(2 + 2 * self.T, device=self.device, dtype=torch.float64)
+        assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == 2 + 2 * self.T
+        B.ra_mppi_step_partial(self.ctx, d_x0.data_ptr(), d_v.data_ptr(), iteration, out.data_ptr(), self._stream())
+        return out
+
+    def combine_partials(self, d_partials: torch.Tensor, d_v_out: torch.Tensor = None):
+        """ra_mppi_combine_partials: [n, 2+2T] fp64 partials of all shards -> v+ [T,2]."""
+        assert d_partials.is_cuda and d_partials.dtype == torch.float64 and d_partials.is_contiguous()
+        assert d_partials.dim() == 2 and d_partials.shape[1] == 2 + 2 * self.T
+        if d_v_out is None:
+            d_v_out = torch.empty(self.T, 2, device=self.device, dtype=torch.float32)
+        B.ra_mppi_combine_partials(self.ctx, d_partials.data_ptr(), d_partials.shape[0], d_v_out.data_ptr(),
+                                   self._stream())
+        return d_v_out
+
     def step_host(self, h_x0: torch.Tensor, h_v: torch.Tensor, iteration: int = 0):
         """ra_mppi_step_host: h_x0 [nx], h_v [T,2] are HOST tensors (pinned for async copies); h_v <- v+."""
         assert not h_x0.is_cuda and not h_v.is_cuda and h_v.is_contiguous() and h_v.dtype == torch.float32

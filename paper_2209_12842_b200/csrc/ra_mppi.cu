@@ -76,6 +76,9 @@ const char* validate(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_statu
   *st = RA_EINVAL;
   if (cfg->struct_size != sizeof(ra_mppi_config)) return "struct_size mismatch";
   if (cfg->K <= 0 || cfg->M <= 0 || cfg->T <= 0) return "K, M, T must be positive";
+  if (cfg->K_total == 0 && cfg->k_offset != 0) return "k_offset needs K_total";
+  if (cfg->K_total != 0 && (cfg->k_offset < 0 || cfg->K_total < cfg->K || cfg->k_offset > cfg->K_total - cfg->K))
+    return "shard [k_offset, k_offset + K) must lie inside [0, K_total)";
   if (!(cfg->dt > 0.0f) || !std::isfinite(cfg->dt)) return "dt must be positive";
   if (cfg->dyn != RA_DYN_KINEMATIC_BICYCLE && cfg->dyn != RA_DYN_SINGLE_TRACK) return "unknown dyn";
   if (cfg->nominal < RA_NOM_GOAL || cfg->nominal > RA_NOM_RACING) return "unknown nominal cost";
@@ -175,7 +178,9 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
 
   Params& p = c->p;
   p.K = cfg->K; p.M = cfg->M; p.T = cfg->T;
-  p.K0 = (int)std::ceil((1.0 - (double)cfg->eta) * (double)cfg->K - 1e-9);
+  const int K_total = cfg->K_total ? cfg->K_total : cfg->K;
+  p.k_off = cfg->k_offset;
+  p.K0 = (int)std::ceil((1.0 - (double)cfg->eta) * (double)K_total - 1e-9);   // on the global index
   p.k_tail = tail_count((double)cfg->alpha, cfg->M);
   c->half = cfg->M <= 16;
   p.G = c->half ? 16 : 32;
@@ -356,7 +361,15 @@ ra_status enqueue_costs(ra_mppi_ctx* c, const Params& p, const float* d_x0, cons
 // Alg.1 l.31: weights (17) and update (4) from the context scratch.
 ra_status enqueue_update(ra_mppi_ctx* c, const Params& p, float* d_v_out, cudaStream_t s) {
   weights_update_kernel<double><<<p.T, kUpdateThreads, 0, s>>>(
-      p, p.S_tilde, p.u_raw, 1LL, (long long)p.K, d_v_out, nullptr, nullptr);
+      p, p.S_tilde, p.u_raw, 1LL, (long long)p.K, d_v_out, nullptr, nullptr, nullptr);
+  RA_CUDA(c, cudaGetLastError());
+  return RA_OK;
+}
+
+// The shard's share of (17)/(4) for the K-sharded step.
+ra_status enqueue_partial(ra_mppi_ctx* c, const Params& p, double* d_partial, cudaStream_t s) {
+  weights_update_kernel<double><<<p.T, kUpdateThreads, 0, s>>>(
+      p, p.S_tilde, p.u_raw, 1LL, (long long)p.K, nullptr, nullptr, nullptr, d_partial);
   RA_CUDA(c, cudaGetLastError());
   return RA_OK;
 }
@@ -391,6 +404,25 @@ ra_status ra_mppi_step(ra_mppi_ctx* c, const float* d_x0, float* d_v, uint64_t i
   return enqueue_update(c, p, d_v, s);
 }
 
+ra_status ra_mppi_step_partial(ra_mppi_ctx* c, const float* d_x0, const float* d_v, uint64_t iteration,
+                               double* d_partial, void* stream) {
+  if (!c) return RA_EINVAL;
+  if (!d_x0 || !d_v || !d_partial) return fail(c, RA_EINVAL, "null device pointer");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const Params p = with_iteration(c, iteration);
+  if (ra_status st = enqueue_costs(c, p, d_x0, d_v, nullptr, nullptr, s, false)) return st;
+  return enqueue_partial(c, p, d_partial, s);
+}
+
+ra_status ra_mppi_combine_partials(ra_mppi_ctx* c, const double* d_partials, int32_t n_parts, float* d_v_plus,
+                                   void* stream) {
+  if (!c) return RA_EINVAL;
+  if (!d_partials || !d_v_plus || n_parts < 1) return fail(c, RA_EINVAL, "bad arguments");
+  combine_partials_kernel<<<1, 256, 0, static_cast<cudaStream_t>(stream)>>>(c->p, d_partials, n_parts, d_v_plus);
+  RA_CUDA(c, cudaGetLastError());
+  return RA_OK;
+}
+
 ra_status ra_mppi_rollout_costs(ra_mppi_ctx* c, const float* d_x0, const float* d_v, uint64_t iteration,
                                 float* d_S, float* d_cvar, float* d_S_tilde, float* d_L, float* d_xT,
                                 float* d_u, void* stream) {
@@ -417,7 +449,7 @@ ra_status ra_mppi_weights_update(ra_mppi_ctx* c, const float* d_S_tilde, const f
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const Params p = with_iteration(c, 0);
   weights_update_kernel<float><<<p.T, kUpdateThreads, 0, s>>>(
-      p, d_S_tilde, reinterpret_cast<const float2*>(d_u), (long long)p.T, 1LL, d_v_plus, d_w, d_stats);
+      p, d_S_tilde, reinterpret_cast<const float2*>(d_u), (long long)p.T, 1LL, d_v_plus, d_w, d_stats, nullptr);
   RA_CUDA(c, cudaGetLastError());
   return RA_OK;
 }

@@ -15,7 +15,8 @@ constexpr int kMaxCirclesSmem = 1024;  // obstacle records staged per CTA (16 B 
 
 struct Params {
   int K, M, T;
-  int K0;       // samples k < K0 use u = v + eps, the rest u = eps   (Alg.1 l.7-10)
+  int K0;       // samples with GLOBAL index < K0 use u = v + eps, the rest u = eps   (Alg.1 l.7-10)
+  int k_off;    // global index of local sample 0 (K-sharding; 0 when not sharded)
   int k_tail;   // ceil((1-alpha) M)                                  (Alg.1 l.25)
   int G;        // lanes per control sample: 32, or 16 when M <= 16
   int R_total;  // realisation slots of G lanes per sample = ceil(M / G)

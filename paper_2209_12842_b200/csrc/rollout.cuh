@@ -51,10 +51,10 @@ __global__ void __launch_bounds__(kSampleThreads) sample_nominal_kernel(const __
   for (int idx = threadIdx.x; idx < p.T * kSampleKB; idx += blockDim.x) {
     const int t = idx / kSampleKB, kl = idx % kSampleKB, k = k0 + kl;
     if (k >= p.K) continue;
-    const uint4 r = philox4x32_10((uint32_t)k, 0u, (uint32_t)t, c3, p.rk);
+    const uint4 r = philox4x32_10((uint32_t)(k + p.k_off), 0u, (uint32_t)t, c3, p.rk);
     float z0, z1;
     box_muller(r.x, r.y, z0, z1);
-    const bool with_mean = k < p.K0;
+    const bool with_mean = k + p.k_off < p.K0;
     const float v0 = v_s[2 * t], v1 = v_s[2 * t + 1];
     const float u0 = fmaf(p.sigma_eps[0], z0, with_mean ? v0 : 0.0f);
     const float u1 = fmaf(p.sigma_eps[1], z1, with_mean ? v1 : 0.0f);
@@ -341,6 +341,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
   if constexpr (DYN == DYN_SINGLE_TRACK) x_init[3] = fmaxf(x_init[3], p.dyn_p[6]);
 
   const uint32_t c3 = iteration_field(p, STREAM_W);
+  const uint32_t kg = (uint32_t)(k + p.k_off);   // global sample index in the Philox counter
 
   for (int chunk = ws * RC; chunk < p.R_total; chunk += wps * RC) {
     float x[RC][NX], L[RC];
@@ -364,7 +365,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
 #pragma unroll
           for (int i = 0; i < NX; ++i) z[i] = __ldg(wp + (size_t)i * p.M_pad);
         } else {
-          state_noise<NX, NOISE>(p, (uint32_t)k, m[r], (uint32_t)t, c3, z);
+          state_noise<NX, NOISE>(p, kg, m[r], (uint32_t)t, c3, z);
         }
         dynamics_step<DYN, true>(p, x[r], ce);   // x~_{t+1} = F(x~_t, u_t) + w_t   (6) PAPER.md:63
 #pragma unroll

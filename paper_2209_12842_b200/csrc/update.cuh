@@ -35,7 +35,7 @@ __global__ void __launch_bounds__(kUpdateThreads)
 weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S_tilde,
                       const float2* __restrict__ u, long long su_k, long long su_t,
                       float* __restrict__ v_out, float* __restrict__ w_out,
-                      float* __restrict__ stats) {
+                      float* __restrict__ stats, double* __restrict__ partial) {
   __shared__ ST red_s[32];
   __shared__ float red_f[96];
   const int t = blockIdx.x;
@@ -72,6 +72,14 @@ weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S
       n1 += __shfl_xor_sync(0xFFFFFFFFu, n1, o);
     }
   }
+  if (partial) {   // K-sharded step: the shard's unnormalised share {beta_g, Z_g, N_g[T][2]}
+    if (threadIdx.x == 0) {
+      if (t == 0) { partial[0] = (double)beta; partial[1] = (double)Z; }
+      partial[2 + 2 * t] = (double)n0;
+      partial[3 + 2 * t] = (double)n1;
+    }
+    return;
+  }
   if (threadIdx.x == 0) {
     v_out[2 * t] = clampf(n0 / Z, p.u_min[0], p.u_max[0]);
     v_out[2 * t + 1] = clampf(n1 / Z, p.u_min[1], p.u_max[1]);
@@ -81,6 +89,27 @@ weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S
     const float invZ = 1.0f / Z;
     for (int k = threadIdx.x; k < p.K; k += blockDim.x)
       w_out[k] = exp2f((float)(S_tilde[k] - beta) * p.neg_log2e_over_lambda) * invZ;
+  }
+}
+
+// Exchange step of the K-sharded iteration: partials [n][2+2T] = {beta_g, Z_g, N_g[T][2]} of the shards
+// -> v+ = clamp(sum_g s_g N_g / sum_g s_g Z_g), s_g = exp(-(beta_g - beta)/lambda), beta = min_g beta_g,
+// which is (17)/(4) over the union of the shards (factor exp(-(beta_g-beta)/lambda) out of every w~_k).
+// Fixed summation order over g => every rank computes bitwise the same v+.  One CTA, thread = (t, i).
+__global__ void combine_partials_kernel(const __grid_constant__ Params p, const double* __restrict__ partials,
+                                        int n_parts, float* __restrict__ v_out) {
+  const int stride = 2 + 2 * p.T;
+  double beta = INFINITY;
+  for (int g = 0; g < n_parts; ++g) beta = fmin(beta, partials[(size_t)g * stride]);
+  for (int j = threadIdx.x; j < 2 * p.T; j += blockDim.x) {
+    float Z = 0.0f, n = 0.0f;
+    for (int g = 0; g < n_parts; ++g) {
+      const double* pg = partials + (size_t)g * stride;
+      const float s = exp2f((float)(pg[0] - beta) * p.neg_log2e_over_lambda);
+      Z = fmaf(s, (float)pg[1], Z);
+      n = fmaf(s, (float)pg[2 + j], n);
+    }
+    v_out[j] = clampf(n / Z, p.u_min[j & 1], p.u_max[j & 1]);
   }
 }
 
@@ -189,7 +218,7 @@ __global__ void __launch_bounds__(256) materialise_noise_kernel(const __grid_con
     const long long kt = i / p.M_pad;
     const int t = (int)(kt % p.T), k = (int)(kt / p.T);
     float z[NX];
-    state_noise<NX, NOISE>(p, (uint32_t)k, (uint32_t)m, (uint32_t)t, c3, z);
+    state_noise<NX, NOISE>(p, (uint32_t)(k + p.k_off), (uint32_t)m, (uint32_t)t, c3, z);
     float* o = w + (size_t)kt * NX * p.M_pad + m;
 #pragma unroll
     for (int j = 0; j < NX; ++j) o[(size_t)j * p.M_pad] = z[j] * p.wscale[j];

@@ -69,6 +69,8 @@ class Problem:
     map_res: float = 0.0
     map_ox: float = 0.0
     map_oy: float = 0.0
+    k_offset: int = 0   # K-sharding: global index of this shard's first sample
+    K_total: int = 0    # K-sharding: samples over all shards (0 = not sharded)
 
     @property
     def nx(self) -> int:

@@ -29,6 +29,12 @@ def test_gloo_two_ranks_max_and_aggregate():
     assert abs(float(rate[0].split()[1]) - 2 * 256 * 16 * 20 * 4 / 11e-3) < 1e-3
 
 
+def test_gloo_two_ranks_k_sharded_step_host_logic():
+    r = _torchrun([os.path.join("tests", "helpers", "gloo_sharded.py")])
+    assert r.returncode == 0, r.stderr[-2000:]
+    assert any(l.startswith("SHARDED_OK") for l in r.stdout.splitlines())
+
+
 def test_reference_arm_under_torchrun_prints_one_line():
     r = _torchrun(["bench.py", "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "0",
                    "--workload", "C0"])
