@@ -464,11 +464,17 @@ def main():
     ap.add_argument("--workload", default="C3")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--pipe-model", action="store_true",
+                    help="print the measured issue-cost model of the SM pipes (one JSON line) and exit")
     ap.add_argument("--sharded", action="store_true",
                     help="one controller, K split over the ranks (strong scaling) instead of N independent replicas")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
-    if args.report:
+    if args.pipe_model:
+        from paper_2209_12842_b200 import binding as B
+        print(json.dumps({"report": "pipe model, cycles per warp-instruction group per SMSP at max SM clock",
+                          **B.ra_mppi_measure_pipe_model(0), "peaks_Tlaneops": B.ra_mppi_measure_pipe_peaks(0)}))
+    elif args.report:
         run_report(args)
     elif args.impl == "reference":
         run_reference(args)

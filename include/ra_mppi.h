@@ -175,6 +175,13 @@ ra_status ra_mppi_state_noise(ra_mppi_ctx* ctx, const int32_t* d_kmt, int32_t n,
  * microbenchmark kernels on the NULL stream and synchronises.  Roofline denominators only.   */
 ra_status ra_mppi_measure_pipe_peaks(int32_t device, float* h_tera_lane_ops);
 
+/* The issue-cost model behind the roofline discussion: h_cycles[8] (HOST) = cycles per
+ * warp-instruction (group) per SM sub-partition at the device's maximum SM clock, 24 warps/SM, for
+ * {FFMA r,c,c; FFMA r,r,r; FMUL r,r; IMAD 32-bit; SHF; IMAD.WIDE.U32 + LOP3 (one Philox half-round);
+ *  the same + 2 FFMA; the same + 4 FFMA}.  The last three show that FFMAs do not overlap the wide multiply.
+ * Runs eight short microbenchmark kernels on the NULL stream and synchronises.                           */
+ra_status ra_mppi_measure_pipe_model(int32_t device, float* h_cycles);
+
 /* Number of kernels one ra_mppi_step launches (for launch accounting).                   */
 int32_t ra_mppi_launches_per_step(const ra_mppi_ctx* ctx);
 /* Last error text, owned by the context (valid until the next call on it).               */

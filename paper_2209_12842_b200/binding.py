@@ -57,7 +57,7 @@ EXPORTS = (
     "ra_mppi_step_partial", "ra_mppi_combine_partials",
     "ra_mppi_step_host", "ra_mppi_enable_kernel_timing", "ra_mppi_last_rollout_ms",
     "ra_mppi_export_costs_f64", "ra_mppi_plant_shift", "ra_mppi_closed_loop", "ra_mppi_philox", "ra_mppi_state_noise",
-    "ra_mppi_measure_pipe_peaks", "ra_mppi_launches_per_step", "ra_mppi_last_error", "ra_mppi_destroy",
+    "ra_mppi_measure_pipe_peaks", "ra_mppi_measure_pipe_model", "ra_mppi_launches_per_step", "ra_mppi_last_error", "ra_mppi_destroy",
 )
 
 _lib = None
@@ -89,6 +89,7 @@ def load():
     L.ra_mppi_philox.argtypes = [vp, vp, i32, vp, vp]
     L.ra_mppi_state_noise.argtypes = [vp, vp, i32, u64, fp, vp]
     L.ra_mppi_measure_pipe_peaks.argtypes = [i32, C.POINTER(C.c_float)]
+    L.ra_mppi_measure_pipe_model.argtypes = [i32, C.POINTER(C.c_float)]
     L.ra_mppi_launches_per_step.argtypes = [vp]
     L.ra_mppi_launches_per_step.restype = i32
     L.ra_mppi_last_error.argtypes = [vp]
@@ -230,6 +231,15 @@ def ra_mppi_measure_pipe_peaks(device=0):
     out = (C.c_float * 4)()
     _check(None, load().ra_mppi_measure_pipe_peaks(int(device), out), "ra_mppi_measure_pipe_peaks")
     return dict(zip(("ffma", "imad_wide", "lop3", "mufu"), (float(x) for x in out)))
+
+
+def ra_mppi_measure_pipe_model(device=0):
+    """{instruction group: cycles per warp-instruction group per SMSP} (see include/ra_mppi.h)."""
+    out = (C.c_float * 8)()
+    _check(None, load().ra_mppi_measure_pipe_model(int(device), out), "ra_mppi_measure_pipe_model")
+    names = ("ffma_rcc", "ffma_rrr", "fmul_rr", "imad", "shf", "imad_wide+lop3", "imad_wide+lop3+2ffma",
+             "imad_wide+lop3+4ffma")
+    return dict(zip(names, (float(x) for x in out)))
 
 
 def ra_mppi_launches_per_step(ctx):
