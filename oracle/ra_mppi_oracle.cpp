@@ -43,11 +43,12 @@ inline void philox_round(uint32_t c[4], const uint32_t k[2]) {
 
 inline double clampd(double x, double lo, double hi) { return x < lo ? lo : (x > hi ? hi : x); }
 
-/* Number of Philox calls per state step.  D:RNG layout. */
-inline uint32_t calls_per_step(const orc_problem* p) {
+/* Number of 32-bit words one state step takes from the (k, m, stream, iteration) word stream: one per state
+ * component, plus (jump noise) one for the trigger and one unused so that Box-Muller pairs stay aligned.
+ * D:RNG layout. */
+inline uint32_t words_per_step(const orc_problem* p) {
   const uint32_t nx = (uint32_t)orc_nx(p->dyn);
-  const uint32_t J = (nx + 3u) / 4u;
-  return p->noise_kind == ORC_NOISE_JUMP ? J + 1u : J;
+  return p->noise_kind == ORC_NOISE_JUMP ? nx + 2u : nx;
 }
 
 }  // namespace
@@ -64,7 +65,8 @@ void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
   out[0] = c[0]; out[1] = c[1]; out[2] = c[2]; out[3] = c[3];
 }
 
-/* D:RNG layout.  ctr = (k, m, t*J + j, stream<<28 | iteration&0x0FFFFFFF). */
+/* D:RNG layout.  ctr = (k, m, t*J + j, stream<<28 | iteration&0x0FFFFFFF); the EPS stream uses J = 1, j = 0, and
+ * the state-noise word stream passes its call index as t. */
 void orc_counter(uint32_t k, uint32_t m, uint32_t t, uint32_t J, uint32_t j,
                  uint32_t stream, uint64_t iteration, uint32_t ctr[4]) {
   ctr[0] = k;
@@ -93,15 +95,20 @@ int orc_nx(int32_t dyn) { return dyn == ORC_DYN_SINGLE_TRACK ? 6 : 4; }
 void orc_state_noise(const orc_problem* p, uint32_t k, uint32_t m, uint32_t t,
                      uint32_t stream, uint64_t iteration, double w[6]) {
   const uint32_t nx = (uint32_t)orc_nx(p->dyn);
-  const uint32_t J = (nx + 3u) / 4u;
-  const uint32_t Jc = calls_per_step(p);
+  const uint32_t Wd = words_per_step(p);
   const uint32_t key[2] = {(uint32_t)(p->seed & 0xFFFFFFFFull), (uint32_t)(p->seed >> 32)};
-  uint32_t r[8];
-  for (uint32_t j = 0; j < J; ++j) {
+  /* D:RNG layout: the realisation (k, m) of a stream owns the word stream
+   *   word n = output (n mod 4) of Philox4x32-10 at counter (k, m, n div 4, stream<<28 | iteration),
+   * and step t takes the words Wd*t .. Wd*t + Wd - 1 in component order. */
+  const uint32_t n0 = Wd * t, c_first = n0 / 4u, c_last = (n0 + Wd - 1u) / 4u;   /* at most 3 calls */
+  uint32_t call[3][4];
+  for (uint32_t c = c_first; c <= c_last; ++c) {
     uint32_t ctr[4];
-    orc_counter(k, m, t, Jc, j, stream, iteration, ctr);
-    orc_philox4x32_10(ctr, key, r + 4 * j);
+    orc_counter(k, m, c, 1u, 0u, stream, iteration, ctr);
+    orc_philox4x32_10(ctr, key, call[c - c_first]);
   }
+  uint32_t r[8];
+  for (uint32_t i = 0; i < Wd; ++i) r[i] = call[(n0 + i) / 4u - c_first][(n0 + i) % 4u];
   double z[8];
   if (p->noise_kind == ORC_NOISE_UNIFORM) {
     /* (2*(r>>9)+1) 2^-23 - 1 : symmetric on (-1,1), exactly representable */
@@ -111,10 +118,7 @@ void orc_state_noise(const orc_problem* p, uint32_t k, uint32_t m, uint32_t t,
     for (uint32_t i = 0; i < nx; i += 2) orc_box_muller(r[i], r[i + 1], z + i);
   }
   if (p->noise_kind == ORC_NOISE_JUMP) {
-    uint32_t ctr[4], rj[4];
-    orc_counter(k, m, t, Jc, J, stream, iteration, ctr);
-    orc_philox4x32_10(ctr, key, rj);
-    const double uj = (double)(rj[0] >> 9) * (1.0 / 8388608.0);
+    const double uj = (double)(r[nx] >> 9) * (1.0 / 8388608.0);   /* the trigger word follows the components */
     double nrm = 0.0;
     for (uint32_t i = 0; i < nx; ++i) nrm += z[i] * z[i];
     nrm = std::sqrt(nrm);

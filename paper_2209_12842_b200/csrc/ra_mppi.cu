@@ -231,8 +231,6 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
   }
   p.neg_log2e_over_lambda = (float)(-1.4426950408889634 / (double)cfg->lambda);
   p.A = cfg->A; p.B = cfg->B; p.C_u = cfg->C_u;
-  const int J = (p.nx + 3) / 4;
-  p.Jc = cfg->noise_kind == RA_NOISE_JUMP ? J + 1 : J;
   philox_round_keys(cfg->seed, p.rk);
   c->noise_variant = cfg->noise_mode == RA_NOISE_MATERIALISED ? NOISE_MATERIALISED : cfg->noise_kind;
   c->rollout = pick_rollout(cfg->dyn, cfg->risk);

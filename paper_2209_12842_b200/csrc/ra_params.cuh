@@ -35,7 +35,6 @@ struct Params {
   float nom_p[12];
   float risk_p[4];
   float noise_p[4];
-  int Jc;           // Philox calls per state step (counter stride)
   uint32_t rk[20];  // the ten Philox round keys (k0_r, k1_r), key = seed
   // environment (device copies owned by the context)
   const float4* circles;  // [n] absolute (cx, cy, r + margin, unused)

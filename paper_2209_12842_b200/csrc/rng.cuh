@@ -1,6 +1,7 @@
 // Counter-based noise in registers: Philox4x32-10 + Box-Muller on exact 23-bit uniforms.
 // BASELINE.json fixes the generator; the counter layout is DESIGN.md "RNG layout":
-//   ctr = (k, m, t*Jc + j, stream<<28 | iteration&0x0FFFFFFF),  key = (seed lo, seed hi).
+//   ctr = (k, m, call index, stream<<28 | iteration&0x0FFFFFFF),  key = (seed lo, seed hi);
+//   EPS stream: call index = t; state-noise streams: the word stream below.
 // No [K,M,T,n] noise tensor goes to HBM in fused mode.
 #pragma once
 #include <cstdint>
@@ -94,35 +95,49 @@ __device__ __forceinline__ float sym_uniform(uint32_t r) {
   return fmaf(__uint2float_rn(2u * (r >> 9) + 1u), 1.1920928955078125e-07f, -1.0f);
 }
 
-// The n_x per-step state-noise factors a of realisation (k,m) at step t; the additive noise of (6)
-// PAPER.md:63 is w_i = Params::wscale[i] * a[i] (wscale = sigma_w times the constant of the noise
-// kind, built by ra_mppi_create).  NX = 4 -> one Philox call, NX = 6 -> two.  Jump noise makes one more.
-template <int NX, int NOISE>
-__device__ __forceinline__ void state_noise(const Params& p, uint32_t k, uint32_t m, uint32_t t,
-                                            uint32_t c3, float (&z)[NX]) {
-  constexpr int J = (NX + 3) / 4;
-  constexpr int Jc = (NOISE == NOISE_JUMP) ? J + 1 : J;
-  const uint32_t c2 = t * (uint32_t)Jc;
-  const uint4 a = philox4x32_10(k, m, c2, c3, p.rk);
-  if constexpr (NOISE == NOISE_UNIFORM) {
-    z[0] = sym_uniform(a.x); z[1] = sym_uniform(a.y); z[2] = sym_uniform(a.z); z[3] = sym_uniform(a.w);
+// ---- state-noise word stream ------------------------------------------------------
+// Realisation (k, m) of a stream owns the word stream  word n = output (n & 3) of Philox4x32-10 at counter
+// (k, m, n >> 2, stream<<28 | iteration); step t takes the WD words WD*t .. WD*t + WD - 1 in component order,
+// WD = n_x (+ 2 for jump noise: trigger word + one spare so that Box-Muller pairs stay aligned).
+// WD = 4: call t.  WD = 8: calls 2t, 2t+1.  WD = 6: 1.5 calls per step -- the rollout kernel walks the horizon in
+// pairs of steps and carries the spare half of the middle call (three calls per two steps, not four).
+template <int NX, int NOISE> struct NoiseWords { static constexpr int value = NX + (NOISE == NOISE_JUMP ? 2 : 0); };
+
+// The words of step t, on their own (probe, plant, materialised-noise generator, odd last step).
+template <int WD>
+__device__ __forceinline__ void step_words(const Params& p, uint32_t k, uint32_t m, uint32_t t, uint32_t c3,
+                                           uint32_t (&w)[WD]) {
+  static_assert(WD == 4 || WD == 6 || WD == 8, "words per step");
+  if constexpr (WD == 4) {
+    const uint4 a = philox4x32_10(k, m, t, c3, p.rk);
+    w[0] = a.x; w[1] = a.y; w[2] = a.z; w[3] = a.w;
+  } else if constexpr (WD == 8) {
+    const uint4 a = philox4x32_10(k, m, 2u * t, c3, p.rk), b = philox4x32_10(k, m, 2u * t + 1u, c3, p.rk);
+    w[0] = a.x; w[1] = a.y; w[2] = a.z; w[3] = a.w; w[4] = b.x; w[5] = b.y; w[6] = b.z; w[7] = b.w;
   } else {
-    box_muller_fast(a.x, a.y, z[0], z[1]);
-    box_muller_fast(a.z, a.w, z[2], z[3]);
+    const uint32_t c = (3u * t) >> 1;   // (6 t) >> 2
+    const uint4 a = philox4x32_10(k, m, c, c3, p.rk), b = philox4x32_10(k, m, c + 1u, c3, p.rk);
+    const bool odd = (t & 1u) != 0u;    // odd steps start at output 2 of their first call
+    w[0] = odd ? a.z : a.x; w[1] = odd ? a.w : a.y; w[2] = odd ? b.x : a.z; w[3] = odd ? b.y : a.w;
+    w[4] = odd ? b.z : b.x; w[5] = odd ? b.w : b.y;
   }
-  if constexpr (NX == 6) {
-    const uint4 b = philox4x32_10(k, m, c2 + 1u, c3, p.rk);
-    if constexpr (NOISE == NOISE_UNIFORM) {
-      z[4] = sym_uniform(b.x); z[5] = sym_uniform(b.y);
-    } else {
-      box_muller_fast(b.x, b.y, z[4], z[5]);
-    }
+}
+
+// The n_x per-step state-noise factors a from the step's words; the additive noise of (6) PAPER.md:63 is
+// w_i = Params::wscale[i] * a[i] (wscale = sigma_w times the constant of the noise kind, built by
+// ra_mppi_create).
+template <int NX, int NOISE>
+__device__ __forceinline__ void noise_from_words(const Params& p, const uint32_t (&w)[NoiseWords<NX, NOISE>::value],
+                                                 float (&z)[NX]) {
+#pragma unroll
+  for (int i = 0; i < NX; i += 2) {
+    if constexpr (NOISE == NOISE_UNIFORM) { z[i] = sym_uniform(w[i]); z[i + 1] = sym_uniform(w[i + 1]); }
+    else box_muller_fast(w[i], w[i + 1], z[i], z[i + 1]);
   }
   if constexpr (NOISE == NOISE_JUMP) {
     // jump of unit length in a uniformly random direction z/|z| (the common factor of the Gaussian
     // draws cancels; its sign is in wscale), with probability noise_p[0]  (G29)
-    const uint4 jr = philox4x32_10(k, m, c2 + (uint32_t)J, c3, p.rk);
-    const float uj = __uint2float_rn(jr.x >> 9) * 1.1920928955078125e-07f;
+    const float uj = __uint2float_rn(w[NX] >> 9) * 1.1920928955078125e-07f;
     float n2 = 0.0f;
 #pragma unroll
     for (int i = 0; i < NX; ++i) n2 = fmaf(z[i], z[i], n2);
@@ -131,6 +146,14 @@ __device__ __forceinline__ void state_noise(const Params& p, uint32_t k, uint32_
 #pragma unroll
     for (int i = 0; i < NX; ++i) z[i] *= inv;
   }
+}
+
+template <int NX, int NOISE>
+__device__ __forceinline__ void state_noise(const Params& p, uint32_t k, uint32_t m, uint32_t t,
+                                            uint32_t c3, float (&z)[NX]) {
+  uint32_t w[NoiseWords<NX, NOISE>::value];
+  step_words(p, k, m, t, c3, w);
+  noise_from_words<NX, NOISE>(p, w, z);
 }
 
 }  // namespace ra

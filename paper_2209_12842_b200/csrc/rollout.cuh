@@ -276,13 +276,20 @@ __device__ __forceinline__ void risk_accumulate(const Params& p, const float4* c
 // effects, then per warp R_total*32 keys.
 // ---------------------------------------------------------------------------------------
 #ifndef RA_MIN_CTAS_BICYCLE
-#define RA_MIN_CTAS_BICYCLE 3   // measured: 3 CTAs (<= 80 regs) beats 4-6 (throughput-, not latency-bound)
+#define RA_MIN_CTAS_BICYCLE 3   // measured: 3 CTAs (<= 80 regs) beats 2 and 4-6 (throughput-, not latency-bound)
 #endif
 #ifndef RA_MIN_CTAS_SINGLE_TRACK
 #define RA_MIN_CTAS_SINGLE_TRACK 3
 #endif
+#ifndef RA_MIN_CTAS_SINGLE_TRACK_RC4
+#define RA_MIN_CTAS_SINGLE_TRACK_RC4 2   // 4 x 6 state registers + carried Philox words spill at 80 registers
+#endif
+template <int DYN, int RC>
+constexpr int rollout_min_ctas() {
+  return DYN == DYN_BICYCLE ? RA_MIN_CTAS_BICYCLE : (RC == 4 ? RA_MIN_CTAS_SINGLE_TRACK_RC4 : RA_MIN_CTAS_SINGLE_TRACK);
+}
 template <int DYN, int RISK, int NOISE, int RC, bool HALF>
-__global__ void __launch_bounds__(kRolloutThreads, DYN == DYN_BICYCLE ? RA_MIN_CTAS_BICYCLE : RA_MIN_CTAS_SINGLE_TRACK)
+__global__ void __launch_bounds__(kRolloutThreads, rollout_min_ctas<DYN, RC>())
 noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__ x0g,
                      float* __restrict__ L_out, float* __restrict__ xT_out) {
   constexpr int NX = StateDim<DYN>::value;
@@ -353,25 +360,67 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
 #pragma unroll
       for (int i = 0; i < NX; ++i) x[r][i] = x_init[i];
     }
-    RA_T_LOOP_UNROLL
-    for (int t = 0; t < p.T; ++t) {
+    // one transition of all RC realisations of this lane: l(x~_t) at the pre-step state, then
+    // x~_{t+1} = F(x~_t, u_t) + w_t   (6) PAPER.md:63 with w_t = wscale (.) a
+    auto advance = [&](int t, const float (&a)[RC][NX]) {
       const float4 ce = ce_s[t];
-      risk_accumulate<RISK, RC, NX>(p, circ_s, n_circ_s, lane, mf, x0X, x0Y, x, L);            // l(x~_t), pre-step
+      risk_accumulate<RISK, RC, NX>(p, circ_s, n_circ_s, lane, mf, x0X, x0Y, x, L);
 #pragma unroll
       for (int r = 0; r < RC; ++r) {
-        float z[NX];
-        if constexpr (NOISE == NOISE_MATERIALISED) {
-          const float* wp = p.w_mat + (((size_t)k * p.T + t) * NX) * p.M_pad + m[r];
-#pragma unroll
-          for (int i = 0; i < NX; ++i) z[i] = __ldg(wp + (size_t)i * p.M_pad);
-        } else {
-          state_noise<NX, NOISE>(p, kg, m[r], (uint32_t)t, c3, z);
-        }
-        dynamics_step<DYN, true>(p, x[r], ce);   // x~_{t+1} = F(x~_t, u_t) + w_t   (6) PAPER.md:63
+        dynamics_step<DYN, true>(p, x[r], ce);
 #pragma unroll
         for (int i = 0; i < NX; ++i)
-          x[r][i] = (NOISE == NOISE_MATERIALISED) ? x[r][i] + z[i] : fmaf(p.wscale[i], z[i], x[r][i]);
+          x[r][i] = (NOISE == NOISE_MATERIALISED) ? x[r][i] + a[r][i] : fmaf(p.wscale[i], a[r][i], x[r][i]);
         if constexpr (DYN == DYN_SINGLE_TRACK) x[r][3] = fmaxf(x[r][3], p.dyn_p[6]);
+      }
+    };
+    if constexpr (NOISE == NOISE_MATERIALISED) {
+      for (int t = 0; t < p.T; ++t) {
+        float a[RC][NX];
+#pragma unroll
+        for (int r = 0; r < RC; ++r) {
+          const float* wp = p.w_mat + (((size_t)k * p.T + t) * NX) * p.M_pad + m[r];
+#pragma unroll
+          for (int i = 0; i < NX; ++i) a[r][i] = __ldg(wp + (size_t)i * p.M_pad);
+        }
+        advance(t, a);
+      }
+    } else if constexpr (NoiseWords<NX, NOISE>::value == 6) {
+      // 1.5 Philox calls per step: two steps share three calls; the spare half of the middle call is carried
+      int t = 0;
+      for (; t + 1 < p.T; t += 2) {
+        const uint32_t c = 3u * (uint32_t)(t >> 1);
+        uint32_t carry[RC][2];
+        float a[RC][NX];
+#pragma unroll
+        for (int r = 0; r < RC; ++r) {
+          const uint4 qa = philox4x32_10(kg, m[r], c, c3, p.rk), qb = philox4x32_10(kg, m[r], c + 1u, c3, p.rk);
+          const uint32_t w[6] = {qa.x, qa.y, qa.z, qa.w, qb.x, qb.y};
+          carry[r][0] = qb.z; carry[r][1] = qb.w;
+          noise_from_words<NX, NOISE>(p, w, a[r]);
+        }
+        advance(t, a);
+#pragma unroll
+        for (int r = 0; r < RC; ++r) {
+          const uint4 qc = philox4x32_10(kg, m[r], c + 2u, c3, p.rk);
+          const uint32_t w[6] = {carry[r][0], carry[r][1], qc.x, qc.y, qc.z, qc.w};
+          noise_from_words<NX, NOISE>(p, w, a[r]);
+        }
+        advance(t + 1, a);
+      }
+      if (t < p.T) {   // odd horizon: the last (even-indexed) step on its own
+        float a[RC][NX];
+#pragma unroll
+        for (int r = 0; r < RC; ++r) state_noise<NX, NOISE>(p, kg, m[r], (uint32_t)t, c3, a[r]);
+        advance(t, a);
+      }
+    } else {
+      RA_T_LOOP_UNROLL
+      for (int t = 0; t < p.T; ++t) {
+        float a[RC][NX];
+#pragma unroll
+        for (int r = 0; r < RC; ++r) state_noise<NX, NOISE>(p, kg, m[r], (uint32_t)t, c3, a[r]);
+        advance(t, a);
       }
     }
 #pragma unroll

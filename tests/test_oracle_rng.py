@@ -127,17 +127,32 @@ def test_normal_moments():
     assert np.abs(c - np.eye(4)).max() < 5 / np.sqrt(zz.shape[0])
 
 
-def test_single_track_uses_two_calls_and_six_components():
+def test_single_track_takes_six_words_per_step_from_the_word_stream():
+    """D:RNG layout: step t of an n_x = 6 realisation takes words 6t..6t+5 of its stream, word n = output n%4 of
+    call n//4; the n_x = 4 layout at step c IS call c, so it serves as the reference for the call contents."""
     class P6(_P):
         dyn = 1; dyn_p = [4, 0.05, 0.17, 0.17, 30, 30, 0.5]
     orc4, orc6 = O.Oracle(_P), O.Oracle(P6)
-    w6 = orc6.state_noise(3, 4, 5, 1, 6)
-    assert w6.shape == (6,)
-    # call j=0 of the n_x=6 layout has counter c2 = t*2+0; the n_x=4 layout at t'=2t gives the same call
-    w4 = orc4.state_noise(3, 4, 10, 1, 6)
-    assert np.array_equal(w6[:4], w4)
-    w4b = orc4.state_noise(3, 4, 11, 1, 6)
-    assert np.array_equal(w6[4:], w4b[:2])
+    call = lambda c: orc4.state_noise(3, 4, c, 1, 6)          # the four normals of call c
+    w_even = orc6.state_noise(3, 4, 4, 1, 6)                   # words 24..29 = call 6 (all), call 7 (outputs 0,1)
+    assert w_even.shape == (6,)
+    assert np.array_equal(w_even[:4], call(6)) and np.array_equal(w_even[4:], call(7)[:2])
+    w_odd = orc6.state_noise(3, 4, 5, 1, 6)                    # words 30..35 = call 7 (outputs 2,3), call 8 (all)
+    assert np.array_equal(w_odd[:2], call(7)[2:]) and np.array_equal(w_odd[2:], call(8))
+    # consecutive steps never reuse a word: 1.5 calls per step on average, no overlap, no gap
+    assert not np.intersect1d(w_even, w_odd).size
+
+
+def test_jump_noise_word_layout():
+    """Jump noise takes n_x + 2 words per step: the components, the trigger, one spare (pairs stay aligned)."""
+    class PJ(_P):
+        noise_kind = 2; noise_p = [1.0, 0, 0, 0]     # always jump: the direction is the normalised Gaussian draw
+    orcj, orc4 = O.Oracle(PJ), O.Oracle(_P)
+    call = lambda c: orc4.state_noise(7, 9, c, 1, 2)
+    for t in (0, 1, 2, 3):                           # words 6t..6t+3 are the components
+        n0 = 6 * t
+        z = np.concatenate([call(n0 // 4), call(n0 // 4 + 1)])[n0 % 4: n0 % 4 + 4]
+        assert np.allclose(orcj.state_noise(7, 9, t, 1, 2), z / np.linalg.norm(z), rtol=1e-13)
 
 
 def test_uniform_and_jump_noise_kinds():
