@@ -31,7 +31,7 @@ struct ra_mppi_ctx {
   float4* d_ce = nullptr;
   double* d_S = nullptr;
   float* d_cvar = nullptr;
-  double* d_S_tilde = nullptr;
+  double* d_pen = nullptr;
   float* d_w_mat = nullptr;
   LoopState* d_loop = nullptr;
   // closed-loop graph cache
@@ -39,6 +39,10 @@ struct ra_mppi_ctx {
   float* d_stage = nullptr;  // [nx + 2T]
   bool timing = false;
   cudaEvent_t ev_k0 = nullptr, ev_k1 = nullptr;
+  // the nominal rollout (A2) runs beside the noisy rollouts (A3-A7) on this stream, forked from and
+  // joined back into the caller's stream with the two events (captured as parallel graph branches)
+  cudaStream_t side = nullptr;
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
   cudaGraphExec_t graph_exec = nullptr;
   float *g_x0 = nullptr, *g_v = nullptr, *g_log = nullptr;
   std::string err;
@@ -203,6 +207,16 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
 #ifdef RA_FORCE_WPS
   if (!c->half) p.wps = RA_FORCE_WPS;
 #endif
+  {
+    // shared-memory carveout (percent of the 228 KB unified L1) that holds three rollout CTAs; the nominal-rollout
+    // kernel asks for the same split so both kernels can share an SM
+    const bool circ = cfg->risk == RA_RISK_CIRCLES || cfg->nominal == RA_NOM_RACING;
+    const size_t ce_slots = c->half ? 2 * kRolloutWarps : kRolloutWarps / p.wps;
+    const size_t smem_cta = (circ && env ? (size_t)((env->n_circles + 31) & ~31) * sizeof(float4) : 0) +
+                            ce_slots * cfg->T * sizeof(float4) + (size_t)kRolloutWarps * p.R_total * 32 * sizeof(uint32_t);
+    const size_t need = 3 * (smem_cta + 1024);
+    p.carveout = need <= 57 * 1024 ? 25 : (need <= 114 * 1024 ? 50 : 100);
+  }
   p.nx = cfg->dyn == RA_DYN_SINGLE_TRACK ? 6 : 4;
   p.dt = cfg->dt;
   std::memcpy(p.dyn_p, cfg->dyn_p, sizeof p.dyn_p);
@@ -276,11 +290,15 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
   const size_t KT = (size_t)cfg->K * cfg->T;
   if (dev_alloc(&c->d_u_raw, KT) != cudaSuccess || dev_alloc(&c->d_ce, KT) != cudaSuccess ||
       dev_alloc(&c->d_S, (size_t)cfg->K) != cudaSuccess || dev_alloc(&c->d_cvar, (size_t)cfg->K) != cudaSuccess ||
-      dev_alloc(&c->d_S_tilde, (size_t)cfg->K) != cudaSuccess || dev_alloc(&c->d_loop, 1) != cudaSuccess ||
+      dev_alloc(&c->d_pen, (size_t)cfg->K) != cudaSuccess || dev_alloc(&c->d_loop, 1) != cudaSuccess ||
       dev_alloc(&c->d_stage, (size_t)(8 + 2 * cfg->T)) != cudaSuccess)
     return bail(RA_ENOMEM);
-  p.u_raw = c->d_u_raw; p.ce = c->d_ce; p.S = c->d_S; p.cvar = c->d_cvar; p.S_tilde = c->d_S_tilde;
+  p.u_raw = c->d_u_raw; p.ce = c->d_ce; p.S = c->d_S; p.cvar = c->d_cvar; p.pen = c->d_pen;
   if (cudaMemset(c->d_loop, 0, sizeof(LoopState)) != cudaSuccess) return bail(RA_ECUDA);
+  if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess)
+    return bail(RA_ECUDA);
   p.M_pad = p.R_total * p.G;
   if (cfg->noise_mode == RA_NOISE_MATERIALISED) {
     const size_t n = KT * (size_t)p.nx * (size_t)p.M_pad;
@@ -298,9 +316,12 @@ ra_status ra_mppi_destroy(ra_mppi_ctx* c) {
   if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
   cudaFree(c->d_circles); cudaFree(c->d_costmap); cudaFree(c->d_u_raw); cudaFree(c->d_ce);
   cudaFree(c->d_stage);
+  if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+  if (c->ev_join) cudaEventDestroy(c->ev_join);
+  if (c->side) cudaStreamDestroy(c->side);
   if (c->ev_k0) cudaEventDestroy(c->ev_k0);
   if (c->ev_k1) cudaEventDestroy(c->ev_k1);
-  cudaFree(c->d_S); cudaFree(c->d_cvar); cudaFree(c->d_S_tilde); cudaFree(c->d_w_mat); cudaFree(c->d_loop);
+  cudaFree(c->d_S); cudaFree(c->d_cvar); cudaFree(c->d_pen); cudaFree(c->d_w_mat); cudaFree(c->d_loop);
   delete c;
   return RA_OK;
 }
@@ -312,15 +333,31 @@ const char* ra_mppi_last_error(const ra_mppi_ctx* c) { return c ? c->err.c_str()
 
 namespace {
 
-cudaError_t launch_sample_nominal(const ra_mppi_ctx* c, const Params& p, const float* d_x0, const float* d_v,
-                                  cudaStream_t s) {
-  const int threads = kSampleThreads, grid = (p.K + kSampleKB - 1) / kSampleKB;
-  const size_t smem = (size_t)p.T * kSampleKB * (sizeof(float4) + sizeof(float)) + (size_t)2 * p.T * sizeof(float);
+cudaError_t launch_sample(const ra_mppi_ctx* c, const Params& p, const float* d_v, cudaStream_t s) {
+  const int grid = (p.K + kSampleKB - 1) / kSampleKB;
+  if (c->cfg.dyn == 0) sample_kernel<0><<<grid, kSampleThreads, 0, s>>>(p, d_v);
+  else sample_kernel<1><<<grid, kSampleThreads, 0, s>>>(p, d_v);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_nominal(const ra_mppi_ctx* c, const Params& p, const float* d_x0, const float* d_v,
+                           cudaStream_t s) {
+  const int grid = (p.K + kNominalThreads - 1) / kNominalThreads;
   const int dyn = c->cfg.dyn, nom = c->cfg.nominal;
-#define RA_SN(D, N) sample_nominal_kernel<D, N><<<grid, threads, smem, s>>>(p, d_x0, d_v)
-  if (dyn == 0) { if (nom == 0) RA_SN(0, 0); else if (nom == 1) RA_SN(0, 1); else RA_SN(0, 2); }
-  else { if (nom == 0) RA_SN(1, 0); else if (nom == 1) RA_SN(1, 1); else RA_SN(1, 2); }
-#undef RA_SN
+#define RA_NOMK(D, N)                                                                                          \
+  do {                                                                                                         \
+    static int carveout_set = -1;   /* same L1 / shared-memory split as the rollout kernel (rollout_inst.cu) */ \
+    if (carveout_set != p.carveout) {                                                                          \
+      const cudaError_t e = cudaFuncSetAttribute(nominal_kernel<D, N>,                                         \
+                                                 cudaFuncAttributePreferredSharedMemoryCarveout, p.carveout);  \
+      if (e != cudaSuccess) return e;                                                                          \
+      carveout_set = p.carveout;                                                                               \
+    }                                                                                                          \
+    nominal_kernel<D, N><<<grid, kNominalThreads, 0, s>>>(p, d_x0, d_v);                                       \
+  } while (0)
+  if (dyn == 0) { if (nom == 0) RA_NOMK(0, 0); else if (nom == 1) RA_NOMK(0, 1); else RA_NOMK(0, 2); }
+  else { if (nom == 0) RA_NOMK(1, 0); else if (nom == 1) RA_NOMK(1, 1); else RA_NOMK(1, 2); }
+#undef RA_NOMK
   return cudaGetLastError();
 }
 
@@ -342,24 +379,31 @@ ra_status enqueue_costs(ra_mppi_ctx* c, const Params& p, const float* d_x0, cons
   // A = 0 is the baseline MPPI of section II: S~ = S by (14)-(16), so unless the caller
   // asks for the risk diagnostics the M noisy rollouts are not needed at all.
   if (c->cfg.A == 0.0f && !diagnostics) {
-    RA_CUDA(c, launch_sample_nominal(c, p, d_x0, d_v, s));
+    RA_CUDA(c, launch_sample(c, p, d_v, s));
+    RA_CUDA(c, launch_nominal(c, p, d_x0, d_v, s));
     RA_CUDA(c, cudaMemsetAsync(c->d_cvar, 0, (size_t)p.K * sizeof(float), s));
-    RA_CUDA(c, cudaMemcpyAsync(c->d_S_tilde, c->d_S, (size_t)p.K * sizeof(double), cudaMemcpyDeviceToDevice, s));
+    RA_CUDA(c, cudaMemsetAsync(c->d_pen, 0, (size_t)p.K * sizeof(double), s));
     return RA_OK;
   }
   if (c->cfg.noise_mode == RA_NOISE_MATERIALISED)
     RA_CUDA(c, p.nx == 4 ? launch_materialise<4>(c, p, s) : launch_materialise<6>(c, p, s));
-  RA_CUDA(c, launch_sample_nominal(c, p, d_x0, d_v, s));
+  RA_CUDA(c, launch_sample(c, p, d_v, s));
+  // fork: the K*T nominal rollout needs only the sampled controls and hides under the K*M*T noisy ones
+  RA_CUDA(c, cudaEventRecord(c->ev_fork, s));
+  RA_CUDA(c, cudaStreamWaitEvent(c->side, c->ev_fork, 0));
+  RA_CUDA(c, launch_nominal(c, p, d_x0, d_v, c->side));
+  RA_CUDA(c, cudaEventRecord(c->ev_join, c->side));
   if (c->timing) RA_CUDA(c, cudaEventRecord(c->ev_k0, s));
   RA_CUDA(c, c->rollout(p, c->noise_variant, c->rc, c->half, d_x0, d_L, d_xT, s));
   if (c->timing) RA_CUDA(c, cudaEventRecord(c->ev_k1, s));
+  RA_CUDA(c, cudaStreamWaitEvent(s, c->ev_join, 0));   // join
   return RA_OK;
 }
 
 // Alg.1 l.31: weights (17) and update (4) from the context scratch.
 ra_status enqueue_update(ra_mppi_ctx* c, const Params& p, float* d_v_out, cudaStream_t s) {
   weights_update_kernel<double><<<p.T, kUpdateThreads, 0, s>>>(
-      p, p.S_tilde, p.u_raw, 1LL, (long long)p.K, d_v_out, nullptr, nullptr, nullptr);
+      p, p.S, p.pen, p.u_raw, 1LL, (long long)p.K, d_v_out, nullptr, nullptr, nullptr);
   RA_CUDA(c, cudaGetLastError());
   return RA_OK;
 }
@@ -367,7 +411,7 @@ ra_status enqueue_update(ra_mppi_ctx* c, const Params& p, float* d_v_out, cudaSt
 // The shard's share of (17)/(4) for the K-sharded step.
 ra_status enqueue_partial(ra_mppi_ctx* c, const Params& p, double* d_partial, cudaStream_t s) {
   weights_update_kernel<double><<<p.T, kUpdateThreads, 0, s>>>(
-      p, p.S_tilde, p.u_raw, 1LL, (long long)p.K, nullptr, nullptr, nullptr, d_partial);
+      p, p.S, p.pen, p.u_raw, 1LL, (long long)p.K, nullptr, nullptr, nullptr, d_partial);
   RA_CUDA(c, cudaGetLastError());
   return RA_OK;
 }
@@ -447,7 +491,7 @@ ra_status ra_mppi_weights_update(ra_mppi_ctx* c, const float* d_S_tilde, const f
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const Params p = with_iteration(c, 0);
   weights_update_kernel<float><<<p.T, kUpdateThreads, 0, s>>>(
-      p, d_S_tilde, reinterpret_cast<const float2*>(d_u), (long long)p.T, 1LL, d_v_plus, d_w, d_stats, nullptr);
+      p, d_S_tilde, nullptr, reinterpret_cast<const float2*>(d_u), (long long)p.T, 1LL, d_v_plus, d_w, d_stats, nullptr);
   RA_CUDA(c, cudaGetLastError());
   return RA_OK;
 }
@@ -497,16 +541,17 @@ ra_status ra_mppi_last_rollout_ms(ra_mppi_ctx* c, float* h_ms) {
 ra_status ra_mppi_export_costs_f64(ra_mppi_ctx* c, double* d_S64, double* d_S_tilde64, void* stream) {
   if (!c) return RA_EINVAL;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
-  const size_t n = (size_t)c->p.K * sizeof(double);
-  if (d_S64) RA_CUDA(c, cudaMemcpyAsync(d_S64, c->d_S, n, cudaMemcpyDeviceToDevice, s));
-  if (d_S_tilde64) RA_CUDA(c, cudaMemcpyAsync(d_S_tilde64, c->d_S_tilde, n, cudaMemcpyDeviceToDevice, s));
+  if (d_S64 || d_S_tilde64) {
+    export_costs_f64_kernel<<<(c->p.K + 255) / 256, 256, 0, s>>>(c->p, d_S64, d_S_tilde64);
+    RA_CUDA(c, cudaGetLastError());
+  }
   return RA_OK;
 }
 
 int32_t ra_mppi_launches_per_step(const ra_mppi_ctx* c) {
   if (!c) return 0;
-  if (c->cfg.A == 0.0f) return 2;   // baseline MPPI: sampling/nominal + weights/update
-  return 3 + (c->cfg.noise_mode == RA_NOISE_MATERIALISED ? 1 : 0);
+  if (c->cfg.A == 0.0f) return 3;   // baseline MPPI: sampling, nominal rollout, weights/update
+  return 4 + (c->cfg.noise_mode == RA_NOISE_MATERIALISED ? 1 : 0);   // + noisy rollouts (+ noise generator)
 }
 
 ra_status ra_mppi_philox(ra_mppi_ctx* c, const uint32_t* d_ctr, int32_t n, uint32_t* d_out, void* stream) {

@@ -22,6 +22,7 @@ struct Params {
   int R_total;  // realisation slots of G lanes per sample = ceil(M / G)
   int wps;      // warps per control sample in the rollout kernel (1, 2, 4 or 8)
   int nx;
+  int carveout; // host only: preferred shared-memory carveout (percent) of the two concurrent rollout kernels
   float dt;
   float dyn_p[8];
   float dyn_q[2];   // single-track: 1/m, 1/Iz
@@ -47,7 +48,7 @@ struct Params {
   float4* ce;      // [K][T] control effects consumed by the rollout kernels
   double* S;        // [K] nominal cost (3), fp64 so weight errors come from q, not from the sum
   float* cvar;      // [K]
-  double* S_tilde;  // [K] modified cost (16)
+  double* pen;      // [K] soft-filter term J_C of (14); the modified cost (16) is S + pen
   const float* w_mat;  // materialised noise [K][T][nx][M_pad] or nullptr
   int M_pad;
   // iteration index: device-resident when replayed from a graph, immediate otherwise

@@ -1,5 +1,6 @@
 // Rollout kernels of the RA-MPPI iteration (Alg.1 l.3-29).
-//   sample_nominal_kernel : A1 + A2  (one thread per control sample k)
+//   sample_kernel         : A1       (parallel over (k, t))
+//   nominal_kernel        : A2       (one thread per control sample k)
 //   noisy_rollout_kernel  : A3 + A4 + A5 + A6 + A7 (one warp, or half-warp when M <= 16, per
 //                           control sample; lanes over the M realisations; noise in registers)
 #pragma once
@@ -24,28 +25,16 @@ constexpr int kRolloutWarps = kRolloutThreads / 32;
 constexpr int NOISE_MATERIALISED = 3;  // rollout-kernel variant that reads w from HBM
 
 // ---------------------------------------------------------------------------------------
-// A1 + A2.  eps^k_t = sigma_eps (.) z, u^k_t = (k < K0 ? v_t : 0) + eps^k_t   (2c) PAPER.md:42,
-// Alg.1 l.4-10; nominal rollout and S_k = sum_t [q(x_t) + gamma v_t^T Sigma^-1 u_t] + phi(x_T)
-// (3) PAPER.md:47, Alg.1 l.11-15.  S is accumulated in fp64 (K*T adds only) because the
-// softmin weights of (17) are sensitive to absolute errors in S~.
+// A1.  eps^k_t = sigma_eps (.) z, u^k_t = (k < K0 ? v_t : 0) + eps^k_t   (2c) PAPER.md:42, Alg.1 l.4-10.
+// Parallel over (k, t): Philox + accurate Box-Muller + tan / sincos of the clamped control, once per
+// (k, t).  Writes u_raw[T][K] (for the update (4)) and the control effects ce[K][T] (for both rollouts).
 // ---------------------------------------------------------------------------------------
 constexpr int kSampleThreads = 128;
 constexpr int kSampleKB = 16;  // control samples per CTA
 
-template <int DYN, int NOM>
-__global__ void __launch_bounds__(kSampleThreads) sample_nominal_kernel(const __grid_constant__ Params p,
-                                                                        const float* __restrict__ x0g,
-                                                                        const float* __restrict__ v) {
-  constexpr int NX = StateDim<DYN>::value;
-  // Phase 1 is parallel over (k, t): Philox + Box-Muller + tan/sincos of the clamped control are
-  // independent across the horizon, so the K*T sampling work is spread over all threads.
-  // Phase 2 is the only sequential chain: one thread per sample rolls the nominal state forward.
-  extern __shared__ float4 sn_smem[];
-  float4* ce_s = sn_smem;                                              // [T][KB]
-  float* ctrl_s = reinterpret_cast<float*>(ce_s + (size_t)p.T * kSampleKB);  // [T][KB]
-  float* v_s = ctrl_s + (size_t)p.T * kSampleKB;                        // [T][2]
-  for (int i = threadIdx.x; i < 2 * p.T; i += blockDim.x) v_s[i] = v[i];
-  __syncthreads();
+template <int DYN>
+__global__ void __launch_bounds__(kSampleThreads) sample_kernel(const __grid_constant__ Params p,
+                                                                const float* __restrict__ v) {
   const int k0 = blockIdx.x * kSampleKB;
   const uint32_t c3 = iteration_field(p, STREAM_EPS);
   for (int idx = threadIdx.x; idx < p.T * kSampleKB; idx += blockDim.x) {
@@ -55,30 +44,45 @@ __global__ void __launch_bounds__(kSampleThreads) sample_nominal_kernel(const __
     float z0, z1;
     box_muller(r.x, r.y, z0, z1);
     const bool with_mean = k + p.k_off < p.K0;
-    const float v0 = v_s[2 * t], v1 = v_s[2 * t + 1];
-    const float u0 = fmaf(p.sigma_eps[0], z0, with_mean ? v0 : 0.0f);
-    const float u1 = fmaf(p.sigma_eps[1], z1, with_mean ? v1 : 0.0f);
-    const float4 ce = control_effect<DYN>(p, u0, u1);
+    const float u0 = fmaf(p.sigma_eps[0], z0, with_mean ? __ldg(v + 2 * t) : 0.0f);
+    const float u1 = fmaf(p.sigma_eps[1], z1, with_mean ? __ldg(v + 2 * t + 1) : 0.0f);
     p.u_raw[(size_t)t * p.K + k] = make_float2(u0, u1);
-    p.ce[(size_t)k * p.T + t] = ce;
-    ce_s[idx] = ce;
-    ctrl_s[idx] = fmaf(p.ctrl_w[0] * v0, u0, p.ctrl_w[1] * v1 * u1);   // gamma v^T Sigma^-1 u  (3)
+    p.ce[(size_t)k * p.T + t] = control_effect<DYN>(p, u0, u1);
   }
-  __syncthreads();
-  const int k = k0 + threadIdx.x;
-  if (threadIdx.x >= kSampleKB || k >= p.K) return;
+}
 
+// ---------------------------------------------------------------------------------------
+// A2.  Nominal rollout and S_k = sum_t [q(x_t) + gamma v_t^T Sigma^-1 u_t] + phi(x_T)   (3) PAPER.md:47,
+// Alg.1 l.11-15: one thread per control sample (the only sequential chain of the K*T work), full warps.
+// S is accumulated in fp64 (K*T adds only) because the softmin weights of (17) are sensitive to
+// absolute errors in S~.  Independent of the noisy rollouts, so ra_mppi_step runs it beside them.
+// ---------------------------------------------------------------------------------------
+#ifndef RA_NOMINAL_THREADS
+#define RA_NOMINAL_THREADS 64
+#endif
+constexpr int kNominalThreads = RA_NOMINAL_THREADS;
+
+template <int DYN, int NOM>
+__global__ void __launch_bounds__(kNominalThreads) nominal_kernel(const __grid_constant__ Params p,
+                                                                  const float* __restrict__ x0g,
+                                                                  const float* __restrict__ v) {
+  constexpr int NX = StateDim<DYN>::value;
+  const int k = blockIdx.x * kNominalThreads + threadIdx.x;
+  if (k >= p.K) return;
   const float x0X = x0g[0], x0Y = x0g[1];
   float x[NX];
   x[0] = 0.0f; x[1] = 0.0f;
 #pragma unroll
   for (int i = 2; i < NX; ++i) x[i] = x0g[i];
   if constexpr (DYN == DYN_SINGLE_TRACK) x[3] = fmaxf(x[3], p.dyn_p[6]);
+  const float4* ce_k = p.ce + (size_t)k * p.T;
   double S = 0.0;
   for (int t = 0; t < p.T; ++t) {
+    const float2 u = p.u_raw[(size_t)t * p.K + k];
+    const float ctrl = fmaf(p.ctrl_w[0] * __ldg(v + 2 * t), u.x, p.ctrl_w[1] * __ldg(v + 2 * t + 1) * u.y);  // gamma v^T Sigma^-1 u  (3)
     const float q = nominal_cost<NOM>(p, x0X + x[0], x0Y + x[1], x[3]);
-    S += (double)q + (double)ctrl_s[t * kSampleKB + threadIdx.x];
-    dynamics_step<DYN>(p, x, ce_s[t * kSampleKB + threadIdx.x]);
+    S += (double)q + (double)ctrl;
+    dynamics_step<DYN>(p, x, ce_k[t]);
   }
   S += (double)terminal_cost<NOM>(p, x0X + x[0], x0Y + x[1], x[3], x0X, x0Y);
   p.S[k] = S;
@@ -453,9 +457,8 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
   if (p.B != 1.0f) cvar = fmaf(p.B, cvar - Lbar, Lbar);
   if (sub == 0 && k_valid) {
     // soft filter (14)-(16) PAPER.md:120-130, strict threshold (15)
-    const double pen = (cvar > p.C_u) ? (double)(p.A * cvar) : 0.0;
     p.cvar[k] = cvar;
-    p.S_tilde[k] = p.S[k] + pen;
+    p.pen[k] = (cvar > p.C_u) ? (double)(p.A * cvar) : 0.0;   // J_C of (14); S~ = S + J_C is formed by its readers
   }
 }
 

@@ -26,6 +26,14 @@ cudaError_t launch(const Params& p, const float* d_x0, float* d_L, float* d_xT, 
         cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 80 * 1024);
     if (attr != cudaSuccess) return attr;
   }
+  // the same L1 / shared-memory split as the nominal-rollout kernel that runs beside this one: CTAs of kernels
+  // with different carveouts do not share an SM (measured: +20 us per closed-loop iteration otherwise)
+  static int carveout_set = -1;
+  if (carveout_set != p.carveout) {
+    const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, p.carveout);
+    if (e != cudaSuccess) return e;
+    carveout_set = p.carveout;
+  }
   kernel<<<grid, kRolloutThreads, smem, stream>>>(p, d_x0, d_L, d_xT);
   return cudaGetLastError();
 }

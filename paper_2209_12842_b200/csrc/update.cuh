@@ -30,22 +30,29 @@ __device__ __forceinline__ T block_reduce(T v, T* smem, Op op, T identity) {
 // u is addressed as u[k*su_k + t*su_t] so both the internal [T][K] scratch and a caller's
 // [K][T] array work.  Reduction order is fixed => bitwise reproducible.
 // ---------------------------------------------------------------------------------------
+// S~_k (16): the caller's array (ST = float), or S + J_C from the context scratch (ST = double, pen != nullptr)
+template <typename ST>
+__device__ __forceinline__ ST s_tilde_at(const ST* __restrict__ S, const double* __restrict__ pen, int k) {
+  if constexpr (sizeof(ST) == sizeof(double)) return pen ? S[k] + pen[k] : S[k];
+  else return S[k];
+}
+
 template <typename ST>
 __global__ void __launch_bounds__(kUpdateThreads)
 weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S_tilde,
-                      const float2* __restrict__ u, long long su_k, long long su_t,
+                      const double* __restrict__ pen, const float2* __restrict__ u, long long su_k, long long su_t,
                       float* __restrict__ v_out, float* __restrict__ w_out,
                       float* __restrict__ stats, double* __restrict__ partial) {
   __shared__ ST red_s[32];
   __shared__ float red_f[96];
   const int t = blockIdx.x;
   ST bmin = (ST)INFINITY;
-  for (int k = threadIdx.x; k < p.K; k += blockDim.x) bmin = min(bmin, S_tilde[k]);
+  for (int k = threadIdx.x; k < p.K; k += blockDim.x) bmin = min(bmin, s_tilde_at<ST>(S_tilde, pen, k));
   const ST beta = block_reduce<ST>(bmin, red_s, [](ST a, ST b) { return a < b ? a : b; }, (ST)INFINITY);
 
   float Z = 0.0f, n0 = 0.0f, n1 = 0.0f;
   for (int k = threadIdx.x; k < p.K; k += blockDim.x) {
-    const float w = exp2f((float)(S_tilde[k] - beta) * p.neg_log2e_over_lambda);
+    const float w = exp2f((float)(s_tilde_at<ST>(S_tilde, pen, k) - beta) * p.neg_log2e_over_lambda);
     const float2 uk = __ldg(u + (long long)k * su_k + (long long)t * su_t);
     Z += w;
     n0 = fmaf(w, uk.x, n0);
@@ -88,7 +95,7 @@ weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S
   if (t == 0 && w_out) {
     const float invZ = 1.0f / Z;
     for (int k = threadIdx.x; k < p.K; k += blockDim.x)
-      w_out[k] = exp2f((float)(S_tilde[k] - beta) * p.neg_log2e_over_lambda) * invZ;
+      w_out[k] = exp2f((float)(s_tilde_at<ST>(S_tilde, pen, k) - beta) * p.neg_log2e_over_lambda) * invZ;
   }
 }
 
@@ -129,7 +136,16 @@ __global__ void export_costs_kernel(const __grid_constant__ Params p, float* __r
   if (k >= p.K) return;
   if (S) S[k] = (float)p.S[k];
   if (cvar) cvar[k] = p.cvar[k];
-  if (S_tilde) S_tilde[k] = (float)p.S_tilde[k];
+  if (S_tilde) S_tilde[k] = (float)(p.S[k] + p.pen[k]);
+}
+
+// fp64 S and S~ = S + J_C of the context scratch (ra_mppi_export_costs_f64)
+__global__ void export_costs_f64_kernel(const __grid_constant__ Params p, double* __restrict__ S,
+                                        double* __restrict__ S_tilde) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= p.K) return;
+  if (S) S[k] = p.S[k];
+  if (S_tilde) S_tilde[k] = p.S[k] + p.pen[k];
 }
 
 // Device-resident loop state for graph replay.

@@ -114,4 +114,4 @@ def test_kernel_timing_hook(torch_cuda):
     ctl.step(d_x0, d_v, 0)
     ms = ctl.last_rollout_ms()
     assert 0.0 < ms < 100.0
-    assert ctl.launches_per_step == 3
+    assert ctl.launches_per_step == 4   # sampling, nominal rollout, noisy rollouts, weights/update

@@ -278,7 +278,7 @@ def test_baseline_mppi_mode_skips_the_noisy_rollouts(torch_cuda):
     torch = torch_cuda
     p = _with_v(W.small(W.config1(), K=300, M=64, T=25)).replace(A=0.0, lam=50.0)
     ctl, orc = _ctl(p), O.Oracle(p)
-    assert ctl.launches_per_step == 2
+    assert ctl.launches_per_step == 3      # sampling, nominal rollout, weights/update
     d_x0, d_v = ctl.tensor(p.x0), ctl.tensor(p.v)
     ctl.step(d_x0, d_v, 3)
     S64, St64 = ctl.costs_f64()
@@ -289,4 +289,4 @@ def test_baseline_mppi_mode_skips_the_noisy_rollouts(torch_cuda):
     # the diagnostic call still runs the risk path and reports CVaR, with S~ = S
     g, r = check_rollout_parity(p, ctl, orc, iteration=3)
     assert (g["cvar"] > 0).any() and np.array_equal(g["S"], g["S_tilde"])
-    assert _ctl(p.replace(A=1.0)).launches_per_step == 3
+    assert _ctl(p.replace(A=1.0)).launches_per_step == 4
