@@ -98,6 +98,12 @@ typedef struct {
  * context (NULL on failure).  RA_EINVAL / RA_EUNSUPPORTED / RA_ECUDA / RA_ENOMEM.        */
 ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_mppi_ctx** out);
 
+/* Replace the environment of an existing context (moving obstacles, a refreshed costmap): env is HOST memory,
+ * copied before the call returns.  Up to 1024 circles; a costmap must keep the map_h x map_w it had at create
+ * (resolution and origin may change).  Synchronises the device and drops the captured closed-loop graph.
+ * Not capturable.  RA_EINVAL / RA_EUNSUPPORTED / RA_ECUDA.                                                */
+ra_status ra_mppi_set_env(ra_mppi_ctx* ctx, const ra_mppi_env* env);
+
 /* One full iteration, Alg.1 l.3-31: sample u^k = v + eps^k, nominal
  * and noisy rollouts, risk costs (9), CVaR (12), soft filter (14)-(16), weights (17),
  * update (4).  d_x0 [n_x] current state; d_v [T,2] in: mean control v, out: v+ (clamped).

@@ -53,7 +53,7 @@ class ra_mppi_env(C.Structure):
 
 
 EXPORTS = (
-    "ra_mppi_create", "ra_mppi_step", "ra_mppi_rollout_costs", "ra_mppi_weights_update",
+    "ra_mppi_create", "ra_mppi_set_env", "ra_mppi_step", "ra_mppi_rollout_costs", "ra_mppi_weights_update",
     "ra_mppi_step_partial", "ra_mppi_combine_partials",
     "ra_mppi_step_host", "ra_mppi_enable_kernel_timing", "ra_mppi_last_rollout_ms",
     "ra_mppi_export_costs_f64", "ra_mppi_plant_shift", "ra_mppi_closed_loop", "ra_mppi_philox", "ra_mppi_state_noise",
@@ -75,6 +75,7 @@ def load():
     L = C.CDLL(LIB_PATH)
     vp, fp, u64, i32 = C.c_void_p, C.c_void_p, C.c_uint64, C.c_int32
     L.ra_mppi_create.argtypes = [C.POINTER(ra_mppi_config), C.POINTER(ra_mppi_env), C.POINTER(vp)]
+    L.ra_mppi_set_env.argtypes = [vp, C.POINTER(ra_mppi_env)]
     L.ra_mppi_step.argtypes = [vp, fp, fp, u64, vp]
     L.ra_mppi_rollout_costs.argtypes = [vp, fp, fp, u64, fp, fp, fp, fp, fp, fp, vp]
     L.ra_mppi_step_partial.argtypes = [vp, fp, fp, u64, vp, vp]
@@ -161,6 +162,10 @@ def ra_mppi_create(cfg: ra_mppi_config, env: ra_mppi_env):
     st = load().ra_mppi_create(C.byref(cfg), C.byref(env), C.byref(ctx))
     _check(None, st, "ra_mppi_create")
     return ctx
+
+
+def ra_mppi_set_env(ctx, env: ra_mppi_env):
+    _check(ctx, load().ra_mppi_set_env(ctx, C.byref(env)), "ra_mppi_set_env")
 
 
 def ra_mppi_step(ctx, d_x0, d_v, iteration, stream=0):

@@ -32,6 +32,20 @@ class RaMppi:
         except Exception:
             pass
 
+    def set_env(self, circles=None, costmap=None, map_res=None, map_ox=None, map_oy=None):
+        """ra_mppi_set_env: replace the obstacle set and/or the costmap (same map size) of this controller."""
+        kw = {}
+        if circles is not None:
+            kw["circles"] = np.asarray(circles)
+        if costmap is not None:
+            kw["costmap"] = np.asarray(costmap)
+        for name, val in (("map_res", map_res), ("map_ox", map_ox), ("map_oy", map_oy)):
+            if val is not None:
+                kw[name] = float(val)
+        self.problem = self.problem.replace(**kw)
+        self.env, self._keep = B.make_env(self.problem)
+        B.ra_mppi_set_env(self.ctx, self.env)
+
     # ---- helpers
     def tensor(self, a, dtype=torch.float32):
         return torch.as_tensor(np.ascontiguousarray(a), dtype=dtype).to(self.device).contiguous()

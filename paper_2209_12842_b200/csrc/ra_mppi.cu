@@ -150,6 +150,50 @@ void philox_round_keys(uint64_t seed, uint32_t rk[20]) {
 template <typename T>
 cudaError_t dev_alloc(T** p, size_t n) { return cudaMalloc(reinterpret_cast<void**>(p), n * sizeof(T)); }
 
+// Copies the environment into the context (synchronously).  first = allocate: the obstacle buffer holds
+// kMaxCirclesSmem records and the costmap table its create-time size, so later uploads never allocate.
+ra_status upload_env(ra_mppi_ctx* c, const ra_mppi_env* env, bool first) {
+  const ra_mppi_config* cfg = &c->cfg;
+  Params& p = c->p;
+  if (cfg->risk == RA_RISK_CIRCLES || cfg->nominal == RA_NOM_RACING) {
+    const float margin = cfg->risk == RA_RISK_CIRCLES ? cfg->risk_p[1] : 0.0f;   // (22) has no margin
+    std::vector<float4> h((size_t)std::max(env->n_circles, 1));
+    for (int i = 0; i < env->n_circles; ++i)
+      h[i] = make_float4(env->circles[3 * i], env->circles[3 * i + 1], env->circles[3 * i + 2] + margin, 0.0f);
+    if (first && dev_alloc(&c->d_circles, (size_t)kMaxCirclesSmem) != cudaSuccess) return fail(c, RA_ENOMEM, "alloc circles");
+    if (cuda_fail(c, cudaMemcpy(c->d_circles, h.data(), h.size() * sizeof(float4), cudaMemcpyHostToDevice), "copy circles"))
+      return RA_ECUDA;
+    p.n_circles = env->n_circles;
+    p.circles = c->d_circles;
+  }
+  if (cfg->risk == RA_RISK_COSTMAP) {
+    // risk-weighted bilinear coefficient table (models.cuh) around grid corner (jx-1/2, jy-1/2)
+    const int H = env->map_h, Wd = env->map_w;
+    const size_t n = (size_t)(H + 1) * (Wd + 1);
+    std::vector<float4> q(n);
+    auto at = [&](int iy, int ix) {
+      iy = iy < 0 ? 0 : (iy > H - 1 ? H - 1 : iy);
+      ix = ix < 0 ? 0 : (ix > Wd - 1 ? Wd - 1 : ix);
+      return (double)env->costmap[(size_t)iy * Wd + ix];
+    };
+    const double w = (double)cfg->risk_p[0];
+    for (int jy = 0; jy <= H; ++jy)
+      for (int jx = 0; jx <= Wd; ++jx) {
+        const double c00 = at(jy - 1, jx - 1), c01 = at(jy - 1, jx), c10 = at(jy, jx - 1), c11 = at(jy, jx);
+        q[(size_t)jy * (Wd + 1) + jx] = make_float4((float)(w * c00), (float)(w * (c01 - c00)), (float)(w * (c10 - c00)),
+                                                    (float)(w * (c11 - c10 - c01 + c00)));
+      }
+    if (first && dev_alloc(&c->d_costmap, n) != cudaSuccess) return fail(c, RA_ENOMEM, "alloc costmap");
+    if (cuda_fail(c, cudaMemcpy(c->d_costmap, q.data(), n * sizeof(float4), cudaMemcpyHostToDevice), "copy costmap"))
+      return RA_ECUDA;
+    p.quadmap = c->d_costmap;
+    p.map_h = env->map_h; p.map_w = env->map_w;
+    p.map_inv_res = (float)(1.0 / (double)env->map_res);
+    p.map_ox = env->map_ox; p.map_oy = env->map_oy;
+  }
+  return RA_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -249,43 +293,8 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
   c->noise_variant = cfg->noise_mode == RA_NOISE_MATERIALISED ? NOISE_MATERIALISED : cfg->noise_kind;
   c->rollout = pick_rollout(cfg->dyn, cfg->risk);
 
-  // environment copies
-  if (cfg->risk == RA_RISK_CIRCLES || cfg->nominal == RA_NOM_RACING) {
-    const float margin = cfg->risk == RA_RISK_CIRCLES ? cfg->risk_p[1] : 0.0f;   // (22) has no margin
-    p.n_circles = env->n_circles;
-    std::vector<float4> h((size_t)std::max(env->n_circles, 1));
-    for (int i = 0; i < env->n_circles; ++i)
-      h[i] = make_float4(env->circles[3 * i], env->circles[3 * i + 1], env->circles[3 * i + 2] + margin, 0.0f);
-    if (cuda_fail(c, dev_alloc(&c->d_circles, h.size()), "alloc circles")) return bail(RA_ENOMEM);
-    if (cudaMemcpy(c->d_circles, h.data(), h.size() * sizeof(float4), cudaMemcpyHostToDevice) != cudaSuccess)
-      return bail(RA_ECUDA);
-    p.circles = c->d_circles;
-  }
-  if (cfg->risk == RA_RISK_COSTMAP) {
-    // risk-weighted bilinear coefficient table (models.cuh) around grid corner (jx-1/2, jy-1/2)
-    const int H = env->map_h, Wd = env->map_w;
-    const size_t n = (size_t)(H + 1) * (Wd + 1);
-    std::vector<float4> q(n);
-    auto at = [&](int iy, int ix) {
-      iy = iy < 0 ? 0 : (iy > H - 1 ? H - 1 : iy);
-      ix = ix < 0 ? 0 : (ix > Wd - 1 ? Wd - 1 : ix);
-      return (double)env->costmap[(size_t)iy * Wd + ix];
-    };
-    const double w = (double)cfg->risk_p[0];
-    for (int jy = 0; jy <= H; ++jy)
-      for (int jx = 0; jx <= Wd; ++jx) {
-        const double c00 = at(jy - 1, jx - 1), c01 = at(jy - 1, jx), c10 = at(jy, jx - 1), c11 = at(jy, jx);
-        q[(size_t)jy * (Wd + 1) + jx] = make_float4((float)(w * c00), (float)(w * (c01 - c00)), (float)(w * (c10 - c00)),
-                                                    (float)(w * (c11 - c10 - c01 + c00)));
-      }
-    if (cuda_fail(c, dev_alloc(&c->d_costmap, n), "alloc costmap")) return bail(RA_ENOMEM);
-    if (cudaMemcpy(c->d_costmap, q.data(), n * sizeof(float4), cudaMemcpyHostToDevice) != cudaSuccess)
-      return bail(RA_ECUDA);
-    p.quadmap = c->d_costmap;
-    p.map_h = env->map_h; p.map_w = env->map_w;
-    p.map_inv_res = (float)(1.0 / (double)env->map_res);
-    p.map_ox = env->map_ox; p.map_oy = env->map_oy;
-  }
+  // environment copies (buffers sized once; ra_mppi_set_env refills them)
+  if (ra_status st_env = upload_env(c, env, true)) return bail(st_env);
   // scratch
   const size_t KT = (size_t)cfg->K * cfg->T;
   if (dev_alloc(&c->d_u_raw, KT) != cudaSuccess || dev_alloc(&c->d_ce, KT) != cudaSuccess ||
@@ -324,6 +333,24 @@ ra_status ra_mppi_destroy(ra_mppi_ctx* c) {
   cudaFree(c->d_S); cudaFree(c->d_cvar); cudaFree(c->d_pen); cudaFree(c->d_w_mat); cudaFree(c->d_loop);
   delete c;
   return RA_OK;
+}
+
+ra_status ra_mppi_set_env(ra_mppi_ctx* c, const ra_mppi_env* env) {
+  if (!c) return RA_EINVAL;
+  const ra_mppi_config* cfg = &c->cfg;
+  const bool uses_circles = cfg->risk == RA_RISK_CIRCLES || cfg->nominal == RA_NOM_RACING;
+  if (!env) return fail(c, RA_EINVAL, "null env");
+  if (uses_circles && (env->n_circles < 0 || (env->n_circles > 0 && !env->circles)))
+    return fail(c, RA_EINVAL, "circle costs need env->circles");
+  if (uses_circles && env->n_circles > kMaxCirclesSmem) return fail(c, RA_EUNSUPPORTED, "too many circles");
+  if (cfg->risk == RA_RISK_COSTMAP &&
+      (!env->costmap || env->map_h != c->p.map_h || env->map_w != c->p.map_w || !(env->map_res > 0.0f)))
+    return fail(c, RA_EINVAL, "costmap must keep the size it had at ra_mppi_create");
+  if (cudaSetDevice(cfg->device) != cudaSuccess) return fail(c, RA_ECUDA, "cudaSetDevice");
+  // earlier launches may still read the old copies; a captured graph holds the old sizes in its kernel arguments
+  RA_CUDA(c, cudaDeviceSynchronize());
+  if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+  return upload_env(c, env, false);
 }
 
 const char* ra_mppi_last_error(const ra_mppi_ctx* c) { return c ? c->err.c_str() : "null context"; }

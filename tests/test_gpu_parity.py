@@ -290,3 +290,45 @@ def test_baseline_mppi_mode_skips_the_noisy_rollouts(torch_cuda):
     g, r = check_rollout_parity(p, ctl, orc, iteration=3)
     assert (g["cvar"] > 0).any() and np.array_equal(g["S"], g["S_tilde"])
     assert _ctl(p.replace(A=1.0)).launches_per_step == 4
+
+
+def test_set_env_replaces_obstacles_and_costmap(torch_cuda):
+    """ra_mppi_set_env: a context whose environment was replaced equals a fresh context built on the new one."""
+    torch = torch_cuda
+    from paper_2209_12842_b200 import binding as B
+    # obstacles (different count, too)
+    p = _with_v(W.small(W.config1(), K=64, M=64, T=20))
+    moved = np.concatenate([p.circles[:20] + np.array([0.15, -0.1, 0.05]), [[10.0, 0.5, 0.4]]])
+    a, b = _ctl(p), _ctl(p.replace(circles=moved))
+    d_x0, d_v = a.tensor(p.x0), a.tensor(p.v)
+    before = a.rollout_costs(d_x0, d_v, 2)["S_tilde"].clone()
+    a.set_env(circles=moved)
+    ga, gb = a.rollout_costs(d_x0, d_v, 2), b.rollout_costs(d_x0, d_v, 2)
+    torch.cuda.synchronize()
+    for key in ("S", "cvar", "S_tilde", "L", "xT"):
+        assert torch.equal(ga[key], gb[key]), key
+    assert not torch.equal(before, ga["S_tilde"])
+    # the captured closed-loop graph is rebuilt after the change
+    xa, va, xb, vb = a.tensor(p.x0), a.tensor(p.v), b.tensor(p.x0), b.tensor(p.v)
+    a.closed_loop(xa, va, 0, 3, log=False, timing=False)
+    a.set_env(circles=moved)
+    xa.copy_(xb); va.copy_(vb)
+    a.closed_loop(xa, va, 0, 3, log=False, timing=False)
+    b.closed_loop(xb, vb, 0, 3, log=False, timing=False)
+    torch.cuda.synchronize()
+    assert torch.equal(xa, xb) and torch.equal(va, vb)
+    with pytest.raises(B.RaMppiError):
+        a.set_env(circles=np.zeros((2000, 3)))
+    a.close(); b.close()
+    # costmap: same size, new content and origin
+    p = _with_v(W.small(W.config3(), K=48, M=32, T=20))
+    cm = np.ascontiguousarray(p.costmap[::-1, ::-1])
+    a, b = _ctl(p), _ctl(p.replace(costmap=cm, map_ox=-0.3))
+    a.set_env(costmap=cm, map_ox=-0.3)
+    d_x0, d_v = a.tensor(p.x0), a.tensor(p.v)
+    ga, gb = a.rollout_costs(d_x0, d_v, 1), b.rollout_costs(d_x0, d_v, 1)
+    torch.cuda.synchronize()
+    assert torch.equal(ga["L"], gb["L"]) and torch.equal(ga["S_tilde"], gb["S_tilde"])
+    with pytest.raises(B.RaMppiError):
+        a.set_env(costmap=cm[:100, :100])
+    a.close(); b.close()
