@@ -32,6 +32,7 @@ struct ra_mppi_ctx {
   double* d_S = nullptr;
   float* d_cvar = nullptr;
   double* d_pen = nullptr;
+  double* d_split = nullptr;   // [kMaxUpdateSplits][2+2T] partials of the update's sample ranges
   float* d_w_mat = nullptr;
   LoopState* d_loop = nullptr;
   // closed-loop graph cache
@@ -49,6 +50,8 @@ struct ra_mppi_ctx {
 };
 
 namespace {
+
+constexpr int kMaxUpdateSplits = 8;
 
 ra_status fail(ra_mppi_ctx* c, ra_status s, const std::string& msg) {
   if (c) c->err = msg;
@@ -299,7 +302,7 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
   const size_t KT = (size_t)cfg->K * cfg->T;
   if (dev_alloc(&c->d_u_raw, KT) != cudaSuccess || dev_alloc(&c->d_ce, KT) != cudaSuccess ||
       dev_alloc(&c->d_S, (size_t)cfg->K) != cudaSuccess || dev_alloc(&c->d_cvar, (size_t)cfg->K) != cudaSuccess ||
-      dev_alloc(&c->d_pen, (size_t)cfg->K) != cudaSuccess || dev_alloc(&c->d_loop, 1) != cudaSuccess ||
+      dev_alloc(&c->d_pen, (size_t)cfg->K) != cudaSuccess || dev_alloc(&c->d_split, (size_t)kMaxUpdateSplits * (2 + 2 * cfg->T)) != cudaSuccess || dev_alloc(&c->d_loop, 1) != cudaSuccess ||
       dev_alloc(&c->d_stage, (size_t)(8 + 2 * cfg->T)) != cudaSuccess)
     return bail(RA_ENOMEM);
   p.u_raw = c->d_u_raw; p.ce = c->d_ce; p.S = c->d_S; p.cvar = c->d_cvar; p.pen = c->d_pen;
@@ -330,7 +333,7 @@ ra_status ra_mppi_destroy(ra_mppi_ctx* c) {
   if (c->side) cudaStreamDestroy(c->side);
   if (c->ev_k0) cudaEventDestroy(c->ev_k0);
   if (c->ev_k1) cudaEventDestroy(c->ev_k1);
-  cudaFree(c->d_S); cudaFree(c->d_cvar); cudaFree(c->d_pen); cudaFree(c->d_w_mat); cudaFree(c->d_loop);
+  cudaFree(c->d_S); cudaFree(c->d_cvar); cudaFree(c->d_pen); cudaFree(c->d_split); cudaFree(c->d_w_mat); cudaFree(c->d_loop);
   delete c;
   return RA_OK;
 }
@@ -427,10 +430,25 @@ ra_status enqueue_costs(ra_mppi_ctx* c, const Params& p, const float* d_x0, cons
   return RA_OK;
 }
 
-// Alg.1 l.31: weights (17) and update (4) from the context scratch.
+// Alg.1 l.31: weights (17) and update (4) from the context scratch.  T CTAs alone leave most SMs idle, so the
+// samples are cut into ranges (enough for one CTA per SM, at least 2048 samples each) that are combined like the
+// shards of the K-sharded step.
+int update_splits(const Params& p) {
+  const int by_sms = std::min(kMaxUpdateSplits, (148 + p.T - 1) / p.T);
+  return std::max(1, std::min(by_sms, p.K / 2048));
+}
+
 ra_status enqueue_update(ra_mppi_ctx* c, const Params& p, float* d_v_out, cudaStream_t s) {
-  weights_update_kernel<double><<<p.T, kUpdateThreads, 0, s>>>(
-      p, p.S, p.pen, p.u_raw, 1LL, (long long)p.K, d_v_out, nullptr, nullptr, nullptr);
+  const int splits = update_splits(p);
+  if (splits == 1) {
+    weights_update_kernel<double><<<p.T, kUpdateThreads, 0, s>>>(
+        p, p.S, p.pen, p.u_raw, 1LL, (long long)p.K, d_v_out, nullptr, nullptr, nullptr);
+  } else {
+    weights_update_kernel<double><<<dim3(p.T, splits), kUpdateThreads, 0, s>>>(
+        p, p.S, p.pen, p.u_raw, 1LL, (long long)p.K, nullptr, nullptr, nullptr, c->d_split);
+    RA_CUDA(c, cudaGetLastError());
+    combine_partials_kernel<<<1, 256, 0, s>>>(p, c->d_split, splits, d_v_out);
+  }
   RA_CUDA(c, cudaGetLastError());
   return RA_OK;
 }
@@ -577,8 +595,9 @@ ra_status ra_mppi_export_costs_f64(ra_mppi_ctx* c, double* d_S64, double* d_S_ti
 
 int32_t ra_mppi_launches_per_step(const ra_mppi_ctx* c) {
   if (!c) return 0;
-  if (c->cfg.A == 0.0f) return 3;   // baseline MPPI: sampling, nominal rollout, weights/update
-  return 4 + (c->cfg.noise_mode == RA_NOISE_MATERIALISED ? 1 : 0);   // + noisy rollouts (+ noise generator)
+  const int update = update_splits(c->p) > 1 ? 2 : 1;   // weights/update (+ combine of its sample ranges)
+  if (c->cfg.A == 0.0f) return 2 + update;   // baseline MPPI: sampling, nominal rollout, weights/update
+  return 3 + update + (c->cfg.noise_mode == RA_NOISE_MATERIALISED ? 1 : 0);   // + noisy rollouts (+ noise generator)
 }
 
 ra_status ra_mppi_philox(ra_mppi_ctx* c, const uint32_t* d_ctr, int32_t n, uint32_t* d_out, void* stream) {

@@ -24,9 +24,11 @@ __device__ __forceinline__ T block_reduce(T v, T* smem, Op op, T identity) {
 }
 
 // ---------------------------------------------------------------------------------------
-// A8 + A9.  One CTA per horizon step t.  Each CTA recomputes beta~ = min_k S~_k (K <= 65536
-// values from L2), then w~_k = exp(-(S~_k - beta~)/lambda), Z = sum w~, and
-// v+_t = clamp(sum_k w~_k u^k_t / Z)   (17) PAPER.md:134, (5) :55, (4) :51.
+// A8 + A9.  One CTA per (horizon step t, sample range blockIdx.y of gridDim.y).  Each CTA recomputes
+// beta~ = min_k S~_k over its range (values from L2), then w~_k = exp(-(S~_k - beta~)/lambda), Z = sum w~, and
+// v+_t = clamp(sum_k w~_k u^k_t / Z)   (17) PAPER.md:134, (5) :55, (4) :51.  With gridDim.y = 1 the CTA writes
+// v+ itself; with `partial` set it writes its range's {beta, Z, N_t} for combine_partials_kernel (the same
+// exchange the K-sharded step uses), which lets T * gridDim.y CTAs cover all SMs when T alone does not.
 // u is addressed as u[k*su_k + t*su_t] so both the internal [T][K] scratch and a caller's
 // [K][T] array work.  Reduction order is fixed => bitwise reproducible.
 // ---------------------------------------------------------------------------------------
@@ -46,12 +48,15 @@ weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S
   __shared__ ST red_s[32];
   __shared__ float red_f[96];
   const int t = blockIdx.x;
+  const int k_chunk = (p.K + gridDim.y - 1) / gridDim.y;
+  const int k_begin = blockIdx.y * k_chunk, k_end = min(p.K, k_begin + k_chunk);
+  if (partial) partial += (size_t)blockIdx.y * (2 + 2 * p.T);
   ST bmin = (ST)INFINITY;
-  for (int k = threadIdx.x; k < p.K; k += blockDim.x) bmin = min(bmin, s_tilde_at<ST>(S_tilde, pen, k));
+  for (int k = k_begin + threadIdx.x; k < k_end; k += blockDim.x) bmin = min(bmin, s_tilde_at<ST>(S_tilde, pen, k));
   const ST beta = block_reduce<ST>(bmin, red_s, [](ST a, ST b) { return a < b ? a : b; }, (ST)INFINITY);
 
   float Z = 0.0f, n0 = 0.0f, n1 = 0.0f;
-  for (int k = threadIdx.x; k < p.K; k += blockDim.x) {
+  for (int k = k_begin + threadIdx.x; k < k_end; k += blockDim.x) {
     const float w = exp2f((float)(s_tilde_at<ST>(S_tilde, pen, k) - beta) * p.neg_log2e_over_lambda);
     const float2 uk = __ldg(u + (long long)k * su_k + (long long)t * su_t);
     Z += w;
