@@ -40,7 +40,7 @@ _SINGLE_TRACK = 80 + 33 + 6 + 75
 ALGO_OPS = {"PAPER": _BICYCLE + 30, "PAPER-ST": _SINGLE_TRACK + 30, "C0": _BICYCLE, "C1": _BICYCLE, "C2": _SINGLE_TRACK,
             "C3": _BICYCLE + 18, "C4": _BICYCLE}
 # DRAM bytes (read + write) of one noisy_rollout_kernel launch, from the committed `ncu --set full` captures
-TRAFFIC_BYTES = {"C3": 13.42e6, "C2": 7.97e6}   # profiles/r1c_c3_c2_c4_pipe_model.md
+TRAFFIC_BYTES = {"C3": 13.29e6, "C2": 7.97e6}   # profiles/r1d_final_pipeline.md, profiles/r1c_c3_c2_c4_pipe_model.md
 ALU_PEAK_LANE_OPS = 148 * 128 * 1.965e9  # 148 SMs x 128 FP32 lanes x 1.965 GHz (B200_PROFILING.md nominal)
 
 
