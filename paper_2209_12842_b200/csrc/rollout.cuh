@@ -279,21 +279,23 @@ __device__ __forceinline__ void risk_accumulate(const Params& p, const float4* c
 // Dynamic shared memory: [n_circles] float4 obstacle records, [samples per CTA][T] float4 control
 // effects, then per warp R_total*32 keys.
 // ---------------------------------------------------------------------------------------
-#ifndef RA_MIN_CTAS_BICYCLE
-#define RA_MIN_CTAS_BICYCLE 3   // measured: 3 CTAs (<= 80 regs) beats 2 and 4-6 (throughput-, not latency-bound)
+// Resident CTAs per SM (register budget).  Measured on B200 (profiles/r1d): with four interleaved realisations
+// per lane (RC = 4) the costmap kernel (127 registers) and the single-track kernels (123; they spill at 80) are
+// faster with 2 CTAs/SM than with 3 CTAs of 80 registers (C3 0.458 -> 0.445 ms); the bicycle + circles kernels
+// (87 registers at most) and everything with RC <= 2 are faster with 3 (C1, C4, M = 256 sweep points).
+// Throughput-, not latency-bound: 4-6 CTAs/SM are slower everywhere.
+#ifndef RA_MIN_CTAS_RC4
+#define RA_MIN_CTAS_RC4 2
 #endif
-#ifndef RA_MIN_CTAS_SINGLE_TRACK
-#define RA_MIN_CTAS_SINGLE_TRACK 3
+#ifndef RA_MIN_CTAS_RC12
+#define RA_MIN_CTAS_RC12 3
 #endif
-#ifndef RA_MIN_CTAS_SINGLE_TRACK_RC4
-#define RA_MIN_CTAS_SINGLE_TRACK_RC4 2   // 4 x 6 state registers + carried Philox words spill at 80 registers
-#endif
-template <int DYN, int RC>
+template <int DYN, int RISK, int RC>
 constexpr int rollout_min_ctas() {
-  return DYN == DYN_BICYCLE ? RA_MIN_CTAS_BICYCLE : (RC == 4 ? RA_MIN_CTAS_SINGLE_TRACK_RC4 : RA_MIN_CTAS_SINGLE_TRACK);
+  return (RC == 4 && (DYN == DYN_SINGLE_TRACK || RISK == RISK_COSTMAP)) ? RA_MIN_CTAS_RC4 : RA_MIN_CTAS_RC12;
 }
 template <int DYN, int RISK, int NOISE, int RC, bool HALF>
-__global__ void __launch_bounds__(kRolloutThreads, rollout_min_ctas<DYN, RC>())
+__global__ void __launch_bounds__(kRolloutThreads, rollout_min_ctas<DYN, RISK, RC>())
 noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__ x0g,
                      float* __restrict__ L_out, float* __restrict__ xT_out) {
   constexpr int NX = StateDim<DYN>::value;
