@@ -8,7 +8,10 @@ MPPI (A = 0) with the same total number of sampled trajectories (l
 collisions the way PAPER.md:263 defines them (the state is inside an obstacle or outside the track) and laps.
 All control computation runs in libra_mppi.so; this module only post-processes the logged states
 (lap / collision bookkeeping is outside the hot path).  The track is the synthetic stand-in of workloads.py, so
-the numbers are not the paper's (its track layout is unpublished); they show the same qualitative trade-off.
+the numbers are not the paper's (its track layout, vehicle model and C_u are unpublished).  On this benign
+stand-in both controllers collide about once per 3000 iterations, so it does not separate their collision rates;
+what it does show is the price of the risk term: with the paper's A = 10 the RA-MPPI controller drives far more
+slowly until C_u is raised towards the typical CVaR (--C_u 8: lap time 6.6 s against the baseline's 4.1 s).
 """
 from __future__ import annotations
 
