@@ -115,3 +115,26 @@ def test_kernel_timing_hook(torch_cuda):
     ms = ctl.last_rollout_ms()
     assert 0.0 < ms < 100.0
     assert ctl.launches_per_step == 4   # sampling, nominal rollout, noisy rollouts, weights/update
+
+
+def test_step_is_capturable_in_a_caller_graph(torch_cuda):
+    """include/ra_mppi.h: ra_mppi_step only enqueues (no sync, no allocation), side-stream fork/join included,
+    so a caller can capture it in its own CUDA graph; replays reproduce the eager result bit for bit."""
+    torch = torch_cuda
+    p = W.small(W.config1(), K=300, M=64, T=30)
+    p = p.replace(v=W.random_mean_control(p, 1))
+    ctl = _ctl(p)
+    d_x0, v0 = ctl.tensor(p.x0), ctl.tensor(p.v)
+    v_eager = v0.clone()
+    ctl.step(d_x0, v_eager, 5)
+    torch.cuda.synchronize()
+    v_graph = v0.clone()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):                      # captures on torch's side stream; RaMppi uses the current stream
+        ctl.step(d_x0, v_graph, 5)
+    for _ in range(3):
+        v_graph.copy_(v0)
+        g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(v_graph, v_eager)
+    ctl.close()
