@@ -251,7 +251,12 @@ __device__ __forceinline__ float bilinear_weighted(const Params& p, const MapFra
   const float tx = gx - (jx - kFloorMagic), ty = gy - (jy - kFloorMagic);
   // all index arithmetic is mod 2^32; the sum is the absolute table index in [0, (H+1)(W+1))
   const uint32_t idx = __float_as_uint(jy) * (uint32_t)(p.map_w + 1) + __float_as_uint(jx) + f.base;
-  const float4 q = __ldg(p.quadmap + idx);
+  // byte address = table + 16 idx with two 32-bit adds on the ALU pipe (add.cc / addc) instead of a 64-bit
+  // IMAD.WIDE, which would hold the FMA pipe for four cycles (profiles/r1c); the table is < 4 GB (validated)
+  const float4* addr;
+  asm("{\n\t.reg .u32 lo, hi;\n\tmov.b64 {lo, hi}, %1;\n\tadd.cc.u32 lo, lo, %2;\n\taddc.u32 hi, hi, 0;\n\tmov.b64 %0, {lo, hi};\n\t}"
+      : "=l"(addr) : "l"(p.quadmap), "r"(idx << 4));
+  const float4 q = __ldg(addr);
   return fmaf(ty, fmaf(tx, q.w, q.z), fmaf(tx, q.y, q.x));
 }
 

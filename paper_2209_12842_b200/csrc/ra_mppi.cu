@@ -119,6 +119,7 @@ const char* validate(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_statu
     if (!env || !env->costmap || env->map_h < 1 || env->map_w < 1 || !(env->map_res > 0.0f))
       return "costmap risk needs env->costmap";
     if (env->map_h > (1 << 20) || env->map_w > (1 << 20)) return "costmap side above 2^20 cells";
+    if ((long long)(env->map_h + 1) * (env->map_w + 1) >= (1LL << 28)) return "costmap table above 4 GB";
   }
   if (cfg->risk == RA_RISK_LINEAR_STATE) {
     const int nx = cfg->dyn == RA_DYN_SINGLE_TRACK ? 6 : 4;
