@@ -55,7 +55,7 @@ def lib():
             f.restype = C.c_double
         L.orc_phi.argtypes = [C.POINTER(OrcProblem), _DP, _DP]
         L.orc_phi.restype = C.c_double
-        for f in (L.orc_racing_offset, L.orc_racing_arclength, L.orc_indicator_margin):
+        for f in (L.orc_racing_offset, L.orc_racing_arclength, L.orc_indicator_margin, L.orc_hinge_margin):
             f.argtypes = [C.POINTER(OrcProblem), C.c_double, C.c_double]
             f.restype = C.c_double
         L.orc_ellipse_offset.argtypes = [C.c_double] * 4
@@ -145,6 +145,9 @@ class Oracle:
 
     def indicator_margin(self, X, Y):
         return lib().orc_indicator_margin(C.byref(self.s), float(X), float(Y))
+
+    def hinge_margin(self, X, Y):
+        return lib().orc_hinge_margin(C.byref(self.s), float(X), float(Y))
 
     def l(self, x):
         x = np.ascontiguousarray(x, dtype=np.float64)

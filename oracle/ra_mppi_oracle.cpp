@@ -212,6 +212,18 @@ double orc_indicator_margin(const orc_problem* p, double X, double Y) {
   return m;
 }
 
+/* smallest |d_i - (r_i + margin)| over the obstacles at (X,Y): distance of the hinge risk cost (circle risk of
+ * orc_l) from the rim where it switches between exactly 0 and > 0.  A diagnostic for the parity tests ("exact
+ * zeros must match" wherever the state is not within rounding of a rim), not part of the method. */
+double orc_hinge_margin(const orc_problem* p, double X, double Y) {
+  double m = std::numeric_limits<double>::infinity();
+  for (int i = 0; i < p->n_circles; ++i) {
+    const double dx = X - p->circles[3 * i + 0], dy = Y - p->circles[3 * i + 1];
+    m = std::min(m, std::fabs(std::sqrt(dx * dx + dy * dy) - (p->circles[3 * i + 2] + p->risk_p[1])));
+  }
+  return m;
+}
+
 namespace {
 /* state part of the nominal running cost; q "can take an arbitrary form" P:45 */
 double q_state(const orc_problem* p, const double* x) {
@@ -397,6 +409,8 @@ void one_sample(const orc_problem* p, const double* x0_in, const double* v, uint
     for (int t = 0; t < T; ++t) {
       if (margin_out && p->risk == ORC_RISK_NOMINAL && p->nominal == ORC_NOM_RACING)
         mgm = std::min(mgm, orc_indicator_margin(p, xt[0], xt[1]));
+      if (margin_out && p->risk == ORC_RISK_CIRCLES)
+        mgm = std::min(mgm, orc_hinge_margin(p, xt[0], xt[1]));
       L += orc_l(p, xt);
       double w[6];
       orc_state_noise(p, (uint32_t)k, (uint32_t)m, (uint32_t)t, ORC_STREAM_W, iteration, w);

@@ -21,6 +21,9 @@
  *                          single-track, Euler order check against a separate RK4
  *   costs                - hand-computed points, bilinear reproduces affine maps
  *   weights/update       - sum to 1, shift invariance, lambda limits
+ *   control draw (O1a)   - std(u - v) = sigma_eps per component (distinct sigmas), mean 0,
+ *                          uncorrelated; u = v + sigma_eps (.) box_muller(r0, r1) of the EPS
+ *                          counter bit for bit through the free functions above
  *   iteration end-to-end - Gaussian closed-form CVaR through the whole rollout
  *                          path with the test-only linear risk; sigma_w=0, A=0,
  *                          M=1, K=1 special cases
@@ -88,6 +91,8 @@ double orc_racing_offset(const orc_problem* p, double X, double Y);
 double orc_racing_arclength(const orc_problem* p, double X, double Y);
 /* smallest |d_i - r_i| over the obstacles at (X,Y): distance of the indicator (22) from its jump */
 double orc_indicator_margin(const orc_problem* p, double X, double Y);
+/* smallest |d_i - (r_i + margin)|: distance of the hinge risk cost from its switch between exactly 0 and > 0 */
+double orc_hinge_margin(const orc_problem* p, double X, double Y);
 
 /* ---- CVaR -------------------------------------------------------------- */
 int32_t orc_tail_count(double alpha, int32_t M);
@@ -104,7 +109,8 @@ int orc_rollout_costs(const orc_problem* p, const double* x0, const double* v,
                       double* u /*[n,T,2]*/, double* S /*[n]*/, double* cvar /*[n]*/,
                       double* S_tilde /*[n]*/, double* L /*[n,M]*/, double* xT /*[n,M,nx]*/,
                       double* x_nom /*[n,nx] nominal terminal state*/,
-                      double* margin /*[n,M+1] min indicator margin: col 0 nominal, 1..M noisy; or NULL*/);
+                      double* margin /*[n,M+1] min over t of the indicator margin (racing costs; col 0 nominal, 1..M noisy)
+                                        or of the hinge margin (circle risk; cols 1..M, col 0 = inf); or NULL*/);
 /* O2-O3: weights and update from S_tilde[K] and u[K,T,2].                   */
 int orc_weights_update(const orc_problem* p, const double* S_tilde, const double* u,
                        double* v_plus /*[T,2]*/, double* w /*[K]*/, double* Z, double* beta);

@@ -170,3 +170,43 @@ def test_plant_and_shift():
     assert np.allclose(x, orc.dynamics(p.x0, [0.1, 1.0]) + orc.state_noise(0, 0, 0, 2, 7), atol=0)
     v = np.arange(10.0).reshape(5, 2)
     assert np.array_equal(O.shift(v), np.array([[2, 3], [4, 5], [6, 7], [8, 9], [8, 9.0]]))
+
+
+def test_eps_draw_scale_layout_and_moments():
+    """O1a, the control perturbation eps^k_t ~ N(0, Sigma_eps) (2c) PAPER.md:42, Alg.1 l.4/8 PAPER.md:179-186.
+
+    Pins (a) the scale: std(u - v) per component equals sigma_eps[i] with DISTINCT sigmas (a swap, a sigma^2 or a
+    missing factor fails), mean 0, components and steps uncorrelated; (b) the layout of DESIGN.md "RNG layout":
+    u[k,t] = v[t] + sigma_eps (.) box_muller(r0, r1) of philox(counter(k, m = 0, t, stream EPS, iteration)), written
+    with the oracle's FREE functions (each pinned on its own in test_oracle_rng.py), words (r2, r3) unused."""
+    it = 5
+    p = W.config0(K=8192, M=1, T=20).replace(seed=0x1234ABCD5678EF01)
+    p = p.replace(v=W.random_mean_control(p, 3))
+    assert p.sigma_eps[0] != p.sigma_eps[1] and np.abs(p.v).min() > 0
+    r = O.Oracle(p).rollout_costs(iteration=it, want_L=False, want_xT=False, n_threads=4)
+    d = r["u"] - p.v[None]                                   # [K, T, 2]
+    n = p.K * p.T
+    for i in range(2):
+        s = p.sigma_eps[i]
+        assert abs(d[..., i].mean()) < 4 * s / math.sqrt(n)
+        assert abs(d[..., i].std() / s - 1.0) < 4 / math.sqrt(2 * n)
+        assert abs(((d[..., i] / s) ** 4).mean() - 3.0) < 4 * math.sqrt(96 / n)
+    z = d / np.asarray(p.sigma_eps)
+    assert abs((z[..., 0] * z[..., 1]).mean()) < 4 / math.sqrt(n)              # the two components of one draw
+    assert abs((z[:, :-1, :] * z[:, 1:, :]).mean()) < 4 / math.sqrt(2 * n)     # consecutive steps
+    assert abs((z[:-1] * z[1:]).mean()) < 4 / math.sqrt(2 * n)                 # consecutive samples
+    # layout, bit for bit
+    key = (p.seed & 0xFFFFFFFF, p.seed >> 32)
+    rng = np.random.default_rng(0)
+    picks = [(0, 0), (p.K - 1, p.T - 1)] + [(int(k), int(t)) for k, t in
+                                            zip(rng.integers(0, p.K, 200), rng.integers(0, p.T, 200))]
+    for k, t in picks:
+        w = O.philox4x32_10(O.counter(k, 0, t, 1, 0, 0, it), key)
+        zz = O.box_muller(w[0], w[1])
+        for i in range(2):
+            assert r["u"][k, t, i] == p.v[t, i] + p.sigma_eps[i] * zz[i]
+        other = O.box_muller(w[2], w[3])                      # the unused half of the call is really unused
+        assert r["u"][k, t, 0] != p.v[t, 0] + p.sigma_eps[0] * other[0]
+    # a different iteration is a different draw; eta's zero-mean samples take the same eps without v
+    r0 = O.Oracle(p).rollout_costs(iteration=0, want_L=False, want_xT=False, n_threads=4)
+    assert not np.array_equal(r0["u"], r["u"])

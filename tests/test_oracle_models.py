@@ -141,6 +141,11 @@ def test_circle_risk_hand_points():
     # both circles contribute (sum over i): point between them with big radii
     p2 = p.replace(circles=np.array([[0.0, 0.0, 2.0], [3.0, 0.0, 2.0]]))
     assert O.Oracle(p2).l(st(1.5, 0.0)) == pytest.approx(2 * 1000 * 0.7**2)
+    # hinge margin (test diagnostic): distance to the nearest rim r + 0.2 where l switches between 0 and > 0
+    assert orc.hinge_margin(5.0, 6.0) == pytest.approx(0.3) and orc.hinge_margin(5.0, 5.5) == pytest.approx(0.2)
+    assert orc.hinge_margin(9.0, 5.4) == pytest.approx(0.1) and orc.hinge_margin(7.0, 5.0) == pytest.approx(1.3)
+    r = O.Oracle(W.small(W.config0(near_obstacle=True), K=6, M=5, T=8)).rollout_costs(want_margin=True)
+    assert r["margin"].shape == (6, 6) and np.isinf(r["margin"][:, 0]).all() and (r["margin"][:, 1:] > 0).all()
 
 
 def test_goal_cost_and_terminal():
