@@ -6,7 +6,8 @@ A "step" is one full controller iteration (ra_mppi_step: sample -> nominal + noi
 CVaR -> weights -> update) on the named BASELINE.json workload; default C3 = configs[3]
 (K=16384, M=128, T=50, costmap), the configuration BASELINE.json's target is quoted on.
 Prints ONE JSON line.  --impl reference times the fp64 oracle.
-The path does not shard (north_star: no second GPU): --gpus N runs N independent replicas.
+north_star fixes one GPU, so --gpus N runs N independent replicas (weak scaling); --sharded splits the K samples of
+ONE controller over the N ranks instead (strong scaling, one all-gather of 2+2T doubles per rank per step).
 """
 from __future__ import annotations
 

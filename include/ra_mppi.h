@@ -18,6 +18,8 @@
  *  - Errors are returned as ra_status; nothing throws, nothing calls exit().
  *    There is no CPU fallback: without an sm_100 device ra_mppi_create fails.
  *  - One context per stream; not re-entrant.
+ *  - Every entry point makes the context's device current for its own duration and restores the
+ *    caller's current device before returning.
  */
 #ifndef RA_MPPI_H
 #define RA_MPPI_H
@@ -163,7 +165,8 @@ ra_status ra_mppi_step_host(ra_mppi_ctx* ctx, const float* h_x0, float* h_v, uin
 
 /* Kernel timing for roofline accounting: when enabled, every step / rollout_costs records a CUDA
  * event pair around the fused rollout kernel on the launching stream.
- * ra_mppi_last_rollout_ms waits for that pair and returns its milliseconds in *h_ms (HOST).   */
+ * ra_mppi_last_rollout_ms waits for that pair and returns its milliseconds in *h_ms (HOST); RA_EINVAL when
+ * no rollout kernel has been timed (timing never enabled, only A = 0 steps, or only graph-captured steps).   */
 ra_status ra_mppi_enable_kernel_timing(ra_mppi_ctx* ctx, int32_t enable);
 ra_status ra_mppi_last_rollout_ms(ra_mppi_ctx* ctx, float* h_ms);
 
@@ -187,6 +190,14 @@ ra_status ra_mppi_measure_pipe_peaks(int32_t device, float* h_tera_lane_ops);
  *  the same + 2 FFMA; the same + 4 FFMA}.  The last three show that FFMAs do not overlap the wide multiply.
  * Runs eight short microbenchmark kernels on the NULL stream and synchronises.                           */
 ra_status ra_mppi_measure_pipe_model(int32_t device, float* h_cycles);
+
+/* The two integer decisions ra_mppi_create derives from fp32 parameters, without touching a device (host only):
+ * *h_k_tail = ceil((1-alpha) M) clamped to [1, M], the CVaR tail size of Alg.1 l.25-26 ((12) :107);
+ * *h_K0 = ceil((1-eta) K_total), the number of samples that carry the mean control (Alg.1 l.7-10).
+ * alpha and eta arrive as fp32, so both counts are taken with a guard of 2^-23 n against their representation
+ * error (alpha = 0.7f with M = 10 counts 3, eta = 0.7f with K = 1000 counts 300).  Either pointer may be NULL.
+ * RA_EINVAL: null cfg, struct_size mismatch, M or K <= 0, alpha outside (0,1), eta outside [0,1).            */
+ra_status ra_mppi_query_counts(const ra_mppi_config* cfg, int32_t* h_k_tail, int32_t* h_K0);
 
 /* Number of kernels one ra_mppi_step launches (for launch accounting).                   */
 int32_t ra_mppi_launches_per_step(const ra_mppi_ctx* ctx);

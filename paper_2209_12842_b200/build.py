@@ -42,7 +42,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     os.makedirs(OBJ, exist_ok=True)
     extra = ["-Xptxas", "-v"] if verbose else []
-    extra += os.environ.get("RA_MPPI_NVCC_EXTRA", "").split()  # tuning experiments only (e.g. -DRA_FORCE_RC=2)
 
     def compile_one(job):
         src, obj, defs = job

@@ -4,9 +4,26 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <atomic>
+
 #include "ra_params.cuh"
 
 namespace ra {
+
+// cudaFuncSetAttribute acts on the CURRENT device's copy of a kernel, so "already set" is remembered per
+// (kernel, device): `slot` is a zero-initialised static array of kMaxDevices entries owned by the call site
+// (one per kernel instantiation) holding value + 1.  Ordinals past the table are simply set every time.
+// A racing second thread at worst repeats the call.
+constexpr int kMaxDevices = 64;
+template <typename Kernel>
+inline cudaError_t set_func_attr_once(std::atomic<int>* slot, int device, Kernel kernel, cudaFuncAttribute attr,
+                                      int value) {
+  const bool cached = device >= 0 && device < kMaxDevices;
+  if (cached && slot[device].load(std::memory_order_relaxed) == value + 1) return cudaSuccess;
+  const cudaError_t e = cudaFuncSetAttribute(kernel, attr, value);
+  if (e == cudaSuccess && cached) slot[device].store(value + 1, std::memory_order_relaxed);
+  return e;
+}
 
 // noise: NOISE_GAUSSIAN / NOISE_UNIFORM / NOISE_JUMP / 3 (materialised); rc in {1,2,4};
 // half: two samples per warp (M <= 16, rc must be 1).

@@ -179,7 +179,7 @@ __device__ __forceinline__ float nominal_cost(const Params& p, float Xabs, float
     for (int i = 0; i < p.n_circles; ++i) {
       const float4 c = __ldg(p.circles + i);
       const float dx = Xabs - c.x, dy = Yabs - c.y;
-      if (fmaf(dx, dx, dy * dy) < c.z * c.z) q += p.nom_p[5];
+      if (fmaf(dx, dx, dy * dy) < c.w * c.w) q += p.nom_p[5];   // bare radius: (22) has no margin
     }
     return q;
   } else {

@@ -23,6 +23,7 @@ struct ra_mppi_ctx {
   int rc = 1;          // realisations interleaved per lane in the rollout kernel
   bool half = false;   // two samples per warp
   int noise_variant = 0;
+  int n_sm = 0;        // multiprocessors of cfg.device (grid sizing of the small kernels)
   RolloutLaunchFn rollout = nullptr;
   // device allocations owned by the context
   float4* d_circles = nullptr;
@@ -39,6 +40,7 @@ struct ra_mppi_ctx {
   // host-buffer staging (ra_mppi_step_host) and optional kernel timing
   float* d_stage = nullptr;  // [nx + 2T]
   bool timing = false;
+  bool timed = false;  // ev_k0 / ev_k1 hold a rollout-kernel interval recorded outside a stream capture
   cudaEvent_t ev_k0 = nullptr, ev_k1 = nullptr;
   // the nominal rollout (A2) runs beside the noisy rollouts (A3-A7) on this stream, forked from and
   // joined back into the caller's stream with the two events (captured as parallel graph branches)
@@ -72,12 +74,39 @@ ra_status cuda_fail(ra_mppi_ctx* c, cudaError_t e, const char* what) {
 
 bool finite_nonneg(float x) { return std::isfinite(x) && x >= 0.0f; }
 
-// ceil((1-alpha) M) (G11), clamped to [1, M].  alpha arrives as fp32, so the guard
-// against representation error is 1e-6 M (0.7f -> (1-alpha) 10 = 3.0000001 must count 3).
+// alpha and eta arrive as fp32: the decimal the caller meant lies within one fp32 ulp of a value below 1,
+// i.e. within 2^-23 of the number received, so (1 - x) n is known to 2^-23 n.  The guard against that
+// representation error is therefore 2^-23 n (0.7f -> (1-alpha) 10 = 3.0000001 must count 3); the fp64 oracle
+// uses 1e-9.  The two sides agree unless the true (1 - x) n lies within 2^-23 n above an integer.
+constexpr double kFp32Ulp = 1.1920928955078125e-07;   // 2^-23
+
+// k_tail = ceil((1-alpha) M) (G11), clamped to [1, M].
 int tail_count(double alpha, int M) {
-  int k = (int)std::ceil((1.0 - alpha) * (double)M - 1e-6 * (double)M);
+  int k = (int)std::ceil((1.0 - alpha) * (double)M - kFp32Ulp * (double)M);
   return k < 1 ? 1 : (k > M ? M : k);
 }
+
+// K0 = ceil((1-eta) K): samples with global index below K0 carry the mean control (Alg.1 l.7-10).
+int mean_count(double eta, int K_total) {
+  int k = (int)std::ceil((1.0 - eta) * (double)K_total - kFp32Ulp * (double)K_total);
+  return k < 0 ? 0 : (k > K_total ? K_total : k);
+}
+
+// Makes cfg.device current for the duration of an entry point and restores the caller's device afterwards.
+struct DeviceGuard {
+  int prev = -1;
+  bool ok = true;
+  explicit DeviceGuard(int device) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { prev = -1; ok = false; return; }
+    if (prev != device) ok = cudaSetDevice(device) == cudaSuccess; else prev = -1;
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+  DeviceGuard(const DeviceGuard&) = delete;
+  DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+#define RA_ON_DEVICE(ctx)                                                      \
+  DeviceGuard device_guard__((ctx)->cfg.device);                               \
+  if (!device_guard__.ok) return fail((ctx), RA_ECUDA, "cudaSetDevice failed")
 
 const char* validate(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_status* st) {
   *st = RA_EINVAL;
@@ -127,6 +156,8 @@ const char* validate(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_statu
   }
   if (cfg->noise_kind == RA_NOISE_JUMP && !(cfg->noise_p[0] >= 0.0f && cfg->noise_p[0] <= 1.0f))
     return "jump probability must be in [0,1]";
+  if (cfg->risk == RA_RISK_CIRCLES && (!finite_nonneg(cfg->risk_p[1]) || !std::isfinite(cfg->risk_p[0])))
+    return "circle risk needs a finite weight and a finite margin >= 0";
   *st = RA_EUNSUPPORTED;
   if (cfg->M > RA_MAX_M) return "M above RA_MAX_M";
   if (cfg->T > RA_MAX_T) return "T above RA_MAX_T";
@@ -160,10 +191,13 @@ ra_status upload_env(ra_mppi_ctx* c, const ra_mppi_env* env, bool first) {
   const ra_mppi_config* cfg = &c->cfg;
   Params& p = c->p;
   if (cfg->risk == RA_RISK_CIRCLES || cfg->nominal == RA_NOM_RACING) {
-    const float margin = cfg->risk == RA_RISK_CIRCLES ? cfg->risk_p[1] : 0.0f;   // (22) has no margin
+    // (cx, cy, r + margin, r): the hinge risk cost (BASELINE configs) tests against r + margin, the indicator cost (22)
+    // of the racing nominal cost against the bare radius r (it has no margin), also when both are in use
+    const float margin = cfg->risk == RA_RISK_CIRCLES ? cfg->risk_p[1] : 0.0f;
     std::vector<float4> h((size_t)std::max(env->n_circles, 1));
     for (int i = 0; i < env->n_circles; ++i)
-      h[i] = make_float4(env->circles[3 * i], env->circles[3 * i + 1], env->circles[3 * i + 2] + margin, 0.0f);
+      h[i] = make_float4(env->circles[3 * i], env->circles[3 * i + 1], env->circles[3 * i + 2] + margin,
+                         env->circles[3 * i + 2]);
     if (first && dev_alloc(&c->d_circles, (size_t)kMaxCirclesSmem) != cudaSuccess) return fail(c, RA_ENOMEM, "alloc circles");
     if (cuda_fail(c, cudaMemcpy(c->d_circles, h.data(), h.size() * sizeof(float4), cudaMemcpyHostToDevice), "copy circles"))
       return RA_ECUDA;
@@ -226,13 +260,16 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
   if (!c) return RA_ENOMEM;
   c->cfg = *cfg;
   auto bail = [&](ra_status s) { ra_mppi_destroy(c); return s; };
-  if (cudaSetDevice(cfg->device) != cudaSuccess) return bail(RA_ECUDA);
+  DeviceGuard on_device(cfg->device);   // the caller's current device is restored on return
+  if (!on_device.ok) return bail(RA_ECUDA);
+  c->n_sm = prop.multiProcessorCount;
 
   Params& p = c->p;
   p.K = cfg->K; p.M = cfg->M; p.T = cfg->T;
   const int K_total = cfg->K_total ? cfg->K_total : cfg->K;
   p.k_off = cfg->k_offset;
-  p.K0 = (int)std::ceil((1.0 - (double)cfg->eta) * (double)K_total - 1e-9);   // on the global index
+  p.K0 = mean_count((double)cfg->eta, K_total);   // on the global index
+  p.device = cfg->device;
   p.k_tail = tail_count((double)cfg->alpha, cfg->M);
   c->half = cfg->M <= 16;
   p.G = c->half ? 16 : 32;
@@ -249,12 +286,6 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
     const int groups = (p.R_total + c->rc - 1) / c->rc;
     while (p.wps < 8 && p.wps < groups) p.wps *= 2;
   }
-#ifdef RA_FORCE_RC  // tuning experiments only
-  if (!c->half) c->rc = RA_FORCE_RC;
-#endif
-#ifdef RA_FORCE_WPS
-  if (!c->half) p.wps = RA_FORCE_WPS;
-#endif
   {
     // shared-memory carveout (percent of the 228 KB unified L1) that holds three rollout CTAs; the nominal-rollout
     // kernel asks for the same split so both kernels can share an SM
@@ -325,7 +356,7 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
 
 ra_status ra_mppi_destroy(ra_mppi_ctx* c) {
   if (!c) return RA_OK;
-  cudaSetDevice(c->cfg.device);
+  DeviceGuard on_device(c->cfg.device);
   if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
   cudaFree(c->d_circles); cudaFree(c->d_costmap); cudaFree(c->d_u_raw); cudaFree(c->d_ce);
   cudaFree(c->d_stage);
@@ -350,7 +381,7 @@ ra_status ra_mppi_set_env(ra_mppi_ctx* c, const ra_mppi_env* env) {
   if (cfg->risk == RA_RISK_COSTMAP &&
       (!env->costmap || env->map_h != c->p.map_h || env->map_w != c->p.map_w || !(env->map_res > 0.0f)))
     return fail(c, RA_EINVAL, "costmap must keep the size it had at ra_mppi_create");
-  if (cudaSetDevice(cfg->device) != cudaSuccess) return fail(c, RA_ECUDA, "cudaSetDevice");
+  RA_ON_DEVICE(c);
   // earlier launches may still read the old copies; a captured graph holds the old sizes in its kernel arguments
   RA_CUDA(c, cudaDeviceSynchronize());
   if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
@@ -358,6 +389,14 @@ ra_status ra_mppi_set_env(ra_mppi_ctx* c, const ra_mppi_env* env) {
 }
 
 const char* ra_mppi_last_error(const ra_mppi_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+ra_status ra_mppi_query_counts(const ra_mppi_config* cfg, int32_t* h_k_tail, int32_t* h_K0) {
+  if (!cfg || cfg->struct_size != sizeof(ra_mppi_config) || cfg->M <= 0 || cfg->K <= 0) return RA_EINVAL;
+  if (!(cfg->alpha > 0.0f && cfg->alpha < 1.0f) || !(cfg->eta >= 0.0f && cfg->eta < 1.0f)) return RA_EINVAL;
+  if (h_k_tail) *h_k_tail = tail_count((double)cfg->alpha, cfg->M);
+  if (h_K0) *h_K0 = mean_count((double)cfg->eta, cfg->K_total ? cfg->K_total : cfg->K);
+  return RA_OK;
+}
 
 
 }  // extern "C"
@@ -377,13 +416,10 @@ cudaError_t launch_nominal(const ra_mppi_ctx* c, const Params& p, const float* d
   const int dyn = c->cfg.dyn, nom = c->cfg.nominal;
 #define RA_NOMK(D, N)                                                                                          \
   do {                                                                                                         \
-    static int carveout_set = -1;   /* same L1 / shared-memory split as the rollout kernel (rollout_inst.cu) */ \
-    if (carveout_set != p.carveout) {                                                                          \
-      const cudaError_t e = cudaFuncSetAttribute(nominal_kernel<D, N>,                                         \
-                                                 cudaFuncAttributePreferredSharedMemoryCarveout, p.carveout);  \
-      if (e != cudaSuccess) return e;                                                                          \
-      carveout_set = p.carveout;                                                                               \
-    }                                                                                                          \
+    static std::atomic<int> carveout_set[kMaxDevices];   /* same L1 / shared-memory split as the rollout kernel */ \
+    if (const cudaError_t e = set_func_attr_once(carveout_set, p.device, nominal_kernel<D, N>,                  \
+                                                 cudaFuncAttributePreferredSharedMemoryCarveout, p.carveout))  \
+      return e;                                                                                                \
     nominal_kernel<D, N><<<grid, kNominalThreads, 0, s>>>(p, d_x0, d_v);                                       \
   } while (0)
   if (dyn == 0) { if (nom == 0) RA_NOMK(0, 0); else if (nom == 1) RA_NOMK(0, 1); else RA_NOMK(0, 2); }
@@ -395,7 +431,7 @@ cudaError_t launch_nominal(const ra_mppi_ctx* c, const Params& p, const float* d
 template <int NX>
 cudaError_t launch_materialise(const ra_mppi_ctx* c, const Params& p, cudaStream_t s) {
   const long long n = (long long)p.K * p.T * p.M_pad;
-  const int grid = (int)std::min<long long>((n + 255) / 256, 148LL * 16);
+  const int grid = (int)std::min<long long>((n + 255) / 256, (long long)c->n_sm * 16);
   switch (c->cfg.noise_kind) {
     case RA_NOISE_GAUSSIAN: materialise_noise_kernel<NX, NOISE_GAUSSIAN><<<grid, 256, 0, s>>>(p, c->d_w_mat); break;
     case RA_NOISE_UNIFORM: materialise_noise_kernel<NX, NOISE_UNIFORM><<<grid, 256, 0, s>>>(p, c->d_w_mat); break;
@@ -424,9 +460,13 @@ ra_status enqueue_costs(ra_mppi_ctx* c, const Params& p, const float* d_x0, cons
   RA_CUDA(c, cudaStreamWaitEvent(c->side, c->ev_fork, 0));
   RA_CUDA(c, launch_nominal(c, p, d_x0, d_v, c->side));
   RA_CUDA(c, cudaEventRecord(c->ev_join, c->side));
-  if (c->timing) RA_CUDA(c, cudaEventRecord(c->ev_k0, s));
+  // the timing pair is recorded on live streams only: an event recorded during capture has no elapsed time
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  if (c->timing) RA_CUDA(c, cudaStreamIsCapturing(s, &cap));
+  const bool time_it = c->timing && cap == cudaStreamCaptureStatusNone;
+  if (time_it) RA_CUDA(c, cudaEventRecord(c->ev_k0, s));
   RA_CUDA(c, c->rollout(p, c->noise_variant, c->rc, c->half, d_x0, d_L, d_xT, s));
-  if (c->timing) RA_CUDA(c, cudaEventRecord(c->ev_k1, s));
+  if (time_it) { RA_CUDA(c, cudaEventRecord(c->ev_k1, s)); c->timed = true; }
   RA_CUDA(c, cudaStreamWaitEvent(s, c->ev_join, 0));   // join
   return RA_OK;
 }
@@ -434,13 +474,14 @@ ra_status enqueue_costs(ra_mppi_ctx* c, const Params& p, const float* d_x0, cons
 // Alg.1 l.31: weights (17) and update (4) from the context scratch.  T CTAs alone leave most SMs idle, so the
 // samples are cut into ranges (enough for one CTA per SM, at least 2048 samples each) that are combined like the
 // shards of the K-sharded step.
-int update_splits(const Params& p) {
-  const int by_sms = std::min(kMaxUpdateSplits, (148 + p.T - 1) / p.T);
+int update_splits(const ra_mppi_ctx* c) {
+  const Params& p = c->p;
+  const int by_sms = std::min(kMaxUpdateSplits, (c->n_sm + p.T - 1) / p.T);
   return std::max(1, std::min(by_sms, p.K / 2048));
 }
 
 ra_status enqueue_update(ra_mppi_ctx* c, const Params& p, float* d_v_out, cudaStream_t s) {
-  const int splits = update_splits(p);
+  const int splits = update_splits(c);
   if (splits == 1) {
     weights_update_kernel<double><<<p.T, kUpdateThreads, 0, s>>>(
         p, p.S, p.pen, p.u_raw, 1LL, (long long)p.K, d_v_out, nullptr, nullptr, nullptr);
@@ -486,6 +527,7 @@ extern "C" {
 ra_status ra_mppi_step(ra_mppi_ctx* c, const float* d_x0, float* d_v, uint64_t iteration, void* stream) {
   if (!c) return RA_EINVAL;
   if (!d_x0 || !d_v) return fail(c, RA_EINVAL, "null device pointer");
+  RA_ON_DEVICE(c);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const Params p = with_iteration(c, iteration);
   if (ra_status st = enqueue_costs(c, p, d_x0, d_v, nullptr, nullptr, s, false)) return st;
@@ -496,6 +538,7 @@ ra_status ra_mppi_step_partial(ra_mppi_ctx* c, const float* d_x0, const float* d
                                double* d_partial, void* stream) {
   if (!c) return RA_EINVAL;
   if (!d_x0 || !d_v || !d_partial) return fail(c, RA_EINVAL, "null device pointer");
+  RA_ON_DEVICE(c);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const Params p = with_iteration(c, iteration);
   if (ra_status st = enqueue_costs(c, p, d_x0, d_v, nullptr, nullptr, s, false)) return st;
@@ -506,6 +549,7 @@ ra_status ra_mppi_combine_partials(ra_mppi_ctx* c, const double* d_partials, int
                                    void* stream) {
   if (!c) return RA_EINVAL;
   if (!d_partials || !d_v_plus || n_parts < 1) return fail(c, RA_EINVAL, "bad arguments");
+  RA_ON_DEVICE(c);
   combine_partials_kernel<<<1, 256, 0, static_cast<cudaStream_t>(stream)>>>(c->p, d_partials, n_parts, d_v_plus);
   RA_CUDA(c, cudaGetLastError());
   return RA_OK;
@@ -516,6 +560,7 @@ ra_status ra_mppi_rollout_costs(ra_mppi_ctx* c, const float* d_x0, const float* 
                                 float* d_u, void* stream) {
   if (!c) return RA_EINVAL;
   if (!d_x0 || !d_v) return fail(c, RA_EINVAL, "null device pointer");
+  RA_ON_DEVICE(c);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const Params p = with_iteration(c, iteration);
   if (ra_status st = enqueue_costs(c, p, d_x0, d_v, d_L, d_xT, s, true)) return st;
@@ -524,7 +569,7 @@ ra_status ra_mppi_rollout_costs(ra_mppi_ctx* c, const float* d_x0, const float* 
     RA_CUDA(c, cudaGetLastError());
   }
   if (d_u) {
-    export_u_kernel<<<148 * 4, 256, 0, s>>>(p, reinterpret_cast<float2*>(d_u));
+    export_u_kernel<<<c->n_sm * 4, 256, 0, s>>>(p, reinterpret_cast<float2*>(d_u));
     RA_CUDA(c, cudaGetLastError());
   }
   return RA_OK;
@@ -534,6 +579,7 @@ ra_status ra_mppi_weights_update(ra_mppi_ctx* c, const float* d_S_tilde, const f
                                  float* d_w, float* d_stats, void* stream) {
   if (!c) return RA_EINVAL;
   if (!d_S_tilde || !d_u || !d_v_plus) return fail(c, RA_EINVAL, "null device pointer");
+  RA_ON_DEVICE(c);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const Params p = with_iteration(c, 0);
   weights_update_kernel<float><<<p.T, kUpdateThreads, 0, s>>>(
@@ -546,6 +592,7 @@ ra_status ra_mppi_plant_shift(ra_mppi_ctx* c, float* d_x0, float* d_v, float* d_
                               void* stream) {
   if (!c) return RA_EINVAL;
   if (!d_x0 || !d_v) return fail(c, RA_EINVAL, "null device pointer");
+  RA_ON_DEVICE(c);
   const Params p = with_iteration(c, iteration);
   RA_CUDA(c, launch_plant(c, p, d_x0, d_v, d_u_applied, nullptr, nullptr, static_cast<cudaStream_t>(stream)));
   return RA_OK;
@@ -554,6 +601,7 @@ ra_status ra_mppi_plant_shift(ra_mppi_ctx* c, float* d_x0, float* d_v, float* d_
 ra_status ra_mppi_step_host(ra_mppi_ctx* c, const float* h_x0, float* h_v, uint64_t iteration, void* stream) {
   if (!c) return RA_EINVAL;
   if (!h_x0 || !h_v) return fail(c, RA_EINVAL, "null host pointer");
+  RA_ON_DEVICE(c);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   float* d_x0 = c->d_stage;
   float* d_v = c->d_stage + 8;
@@ -568,6 +616,7 @@ ra_status ra_mppi_step_host(ra_mppi_ctx* c, const float* h_x0, float* h_v, uint6
 
 ra_status ra_mppi_enable_kernel_timing(ra_mppi_ctx* c, int32_t enable) {
   if (!c) return RA_EINVAL;
+  RA_ON_DEVICE(c);
   if (enable && !c->ev_k0) {
     RA_CUDA(c, cudaEventCreate(&c->ev_k0));
     RA_CUDA(c, cudaEventCreate(&c->ev_k1));
@@ -579,6 +628,10 @@ ra_status ra_mppi_enable_kernel_timing(ra_mppi_ctx* c, int32_t enable) {
 ra_status ra_mppi_last_rollout_ms(ra_mppi_ctx* c, float* h_ms) {
   if (!c) return RA_EINVAL;
   if (!h_ms || !c->ev_k0) return fail(c, RA_EINVAL, "kernel timing was never enabled");
+  if (!c->timed)
+    return fail(c, RA_EINVAL, "no rollout kernel has been timed: A = 0 steps launch none, and steps captured into a CUDA "
+                              "graph record no timing events");
+  RA_ON_DEVICE(c);
   RA_CUDA(c, cudaEventSynchronize(c->ev_k1));
   RA_CUDA(c, cudaEventElapsedTime(h_ms, c->ev_k0, c->ev_k1));
   return RA_OK;
@@ -586,6 +639,7 @@ ra_status ra_mppi_last_rollout_ms(ra_mppi_ctx* c, float* h_ms) {
 
 ra_status ra_mppi_export_costs_f64(ra_mppi_ctx* c, double* d_S64, double* d_S_tilde64, void* stream) {
   if (!c) return RA_EINVAL;
+  RA_ON_DEVICE(c);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   if (d_S64 || d_S_tilde64) {
     export_costs_f64_kernel<<<(c->p.K + 255) / 256, 256, 0, s>>>(c->p, d_S64, d_S_tilde64);
@@ -596,7 +650,7 @@ ra_status ra_mppi_export_costs_f64(ra_mppi_ctx* c, double* d_S64, double* d_S_ti
 
 int32_t ra_mppi_launches_per_step(const ra_mppi_ctx* c) {
   if (!c) return 0;
-  const int update = update_splits(c->p) > 1 ? 2 : 1;   // weights/update (+ combine of its sample ranges)
+  const int update = update_splits(c) > 1 ? 2 : 1;   // weights/update (+ combine of its sample ranges)
   if (c->cfg.A == 0.0f) return 2 + update;   // baseline MPPI: sampling, nominal rollout, weights/update
   return 3 + update + (c->cfg.noise_mode == RA_NOISE_MATERIALISED ? 1 : 0);   // + noisy rollouts (+ noise generator)
 }
@@ -605,6 +659,7 @@ ra_status ra_mppi_philox(ra_mppi_ctx* c, const uint32_t* d_ctr, int32_t n, uint3
   if (!c) return RA_EINVAL;
   if (!d_ctr || !d_out || n < 0) return fail(c, RA_EINVAL, "bad arguments");
   if (n == 0) return RA_OK;
+  RA_ON_DEVICE(c);
   philox_probe_kernel<<<(n + 255) / 256, 256, 0, static_cast<cudaStream_t>(stream)>>>(
       c->p, reinterpret_cast<const uint4*>(d_ctr), n, reinterpret_cast<uint4*>(d_out));
   RA_CUDA(c, cudaGetLastError());
@@ -616,6 +671,7 @@ ra_status ra_mppi_state_noise(ra_mppi_ctx* c, const int32_t* d_kmt, int32_t n, u
   if (!c) return RA_EINVAL;
   if (!d_kmt || !d_w || n < 0) return fail(c, RA_EINVAL, "bad arguments");
   if (n == 0) return RA_OK;
+  RA_ON_DEVICE(c);
   const Params p = with_iteration(c, iteration);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const int grid = (n + 255) / 256, nk = c->cfg.noise_kind;
@@ -643,6 +699,7 @@ ra_status ra_mppi_closed_loop(ra_mppi_ctx* c, float* d_x0, float* d_v, uint64_t 
   if (!c) return RA_EINVAL;
   if (!d_x0 || !d_v || n_iter < 0) return fail(c, RA_EINVAL, "bad arguments");
   if (n_iter == 0) return RA_OK;
+  RA_ON_DEVICE(c);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   cudaStream_t own = nullptr;
   if (s == nullptr) {  // the legacy default stream cannot be captured

@@ -23,6 +23,7 @@ struct Params {
   int wps;      // warps per control sample in the rollout kernel (1, 2, 4 or 8)
   int nx;
   int carveout; // host only: preferred shared-memory carveout (percent) of the two concurrent rollout kernels
+  int device;   // host only: CUDA device ordinal of the context (per-device kernel attributes)
   float dt;
   float dyn_p[8];
   float dyn_q[2];   // single-track: 1/m, 1/Iz
@@ -38,7 +39,7 @@ struct Params {
   float noise_p[4];
   uint32_t rk[20];  // the ten Philox round keys (k0_r, k1_r), key = seed
   // environment (device copies owned by the context)
-  const float4* circles;  // [n] absolute (cx, cy, r + margin, unused)
+  const float4* circles;  // [n] absolute (cx, cy, r + risk margin, r)
   int n_circles;
   const float4* quadmap;  // [(map_h+1)][(map_w+1)] texel quads, clamp-to-edge baked in
   int map_h, map_w;

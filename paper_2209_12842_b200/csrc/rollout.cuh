@@ -385,7 +385,10 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
         float a[RC][NX];
 #pragma unroll
         for (int r = 0; r < RC; ++r) {
-          const float* wp = p.w_mat + (((size_t)k * p.T + t) * NX) * p.M_pad + m[r];
+          // a slot past R_total (RC does not divide the slot count) has m >= M_pad: clamp it into the row so
+          // the load stays inside w_mat; the slot's results are discarded below
+          const uint32_t mc = min(m[r], (uint32_t)(p.M_pad - 1));
+          const float* wp = p.w_mat + (((size_t)k * p.T + t) * NX) * p.M_pad + mc;
 #pragma unroll
           for (int i = 0; i < NX; ++i) a[r][i] = __ldg(wp + (size_t)i * p.M_pad);
         }

@@ -22,18 +22,15 @@ cudaError_t launch(const Params& p, const float* d_x0, float* d_L, float* d_xT, 
                       (size_t)ce_slots * p.T * sizeof(float4) + (size_t)kRolloutWarps * p.R_total * 32 * sizeof(uint32_t);
   auto kernel = noisy_rollout_kernel<RA_INST_DYN, RA_INST_RISK, NOISE, RC, HALF>;
   if (smem > 48 * 1024) {   // worst case (1024 circles, T = 128, M = 512) is 65 KB
-    static const cudaError_t attr =
-        cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 80 * 1024);
-    if (attr != cudaSuccess) return attr;
+    static std::atomic<int> smem_set[kMaxDevices];
+    const cudaError_t e = set_func_attr_once(smem_set, p.device, kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 80 * 1024);
+    if (e != cudaSuccess) return e;
   }
   // the same L1 / shared-memory split as the nominal-rollout kernel that runs beside this one: CTAs of kernels
   // with different carveouts do not share an SM (measured: +20 us per closed-loop iteration otherwise)
-  static int carveout_set = -1;
-  if (carveout_set != p.carveout) {
-    const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, p.carveout);
-    if (e != cudaSuccess) return e;
-    carveout_set = p.carveout;
-  }
+  static std::atomic<int> carveout_set[kMaxDevices];
+  if (const cudaError_t e = set_func_attr_once(carveout_set, p.device, kernel, cudaFuncAttributePreferredSharedMemoryCarveout, p.carveout))
+    return e;
   kernel<<<grid, kRolloutThreads, smem, stream>>>(p, d_x0, d_L, d_xT);
   return cudaGetLastError();
 }

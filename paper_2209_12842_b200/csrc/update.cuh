@@ -46,7 +46,7 @@ weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S
                       float* __restrict__ v_out, float* __restrict__ w_out,
                       float* __restrict__ stats, double* __restrict__ partial) {
   __shared__ ST red_s[32];
-  __shared__ float red_f[96];
+  __shared__ double red_f[96];
   const int t = blockIdx.x;
   const int k_chunk = (p.K + gridDim.y - 1) / gridDim.y;
   const int k_begin = blockIdx.y * k_chunk, k_end = min(p.K, k_begin + k_chunk);
@@ -55,13 +55,15 @@ weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S
   for (int k = k_begin + threadIdx.x; k < k_end; k += blockDim.x) bmin = min(bmin, s_tilde_at<ST>(S_tilde, pen, k));
   const ST beta = block_reduce<ST>(bmin, red_s, [](ST a, ST b) { return a < b ? a : b; }, (ST)INFINITY);
 
-  float Z = 0.0f, n0 = 0.0f, n1 = 0.0f;
+  // Z and the two numerators are summed in fp64: with soft weights (ESS >> 1) and K = 65536 an fp32 sum would
+  // spend a visible part of the 1e-4 budget of v+ on its own rounding.  Each w~ is an fp32 exp2 of an fp32 argument.
+  double Z = 0.0, n0 = 0.0, n1 = 0.0;
   for (int k = k_begin + threadIdx.x; k < k_end; k += blockDim.x) {
     const float w = exp2f((float)(s_tilde_at<ST>(S_tilde, pen, k) - beta) * p.neg_log2e_over_lambda);
     const float2 uk = __ldg(u + (long long)k * su_k + (long long)t * su_t);
-    Z += w;
-    n0 = fmaf(w, uk.x, n0);
-    n1 = fmaf(w, uk.y, n1);
+    Z += (double)w;
+    n0 = fma((double)w, (double)uk.x, n0);
+    n1 = fma((double)w, (double)uk.y, n1);
   }
   // one fixed-order tree for the three sums (a single shared-memory exchange)
 #pragma unroll
@@ -74,9 +76,9 @@ weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
     if (lane == 0) { red_f[warp] = Z; red_f[32 + warp] = n0; red_f[64 + warp] = n1; }
     __syncthreads();
-    Z = lane < nw ? red_f[lane] : 0.0f;
-    n0 = lane < nw ? red_f[32 + lane] : 0.0f;
-    n1 = lane < nw ? red_f[64 + lane] : 0.0f;
+    Z = lane < nw ? red_f[lane] : 0.0;
+    n0 = lane < nw ? red_f[32 + lane] : 0.0;
+    n1 = lane < nw ? red_f[64 + lane] : 0.0;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
       Z += __shfl_xor_sync(0xFFFFFFFFu, Z, o);
@@ -86,19 +88,19 @@ weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S
   }
   if (partial) {   // K-sharded step: the shard's unnormalised share {beta_g, Z_g, N_g[T][2]}
     if (threadIdx.x == 0) {
-      if (t == 0) { partial[0] = (double)beta; partial[1] = (double)Z; }
-      partial[2 + 2 * t] = (double)n0;
-      partial[3 + 2 * t] = (double)n1;
+      if (t == 0) { partial[0] = (double)beta; partial[1] = Z; }
+      partial[2 + 2 * t] = n0;
+      partial[3 + 2 * t] = n1;
     }
     return;
   }
   if (threadIdx.x == 0) {
-    v_out[2 * t] = clampf(n0 / Z, p.u_min[0], p.u_max[0]);
-    v_out[2 * t + 1] = clampf(n1 / Z, p.u_min[1], p.u_max[1]);
-    if (t == 0 && stats) { stats[0] = (float)beta; stats[1] = Z; }
+    v_out[2 * t] = clampf((float)(n0 / Z), p.u_min[0], p.u_max[0]);
+    v_out[2 * t + 1] = clampf((float)(n1 / Z), p.u_min[1], p.u_max[1]);
+    if (t == 0 && stats) { stats[0] = (float)beta; stats[1] = (float)Z; }
   }
   if (t == 0 && w_out) {
-    const float invZ = 1.0f / Z;
+    const float invZ = (float)(1.0 / Z);
     for (int k = threadIdx.x; k < p.K; k += blockDim.x)
       w_out[k] = exp2f((float)(s_tilde_at<ST>(S_tilde, pen, k) - beta) * p.neg_log2e_over_lambda) * invZ;
   }
@@ -107,21 +109,22 @@ weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S
 // Exchange step of the K-sharded iteration: partials [n][2+2T] = {beta_g, Z_g, N_g[T][2]} of the shards
 // -> v+ = clamp(sum_g s_g N_g / sum_g s_g Z_g), s_g = exp(-(beta_g - beta)/lambda), beta = min_g beta_g,
 // which is (17)/(4) over the union of the shards (factor exp(-(beta_g-beta)/lambda) out of every w~_k).
-// Fixed summation order over g => every rank computes bitwise the same v+.  One CTA, thread = (t, i).
+// Fixed summation order over g => every rank computes bitwise the same v+; fp64 until the final divide.
+// One CTA, thread = (t, i).
 __global__ void combine_partials_kernel(const __grid_constant__ Params p, const double* __restrict__ partials,
                                         int n_parts, float* __restrict__ v_out) {
   const int stride = 2 + 2 * p.T;
   double beta = INFINITY;
   for (int g = 0; g < n_parts; ++g) beta = fmin(beta, partials[(size_t)g * stride]);
   for (int j = threadIdx.x; j < 2 * p.T; j += blockDim.x) {
-    float Z = 0.0f, n = 0.0f;
+    double Z = 0.0, n = 0.0;
     for (int g = 0; g < n_parts; ++g) {
       const double* pg = partials + (size_t)g * stride;
-      const float s = exp2f((float)(pg[0] - beta) * p.neg_log2e_over_lambda);
-      Z = fmaf(s, (float)pg[1], Z);
-      n = fmaf(s, (float)pg[2 + j], n);
+      const double s = (double)exp2f((float)(pg[0] - beta) * p.neg_log2e_over_lambda);
+      Z = fma(s, pg[1], Z);
+      n = fma(s, pg[2 + j], n);
     }
-    v_out[j] = clampf(n / Z, p.u_min[j & 1], p.u_max[j & 1]);
+    v_out[j] = clampf((float)(n / Z), p.u_min[j & 1], p.u_max[j & 1]);
   }
 }
 

@@ -4,6 +4,11 @@ import numpy as np
 TOL_STATE_ABS = 1e-3     # rollout states at t = T: m, rad, m/s
 TOL_COST_REL = 1e-4      # CVaR and total costs
 TOL_V_ABS = 1e-4         # updated mean control
+ZERO_MARGIN_M = 1e-5     # "exact zeros must match" (G28) away from an obstacle rim by more than this
+
+# every end-to-end v+ comparison of the session: (case, verdict, err, max|dS~|, gap of the two smallest S~, bound);
+# tests/conftest.py prints the tally and writes gpurun_out/parity_verdicts.md at session end
+VERDICTS = []
 
 
 def rel_err(a, b):
@@ -32,7 +37,9 @@ def check_rollout_parity(p, ctl, orc, iteration=0, x0=None, v=None, k_begin=0, k
     """Stage-wise parity of A1-A7 (SURVEY.md section 8(c) 'How parity is checked')."""
     from oracle import oracle as O
     g = gpu_outputs(ctl, p, iteration, x0, v)
-    r = orc.rollout_costs(x0=x0, v=v, iteration=iteration, k_begin=k_begin, k_end=k_end, n_threads=8)
+    hinge = p.risk == 0          # circle risk: the oracle also reports each rollout's closest approach to a rim
+    r = orc.rollout_costs(x0=x0, v=v, iteration=iteration, k_begin=k_begin, k_end=k_end, n_threads=8,
+                          want_margin=hinge)
     sl = slice(k_begin, k_end)
     gs = {k: a[sl] for k, a in g.items()}
     # A1: sampled controls
@@ -43,8 +50,15 @@ def check_rollout_parity(p, ctl, orc, iteration=0, x0=None, v=None, k_begin=0, k
     # A2/A4: costs
     assert_costs_close(gs["S"], r["S"], "S")
     assert_costs_close(gs["L"], r["L"], "L")
-    assert np.array_equal(gs["L"][r["L"] == 0] == 0, np.ones((r["L"] == 0).sum(), bool)) or \
-        (gs["L"][r["L"] == 0] < 1e-4 * max(1.0, np.median(np.abs(r["L"][r["L"] != 0])) if (r["L"] != 0).any() else 1)).all()
+    if hinge:
+        # exact zeros must match (G28): a rollout the oracle scores exactly 0 and whose closest approach to
+        # any rim r + margin exceeds ZERO_MARGIN_M must be exactly 0 on the GPU too (exact culling, no leakage); within
+        # ZERO_MARGIN_M of a rim both answers are correct and the relative tolerance above already bounds the value
+        clear = (r["L"] == 0) & (r["margin"][:, 1:] > ZERO_MARGIN_M)
+        assert (gs["L"][clear] == 0).all(), f"{(gs['L'][clear] != 0).sum()} rollouts clear of every obstacle have L != 0"
+        # and the other way round: nothing the oracle scores > 0 clear of a rim may vanish on the GPU
+        inside = (r["L"] > 0) & (r["margin"][:, 1:] > ZERO_MARGIN_M)
+        assert (gs["L"][inside] > 0).all()
     # A5/A6 isolated: the oracle's sort-based CVaR of the GPU's own L must equal the GPU's CVaR
     k_tail = O.tail_count(p.alpha, p.M)
     iso = np.array([O.cvar_topk(O.sensitivity_scale(gs["L"][i].astype(np.float64), p.B), k_tail)
@@ -75,8 +89,19 @@ def check_update_parity(p, ctl, orc, r):
     assert int(w.argmax()) == int(np.argmax(ref["w"])) or np.sort(ref["w"])[-2] > 1 - 1e-3
 
 
-def check_step_parity(p, ctl, orc, r, iteration=0, x0=None, v=None):
-    """End-to-end v+ (gap-aware: the softmin is one-hot at the BASELINE cost scales)."""
+def check_step_parity(p, ctl, orc, r, iteration=0, x0=None, v=None, case=None):
+    """End-to-end v+ against the oracle.
+
+    "match": |v+ - oracle v+| < 1e-4 outright.  Otherwise the mismatch must be explained, and bounded, by the
+    sensitivity of the softmin (17) to the fp32 error dS~ of the costs -- the softmin is one-hot at the BASELINE cost
+    scales, so two near-tied minima can swap:
+      (a) A8-A9 in isolation: the GPU's own fp64 S~ through the ORACLE's update reproduces the GPU's v+ to 1e-4;
+      (b) a rigorous bound: perturbing every S~_k by at most D changes each normalised weight by a factor within
+          exp(+-2D/lambda), hence |dv+| <= (exp(2D/lambda) - 1) max_{t,i} sum_k w_k |u_k - v+| (clamping is 1-Lipschitz).
+          D = max |dS~| over the samples that can carry weight (S~ - beta <= 30 lambda on either side); the rest hold at
+          most K exp(-30) of the weight.  The observed error must lie within that bound.
+    The verdict says which it was: "near-tie" when the two smallest oracle S~ are closer than 2D (SURVEY's condition),
+    else "weight-sensitive".  Every call is recorded in VERDICTS."""
     import torch
     d_x0 = ctl.tensor(p.x0 if x0 is None else x0)
     d_v = ctl.tensor(p.v if v is None else v)
@@ -84,16 +109,25 @@ def check_step_parity(p, ctl, orc, r, iteration=0, x0=None, v=None):
     torch.cuda.synchronize()
     vp = d_v.cpu().numpy()
     ref = orc.weights_update(r["S_tilde"], r["u"])
-    err = np.abs(vp - ref["v_plus"]).max()
+    err = float(np.abs(vp - ref["v_plus"]).max())
+    name = case or f"{p.name} K={p.K} M={p.M} T={p.T} lambda={p.lam:g}"
+    s2 = np.sort(r["S_tilde"])[:2]
+    gap = float(s2[1] - s2[0]) if s2.size > 1 else float("inf")
     if err < TOL_V_ABS:
+        VERDICTS.append((name, "match", err, None, gap, None))
         return "match", err
-    # The softmin is sharp at the BASELINE cost scales: fp32 error in q perturbs the weights by
-    # exp(+-dS/lambda).  Isolate A8-A9: the GPU's own fp64 S~ through the oracle's update must
-    # reproduce the GPU's v+.
     _, St = ctl.costs_f64()
     St = St.cpu().numpy()
     ref2 = orc.weights_update(St, r["u"])
     err2 = np.abs(vp - ref2["v_plus"]).max()
-    assert err2 < TOL_V_ABS, f"v+ with GPU S~ through oracle update: {err2:.3e}"
-    dS = np.abs(St - r["S_tilde"])
-    return f"weight-sensitive (end-to-end err {err:.2e}, max|dS~| {dS.max():.2e}, lambda {p.lam})", err
+    assert err2 < TOL_V_ABS, f"v+ with GPU S~ through oracle update: {err2:.3e}"              # (a)
+    live = ((r["S_tilde"] - r["S_tilde"].min()) <= 30 * p.lam) | ((St - St.min()) <= 30 * p.lam)
+    D = float(np.abs(St - r["S_tilde"])[live].max())
+    w = ref["w"] / ref["Z"]
+    mad = np.einsum("k,kti->ti", w, np.abs(r["u"] - ref["v_plus"][None])).max()
+    span = np.abs(r["u"] - ref["v_plus"][None]).max()
+    bound = TOL_V_ABS + float(np.expm1(2 * D / p.lam)) * mad + p.K * np.exp(-30.0) * span
+    assert err <= bound, f"v+ err {err:.3e} exceeds the weight-sensitivity bound {bound:.3e} (max|dS~| {D:.3e}, lambda {p.lam})"   # (b)
+    kind = "near-tie" if gap < 2 * D else "weight-sensitive"
+    VERDICTS.append((name, kind, err, D, gap, bound))
+    return f"{kind} (end-to-end err {err:.2e} <= bound {bound:.2e}; max|dS~| {D:.2e}, gap {gap:.2e}, lambda {p.lam})", err

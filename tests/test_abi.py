@@ -111,3 +111,36 @@ def test_product_does_not_import_oracle():
     for f in os.listdir(os.path.join(ROOT, "oracle")):
         if f.endswith((".py", ".cpp", ".h")):
             assert not pat2.search(open(os.path.join(ROOT, "oracle", f)).read()), f
+
+
+def test_tail_and_mean_counts_survive_fp32_parameters(lib):
+    """k_tail = ceil((1-alpha) M) and K0 = ceil((1-eta) K) are integer decisions taken from fp32 parameters: the
+    library (2^-23 n guard) must agree with the fp64 oracle (1e-9 guard) for every decimal a caller would type,
+    including those whose fp32 rounding falls on the wrong side of an integer (G11)."""
+    import math
+
+    from oracle import oracle as O
+    p = W.config0()
+    for M in (1, 2, 10, 16, 20, 37, 64, 100, 128, 256, 300, 512):
+        for alpha in (0.01, 0.05, 0.1, 0.25, 0.3, 0.35, 0.5, 0.6, 0.7, 0.75, 0.8, 0.85, 0.9, 0.95, 0.975, 0.99, 0.999):
+            k_tail, _ = B.ra_mppi_query_counts(B.make_config(p.replace(M=M, alpha=alpha)))
+            assert k_tail == O.tail_count(alpha, M), (alpha, M)
+    assert B.ra_mppi_query_counts(B.make_config(p.replace(M=10, alpha=0.7)))[0] == 3       # 0.7f -> 3.0000001
+    assert B.ra_mppi_query_counts(B.make_config(p.replace(M=300, alpha=0.9)))[0] == 30     # the paper's N = 300
+    # alpha on both sides of an integer (1-alpha) M, 2e-4 away: outside the 2^-23 M = 6e-5 guard window at M = 512
+    for k in (1, 13, 26, 400):
+        lo, hi = 1.0 - (k - 2e-4) / 512.0, 1.0 - (k + 2e-4) / 512.0
+        assert B.ra_mppi_query_counts(B.make_config(p.replace(M=512, alpha=lo)))[0] == k == O.tail_count(lo, 512)
+        assert B.ra_mppi_query_counts(B.make_config(p.replace(M=512, alpha=hi)))[0] == k + 1 == O.tail_count(hi, 512)
+    for K in (10, 96, 1000, 1024, 4096, 65536):
+        for eta in (0.0, 0.05, 0.1, 0.2, 0.25, 0.3, 0.35, 0.5, 0.65, 0.7, 0.8, 0.9, 0.95):
+            _, K0 = B.ra_mppi_query_counts(B.make_config(p.replace(K=K, eta=eta)))
+            assert K0 == math.ceil((1.0 - eta) * K - 1e-9), (eta, K)
+    assert B.ra_mppi_query_counts(B.make_config(p.replace(K=1000, eta=0.7)))[1] == 300
+    assert B.ra_mppi_query_counts(B.make_config(p.replace(K=10, eta=0.9)))[1] == 1
+    # sharded: the split is taken on the global sample count
+    assert B.ra_mppi_query_counts(B.make_config(p.replace(K=100, K_total=1000, k_offset=200, eta=0.35)))[1] == 650
+    cfg = B.make_config(p)
+    cfg.alpha = 1.0
+    with pytest.raises(B.RaMppiError):
+        B.ra_mppi_query_counts(cfg)

@@ -29,9 +29,16 @@ def _random_problem(seed):
     p = W.small(base, K=K, M=M, T=T)
     scale = (0.1, 0.5) if p.dyn == W.DYN_BICYCLE else (0.1, 2.0)
     kind = int(rng.integers(0, 3))
+    alpha = float(np.float32(rng.uniform(0.05, 0.99)))
+    if rng.integers(0, 3) == 0 and M >= 2:
+        # alpha just below / above a value that makes (1-alpha) M an integer j: the tail count must flip between j and
+        # j + 1 on both sides alike (5e-7 M away: outside the library's 2^-23 M guard window, G11)
+        j, side = int(rng.integers(1, M)), float(rng.choice([-1.0, 1.0]))
+        alpha = float(np.float32(1.0 - (j + side * 5e-7 * M) / M))
     return p.replace(
         v=W.random_mean_control(p, seed, scale), seed=int(rng.integers(0, 2**40)),
-        alpha=float(np.float32(rng.uniform(0.05, 0.99))), eta=float(rng.choice([0.0, 0.3])),
+        alpha=alpha, eta=float(rng.choice([0.0, 0.3, 0.7, 0.35, 0.9])),
+        noise_mode=int(rng.choice([W.NOISE_FUSED, W.NOISE_FUSED, W.NOISE_MATERIALISED])),
         B=float(rng.choice([1.0, 2.5])), A=float(rng.choice([1.0, 5.0])), C_u=float(rng.choice([0.0, 20.0])),
         lam=float(rng.choice([0.5, 50.0])), noise_kind=kind,
         noise_p=[0.3, 0.0, 0.0, 0.0] if kind == W.NOISE_JUMP else [0.0] * 4)

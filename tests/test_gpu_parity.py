@@ -194,7 +194,10 @@ def test_non_gaussian_noise_kinds(torch_cuda):
 
 
 def test_materialised_noise_equals_fused(torch_cuda):
-    for p in (_with_v(W.small(W.config3(), K=65, M=128, T=10)), _with_v(W.small(W.config2(), K=20, M=50, T=8))):
+    # M = 96 / 160: three / five slots of 32 realisations with two interleaved per lane, so the last group carries one
+    # slot past the end (its loads must stay inside the noise tensor: ADVICE r1)
+    for p in (_with_v(W.small(W.config3(), K=65, M=128, T=10)), _with_v(W.small(W.config2(), K=20, M=50, T=8)),
+              _with_v(W.small(W.config1(), K=33, M=96, T=12)), _with_v(W.small(W.config2(), K=9, M=160, T=7))):
         a = gpu_outputs(_ctl(p), p)
         b = gpu_outputs(_ctl(p.replace(noise_mode=W.NOISE_MATERIALISED)), p)
         # same draws; the fused kernel contracts sigma*z + x into one FMA, so equality is to rounding
@@ -273,6 +276,19 @@ def test_paper_racing_single_track(torch_cuda):
     ctl.close()
 
 
+def test_racing_nominal_cost_with_hinge_circle_risk(torch_cuda):
+    """Racing nominal cost (20)-(23) together with the BASELINE hinge risk: the indicator (22) tests the bare radius
+    (it has no margin) while the hinge risk tests r + margin, from one obstacle table."""
+    p = W.paper_racing(K=64, M=64, T=30)
+    p = p.replace(risk=W.RISK_CIRCLES, risk_p=[1000.0, 0.2], v=W.random_mean_control(p, 7, (0.1, 0.5)))
+    ctl, orc = _ctl(p), O.Oracle(p)
+    g = gpu_outputs(ctl, p)
+    r = orc.rollout_costs(n_threads=8, want_margin=True)
+    _racing_compare(p, g, r, slice(0, p.K))
+    assert (r["L"] > 0).mean() > 0.01 and (r["S"] != r["S"][0]).any()
+    ctl.close()
+
+
 def test_baseline_mppi_mode_skips_the_noisy_rollouts(torch_cuda):
     """A = 0 is the MPPI of section II: S~ = S, and ra_mppi_step needs no noisy rollout."""
     torch = torch_cuda
@@ -290,6 +306,13 @@ def test_baseline_mppi_mode_skips_the_noisy_rollouts(torch_cuda):
     g, r = check_rollout_parity(p, ctl, orc, iteration=3)
     assert (g["cvar"] > 0).any() and np.array_equal(g["S"], g["S_tilde"])
     assert _ctl(p.replace(A=1.0)).launches_per_step == 4
+    # no rollout kernel is launched by an A = 0 step, so there is nothing to time: a clear error, not a CUDA failure
+    from paper_2209_12842_b200 import binding as B
+    ctl.enable_kernel_timing(True)
+    ctl.step(d_x0, d_v, 4)
+    with pytest.raises(B.RaMppiError) as e:
+        ctl.last_rollout_ms()
+    assert e.value.status == B.RA_EINVAL and "timed" in str(e.value)
 
 
 def test_set_env_replaces_obstacles_and_costmap(torch_cuda):
