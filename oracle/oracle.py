@@ -46,6 +46,7 @@ def lib():
         L.orc_philox4x32_10.argtypes = [_U32P, _U32P, _U32P]
         L.orc_counter.argtypes = [C.c_uint32] * 6 + [C.c_uint64, _U32P]
         L.orc_box_muller.argtypes = [C.c_uint32, C.c_uint32, _DP]
+        L.orc_box_muller16.argtypes = [C.c_uint32, _DP]
         L.orc_state_noise.argtypes = [C.POINTER(OrcProblem), C.c_uint32, C.c_uint32, C.c_uint32,
                                       C.c_uint32, C.c_uint64, _DP]
         L.orc_nx.argtypes = [C.c_int32]
@@ -230,6 +231,12 @@ def counter(k, m, t, J, j, stream, iteration):
 def box_muller(ra, rb):
     z = np.zeros(2)
     lib().orc_box_muller(int(ra), int(rb), _dp(z))
+    return z
+
+
+def box_muller16(w):
+    z = np.zeros(2)
+    lib().orc_box_muller16(int(w), _dp(z))
     return z
 
 

@@ -43,12 +43,12 @@ inline void philox_round(uint32_t c[4], const uint32_t k[2]) {
 
 inline double clampd(double x, double lo, double hi) { return x < lo ? lo : (x > hi ? hi : x); }
 
-/* Number of 32-bit words one state step takes from the (k, m, stream, iteration) word stream: one per state
- * component, plus (jump noise) one for the trigger and one unused so that Box-Muller pairs stay aligned.
- * D:RNG layout. */
+/* Number of 32-bit words one state step takes from the (k, m, stream, iteration) word stream.  State noise spends
+ * 16 bits per uniform (D:RNG layout): one word carries one Box-Muller pair (two state components) or two uniform
+ * draws, so a step takes n_x / 2 words, plus (jump noise) one word whose high half is the trigger. */
 inline uint32_t words_per_step(const orc_problem* p) {
   const uint32_t nx = (uint32_t)orc_nx(p->dyn);
-  return p->noise_kind == ORC_NOISE_JUMP ? nx + 2u : nx;
+  return p->noise_kind == ORC_NOISE_JUMP ? nx / 2u + 1u : nx / 2u;
 }
 
 }  // namespace
@@ -85,6 +85,18 @@ void orc_box_muller(uint32_t ra, uint32_t rb, double z[2]) {
   z[1] = rho * std::sin(2.0 * kPi * u2);
 }
 
+/* Box-Muller pair from ONE Philox word, 16 bits per uniform (state-noise streams; D:RNG layout):
+ * u1 = ((w >> 16) + 1/2) 2^-16 in (0,1), u2 = (w & 0xFFFF) 2^-16 in [0,1), both exactly representable in fp32 and
+ * fp64.  |z| <= sqrt(2 * 17 ln 2) = 4.855 (truncated mass 1.2e-6 per draw); E z^2 = 1 - 5.3e-6, E z^4 = 3 - 2.1e-4
+ * on this lattice (exact sums, pinned in tests/test_oracle_rng.py). */
+void orc_box_muller16(uint32_t w, double z[2]) {
+  const double u1 = ((double)(w >> 16) + 0.5) * (1.0 / 65536.0);
+  const double u2 = (double)(w & 0xFFFFu) * (1.0 / 65536.0);
+  const double rho = std::sqrt(-2.0 * std::log(u1));
+  z[0] = rho * std::cos(2.0 * kPi * u2);
+  z[1] = rho * std::sin(2.0 * kPi * u2);
+}
+
 int orc_nx(int32_t dyn) { return dyn == ORC_DYN_SINGLE_TRACK ? 6 : 4; }
 
 /* w_t of (6) P:63 for realisation (k,m) at step t.  BASELINE configs: additive,
@@ -99,26 +111,28 @@ void orc_state_noise(const orc_problem* p, uint32_t k, uint32_t m, uint32_t t,
   const uint32_t key[2] = {(uint32_t)(p->seed & 0xFFFFFFFFull), (uint32_t)(p->seed >> 32)};
   /* D:RNG layout: the realisation (k, m) of a stream owns the word stream
    *   word n = output (n mod 4) of Philox4x32-10 at counter (k, m, n div 4, stream<<28 | iteration),
-   * and step t takes the words Wd*t .. Wd*t + Wd - 1 in component order. */
-  const uint32_t n0 = Wd * t, c_first = n0 / 4u, c_last = (n0 + Wd - 1u) / 4u;   /* at most 3 calls */
-  uint32_t call[3][4];
+   * and step t takes the words Wd*t .. Wd*t + Wd - 1: word j carries state components 2j, 2j+1. */
+  const uint32_t n0 = Wd * t, c_first = n0 / 4u, c_last = (n0 + Wd - 1u) / 4u;   /* at most 2 calls */
+  uint32_t call[2][4];
   for (uint32_t c = c_first; c <= c_last; ++c) {
     uint32_t ctr[4];
     orc_counter(k, m, c, 1u, 0u, stream, iteration, ctr);
     orc_philox4x32_10(ctr, key, call[c - c_first]);
   }
-  uint32_t r[8];
+  uint32_t r[4];
   for (uint32_t i = 0; i < Wd; ++i) r[i] = call[(n0 + i) / 4u - c_first][(n0 + i) % 4u];
-  double z[8];
+  double z[6];
   if (p->noise_kind == ORC_NOISE_UNIFORM) {
-    /* (2*(r>>9)+1) 2^-23 - 1 : symmetric on (-1,1), exactly representable */
-    for (uint32_t i = 0; i < nx; ++i)
-      z[i] = (double)(2u * (r[i] >> 9) + 1u) * (1.0 / 8388608.0) - 1.0;
+    /* (2 h + 1) 2^-16 - 1 : symmetric on (-1,1), exactly representable; component 2j from the high half */
+    for (uint32_t j = 0; j < nx / 2u; ++j) {
+      z[2 * j] = (double)(2u * (r[j] >> 16) + 1u) * (1.0 / 65536.0) - 1.0;
+      z[2 * j + 1] = (double)(2u * (r[j] & 0xFFFFu) + 1u) * (1.0 / 65536.0) - 1.0;
+    }
   } else {
-    for (uint32_t i = 0; i < nx; i += 2) orc_box_muller(r[i], r[i + 1], z + i);
+    for (uint32_t j = 0; j < nx / 2u; ++j) orc_box_muller16(r[j], z + 2 * j);
   }
   if (p->noise_kind == ORC_NOISE_JUMP) {
-    const double uj = (double)(r[nx] >> 9) * (1.0 / 8388608.0);   /* the trigger word follows the components */
+    const double uj = (double)(r[nx / 2u] >> 16) * (1.0 / 65536.0);   /* trigger: high half of the word after the pairs */
     double nrm = 0.0;
     for (uint32_t i = 0; i < nx; ++i) nrm += z[i] * z[i];
     nrm = std::sqrt(nrm);

@@ -14,7 +14,9 @@
  * Pins (tests/test_oracle_*.py, all `-m "not gpu"`):
  *   philox4x32_10        - agreement with ATen's at::philox_engine (compiled from
  *                          torch's header by the test) and cuRAND's host generator
- *   box_muller           - moments of 2^22 draws, exact end points
+ *   box_muller           - moments of 2^19 draws, exact end points
+ *   box_muller16         - exact end points, exact lattice moments, sample moments, Kolmogorov-Smirnov
+ *                          distance and tail mass at the alpha quantiles in use, word / half-word layout
  *   cvar_topk / literal  - brute force on hand arrays, Rockafellar-Uryasev
  *                          identity, closed-form Gaussian CVaR
  *   dynamics             - closed-form Euler sums, straight-line / steady-state
@@ -73,7 +75,8 @@ typedef struct {
 void   orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
 void   orc_counter(uint32_t k, uint32_t m, uint32_t t, uint32_t J, uint32_t j,
                    uint32_t stream, uint64_t iteration, uint32_t ctr[4]);
-void   orc_box_muller(uint32_t ra, uint32_t rb, double z[2]);
+void   orc_box_muller(uint32_t ra, uint32_t rb, double z[2]);   /* 23-bit uniforms, two words (control draw eps) */
+void   orc_box_muller16(uint32_t w, double z[2]);                /* 16-bit uniforms, one word (state noise)     */
 /* the n_x noise values added to the state at step t of realisation (k,m)     */
 void   orc_state_noise(const orc_problem* p, uint32_t k, uint32_t m, uint32_t t,
                        uint32_t stream, uint64_t iteration, double w[6]);

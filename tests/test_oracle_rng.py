@@ -113,6 +113,45 @@ def _draws(p, n_calls):
     return np.array([orc.state_noise(i & 0xFFFF, i >> 16, 0, 1, 0) for i in range(n_calls)])
 
 
+def test_box_muller16_end_points():
+    """State-noise normals: ONE word per pair, 16 bits per uniform:
+    u1 = (hi + 1/2) 2^-16 in (0,1) from the high half, u2 = lo 2^-16 from the low half."""
+    rho_max = np.sqrt(2 * 17 * np.log(2.0))                   # u1 = 2^-17
+    z = O.box_muller16(0x00000000)
+    assert z[0] == pytest.approx(rho_max, rel=1e-15) and z[1] == 0.0
+    z = O.box_muller16(0x00004000)                             # u2 = 1/4 -> angle pi/2
+    assert abs(z[0]) < 1e-15 and z[1] == pytest.approx(rho_max, rel=1e-15)
+    z = O.box_muller16(0x00008000)                             # u2 = 1/2 -> angle pi
+    assert z[0] == pytest.approx(-rho_max, rel=1e-15) and abs(z[1]) < 1e-15
+    z = O.box_muller16(0xFFFF0000)                             # u1 = 1 - 2^-17: the smallest radius, never exactly 0
+    assert z[0] == pytest.approx(np.sqrt(-2 * np.log1p(-2.0**-17)), rel=1e-12) and z[0] > 0
+    z = O.box_muller16(0x7FFF0000)                             # u1 = (32767.5) 2^-16
+    assert z[0] == pytest.approx(np.sqrt(-2 * np.log(32767.5 / 65536)), rel=1e-15)
+    # the halves are not swapped: changing the low half rotates, changing the high half rescales
+    a, b, c = O.box_muller16(0x12340000), O.box_muller16(0x12344000), O.box_muller16(0x56780000)
+    assert np.hypot(*a) == pytest.approx(np.hypot(*b), rel=1e-15) and np.hypot(*a) != pytest.approx(np.hypot(*c), rel=1e-3)
+    assert a[1] == 0.0 and c[1] == 0.0 and abs(b[0]) < 1e-15
+
+
+def test_box_muller16_exact_lattice_moments():
+    """The 2^32 words map to a polar lattice; its moments are exact finite sums: E z^2 = 1 - 5.3e-6,
+    E z^4 = 3 - 2.1e-4, |z| <= 4.855 (the numbers DESIGN.md states for the 16-bit layout).  The radial sum is over
+    all 65536 radii; the angular sums over 65536 equally spaced angles are exact by symmetry
+    (mean cos^2 = 1/2, mean cos^4 = 3/8)."""
+    hi = np.arange(65536, dtype=np.uint64)
+    rho = np.array([np.hypot(*O.box_muller16(int(h) << 16)) for h in hi[::257]])       # sampled radii via the oracle
+    r2_all = -2.0 * np.log((hi.astype(np.float64) + 0.5) / 65536.0)
+    assert np.allclose(rho**2, r2_all[::257], rtol=1e-13)
+    Ez2, Ez4 = r2_all.mean() / 2.0, (r2_all**2).mean() * 3.0 / 8.0
+    assert Ez2 == pytest.approx(1.0 - 5.29e-6, abs=2e-8) and Ez4 == pytest.approx(3.0 - 2.106e-4, abs=1e-6)
+    assert np.sqrt(r2_all.max()) == pytest.approx(4.8546, abs=1e-4)
+    lo = np.arange(0, 65536, 97)
+    ang = np.array([O.box_muller16(0x80000000 | int(l)) for l in lo])
+    r0 = np.sqrt(-2.0 * np.log(32768.5 / 65536.0))
+    assert np.allclose(ang[:, 0], r0 * np.cos(2 * np.pi * lo / 65536.0), atol=1e-15)
+    assert np.allclose(ang[:, 1], r0 * np.sin(2 * np.pi * lo / 65536.0), atol=1e-15)
+
+
 def test_normal_moments():
     z = _draws(_P, 1 << 17).ravel()  # 2^19 normals
     n = z.size
@@ -120,39 +159,91 @@ def test_normal_moments():
     assert abs(z.var() - 1) < 4 * np.sqrt(2 / n)
     assert abs((z**4).mean() - 3) < 4 * np.sqrt(96 / n)
     assert abs((z**3).mean()) < 4 * np.sqrt(15 / n)
-    assert np.abs(z).max() <= 5.65
-    # the four components of one call are uncorrelated
+    assert np.abs(z).max() <= 4.8546
+    # the four components of one step are uncorrelated (two pairs from two words)
     zz = z.reshape(-1, 4)
     c = np.corrcoef(zz.T)
     assert np.abs(c - np.eye(4)).max() < 5 / np.sqrt(zz.shape[0])
+    # squares too (a pair shares its radius only through independent angles): cov(z0^2, z1^2) = 0 for exact normals
+    c2 = np.corrcoef((zz**2).T)
+    assert np.abs(c2 - np.eye(4)).max() < 5 / np.sqrt(zz.shape[0])
 
 
-def test_single_track_takes_six_words_per_step_from_the_word_stream():
-    """D:RNG layout: step t of an n_x = 6 realisation takes words 6t..6t+5 of its stream, word n = output n%4 of
-    call n//4; the n_x = 4 layout at step c IS call c, so it serves as the reference for the call contents."""
+def test_state_noise_distribution_ks_and_tail_mass():
+    """16 bits per uniform must not show in the distribution the CVaR reads: Kolmogorov-Smirnov distance to N(0,1)
+    and the tail mass beyond the alpha-quantiles the configs use (0.9, 0.95, 0.99; both tails), on 2^21 draws."""
+    from scipy import stats
+    z = _draws(_P, 1 << 19).ravel()
+    n = z.size
+    d = stats.kstest(z, "norm").statistic
+    assert d < 1.63 / np.sqrt(n), d                      # 1 % critical value of the KS statistic
+    for alpha in (0.9, 0.95, 0.99, 0.999):
+        q = stats.norm.ppf(alpha)
+        for tail in ((z > q).mean(), (z < -q).mean()):
+            assert abs(tail - (1 - alpha)) < 4 * np.sqrt(alpha * (1 - alpha) / n), (alpha, tail)
+    # tail mean beyond the quantile = the closed-form Gaussian CVaR (golden file: scipy)
+    for alpha, want in ((0.9, 1.7549833), (0.99, 2.6652142)):
+        q = stats.norm.ppf(alpha)
+        got = z[z > q].mean()
+        assert got == pytest.approx(want, abs=4 * 0.6 / np.sqrt((1 - alpha) * n))
+
+
+def _word(k, m, n, stream, it, seed=_P.seed):
+    """Word n of the (k, m, stream, iteration) word stream, from the free functions (pinned above)."""
+    key = (seed & 0xFFFFFFFF, seed >> 32)
+    return O.philox4x32_10(O.counter(k, m, n // 4, 1, 0, stream, it), key)[n % 4]
+
+
+def test_state_noise_word_layout_nx4_and_nx6():
+    """D:RNG layout: step t of a realisation takes the n_x/2 words (n_x/2) t .. of its word stream, word j -> the
+    Box-Muller pair of components (2j, 2j+1): n_x = 4 spends one Philox call on two steps, n_x = 6 three calls on
+    four steps."""
     class P6(_P):
         dyn = 1; dyn_p = [4, 0.05, 0.17, 0.17, 30, 30, 0.5]
     orc4, orc6 = O.Oracle(_P), O.Oracle(P6)
-    call = lambda c: orc4.state_noise(3, 4, c, 1, 6)          # the four normals of call c
-    w_even = orc6.state_noise(3, 4, 4, 1, 6)                   # words 24..29 = call 6 (all), call 7 (outputs 0,1)
-    assert w_even.shape == (6,)
-    assert np.array_equal(w_even[:4], call(6)) and np.array_equal(w_even[4:], call(7)[:2])
-    w_odd = orc6.state_noise(3, 4, 5, 1, 6)                    # words 30..35 = call 7 (outputs 2,3), call 8 (all)
-    assert np.array_equal(w_odd[:2], call(7)[2:]) and np.array_equal(w_odd[2:], call(8))
-    # consecutive steps never reuse a word: 1.5 calls per step on average, no overlap, no gap
-    assert not np.intersect1d(w_even, w_odd).size
+    for t in (0, 1, 2, 3, 7, 58):
+        w4 = orc4.state_noise(3, 4, t, 1, 6)
+        assert w4.shape == (4,)
+        assert np.array_equal(w4, np.concatenate([O.box_muller16(_word(3, 4, 2 * t + j, 1, 6)) for j in range(2)]))
+        w6 = orc6.state_noise(3, 4, t, 1, 6)
+        assert w6.shape == (6,)
+        assert np.array_equal(w6, np.concatenate([O.box_muller16(_word(3, 4, 3 * t + j, 1, 6)) for j in range(3)]))
+    # steps 2s and 2s+1 of an n_x = 4 realisation share call s and nothing else; no word is used twice
+    used = [2 * t + j for t in range(8) for j in range(2)]
+    assert used == list(range(16))
+    # stream and iteration enter the counter; the PLANT stream is realisation (0, 0), step 0
+    assert not np.array_equal(orc4.state_noise(3, 4, 0, 1, 6), orc4.state_noise(3, 4, 0, 2, 6))
+    assert np.array_equal(orc4.state_noise(0, 0, 0, 2, 9),
+                          np.concatenate([O.box_muller16(_word(0, 0, j, 2, 9)) for j in range(2)]))
 
 
 def test_jump_noise_word_layout():
-    """Jump noise takes n_x + 2 words per step: the components, the trigger, one spare (pairs stay aligned)."""
+    """Jump noise takes n_x/2 + 1 words per step: the pairs, then a word whose HIGH half is the trigger."""
     class PJ(_P):
         noise_kind = 2; noise_p = [1.0, 0, 0, 0]     # always jump: the direction is the normalised Gaussian draw
-    orcj, orc4 = O.Oracle(PJ), O.Oracle(_P)
-    call = lambda c: orc4.state_noise(7, 9, c, 1, 2)
-    for t in (0, 1, 2, 3):                           # words 6t..6t+3 are the components
-        n0 = 6 * t
-        z = np.concatenate([call(n0 // 4), call(n0 // 4 + 1)])[n0 % 4: n0 % 4 + 4]
+    class PJh(_P):
+        noise_kind = 2; noise_p = [0.5, 0, 0, 0]
+    orcj, orch = O.Oracle(PJ), O.Oracle(PJh)
+    n_hit = 0
+    for t in range(40):
+        z = np.concatenate([O.box_muller16(_word(7, 9, 3 * t + j, 1, 2)) for j in range(2)])
         assert np.allclose(orcj.state_noise(7, 9, t, 1, 2), z / np.linalg.norm(z), rtol=1e-13)
+        trig = (_word(7, 9, 3 * t + 2, 1, 2) >> 16) / 65536.0
+        got = orch.state_noise(7, 9, t, 1, 2)
+        assert (np.linalg.norm(got) > 0) == (trig < 0.5)
+        n_hit += trig < 0.5
+    assert 8 < n_hit < 32
+
+
+def test_uniform_noise_word_layout():
+    class PU(_P):
+        noise_kind = 1
+    orc = O.Oracle(PU)
+    for t in (0, 1, 5):
+        u = orc.state_noise(2, 3, t, 1, 4)
+        for j in range(2):
+            w = _word(2, 3, 2 * t + j, 1, 4)
+            assert u[2 * j] == (2 * (w >> 16) + 1) / 65536.0 - 1.0 and u[2 * j + 1] == (2 * (w & 0xFFFF) + 1) / 65536.0 - 1.0
 
 
 def test_uniform_and_jump_noise_kinds():
