@@ -70,56 +70,78 @@ __device__ __forceinline__ void box_muller(uint32_t ra, uint32_t rb, float& z0, 
   z1 = rho * (neg ? -sn : sn);
 }
 
-// Fast Box-Muller pair for the state-noise stream (K*M*T*n_x/2 evaluations per iteration): same
-// exact uniforms, but log2 / sqrt / sin / cos on the MUFU unit (lg2.approx, sqrt.approx, sin.approx,
-// cos.approx).  Error budget: |dz| <= ~2e-6 |z| + 2e-7 / max(rho, 1e-3); scaled by
-// sigma_w <= 0.05 that is <= 1e-7 m per step, below the fp32 rounding of the positions themselves.
-//   u1 = as_float(0x3F800000 | n1) - (1 - 2^-23) = (n1 + 1) 2^-23      (one funnel shift + one FADD)
-//   angle = 2 pi (u2 - 1/2) in [-pi, pi) where MUFU.SIN/COS are most accurate (one funnel shift + one
-//   FFMA); the half-turn offset flips both signs.
-// Returns the UNSCALED pair (a0, a1) = sqrt(-log2 u1) (cos, sin)(angle); the normals are
-// z = -sqrt(2 ln 2) a, and that constant is folded into Params::wscale together with sigma_w, so the
-// caller's x += wscale * a is one FFMA per component (12 instructions per pair, 4 of them MUFU).
-__device__ __forceinline__ void box_muller_fast(uint32_t ra, uint32_t rb, float& a0, float& a1) {
-  const float u1 = __uint_as_float(__funnelshift_r(ra, 0x7Fu, 9)) - 0.99999988079071044921875f;
+// Box-Muller pair for the state-noise streams (K*M*T*n_x/2 evaluations per iteration) from ONE Philox word with 16 bits
+// per uniform: u1 = ((w >> 16) + 1/2) 2^-16 in (0,1), u2 = (w & 0xFFFF) 2^-16 in [0,1), both
+// exact in fp32; log2 / sqrt / sin / cos on the MUFU unit (lg2.approx, sqrt.approx, sin.approx, cos.approx).
+// Error budget: |dz| <= ~2e-6 |z| + 2e-7 / max(rho, 1e-3); scaled by sigma_w <= 0.05 that is
+// <= 1e-7 m per step, below the fp32 rounding of the positions themselves.
+//   u1: PRMT builds the float 1 + hi 2^-23 (bytes 0x3F80 : hi16), one FFMA scales it: (1 + hi 2^-23) 128 - (128 - 2^-17)
+//       = (hi + 1/2) 2^-16 exactly (only relative accuracy matters under the logarithm).
+//   angle = 2 pi (u2 - 1/2) in [-pi, pi) where MUFU.SIN/COS are most accurate; here the uniform must sit at the TOP of
+//       the mantissa (x = 1 + lo 2^-16 in [1,2)) so that 2 pi x - 3 pi cancels against 2 pi, not against 2 pi 2^7:
+//       one shift, one funnel shift, one FFMA.  The half-turn offset flips both signs.
+// Returns the UNSCALED pair (a0, a1) = sqrt(-log2 u1) (cos, sin)(angle); the normals are z = -sqrt(2 ln 2) a, and
+// that constant is folded into Params::wscale together with sigma_w, so the caller's x += wscale * a is one FFMA
+// per component.
+__device__ __forceinline__ void box_muller16_fast(uint32_t w, float& a0, float& a1) {
+  const float u1 = fmaf(__uint_as_float(__byte_perm(w, 0x3F800000u, 0x7632)), 128.0f, -127.99999237060546875f);
   float lg, s;
   asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lg) : "f"(u1));
   asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(s) : "f"(-lg));
-  const float th = fmaf(__uint_as_float(__funnelshift_r(rb, 0x7Fu, 9)), 6.283185307179586f, -9.42477796076938f);
+  const float th = fmaf(__uint_as_float(__funnelshift_r(w << 16, 0x7Fu, 9)), 6.283185307179586f, -9.42477796076938f);
   a0 = s * __cosf(th);
   a1 = s * __sinf(th);
 }
 
-// Uniform on (-1,1): (2 (r>>9) + 1) 2^-23 - 1, exact.
-__device__ __forceinline__ float sym_uniform(uint32_t r) {
-  return fmaf(__uint2float_rn(2u * (r >> 9) + 1u), 1.1920928955078125e-07f, -1.0f);
+// h 2^-16 for a 16-bit field already placed in the low mantissa bits (bits 0x3F80 : h = 1 + h 2^-23), exact
+__device__ __forceinline__ float unit16(uint32_t bits) { return fmaf(__uint_as_float(bits), 128.0f, -128.0f); }
+
+// Two uniforms on (-1,1) from one word: (2 h + 1) 2^-16 - 1 for the high and the low half, exact (h 2^-15 by one FFMA,
+// then one FADD; no I2F on the XU pipe).
+__device__ __forceinline__ void sym_uniform16(uint32_t w, float& z_hi, float& z_lo) {
+  const float th = fmaf(__uint_as_float(__byte_perm(w, 0x3F800000u, 0x7632)), 256.0f, -256.0f);
+  const float tl = fmaf(__uint_as_float(__byte_perm(w, 0x3F800000u, 0x7610)), 256.0f, -256.0f);
+  z_hi = th - 0.9999847412109375f;   // 1 - 2^-16
+  z_lo = tl - 0.9999847412109375f;
 }
 
 // ---- state-noise word stream ------------------------------------------------------
 // Realisation (k, m) of a stream owns the word stream  word n = output (n & 3) of Philox4x32-10 at counter
-// (k, m, n >> 2, stream<<28 | iteration); step t takes the WD words WD*t .. WD*t + WD - 1 in component order,
-// WD = n_x (+ 2 for jump noise: trigger word + one spare so that Box-Muller pairs stay aligned).
-// WD = 4: call t.  WD = 8: calls 2t, 2t+1.  WD = 6: 1.5 calls per step -- the rollout kernel walks the horizon in
-// pairs of steps and carries the spare half of the middle call (three calls per two steps, not four).
-template <int NX, int NOISE> struct NoiseWords { static constexpr int value = NX + (NOISE == NOISE_JUMP ? 2 : 0); };
+// (k, m, n >> 2, stream<<28 | iteration); step t takes the WD words WD*t .. WD*t + WD - 1, word j -> state
+// components (2j, 2j+1); WD = n_x / 2 (+ 1 for jump noise: a word whose high half is the trigger).
+// WD = 2: one call per two steps.  WD = 3: three calls per four steps.  WD = 4: one call per step.  The rollout
+// kernel walks the horizon in groups of steps that share calls and carries the spare words.
+template <int NX, int NOISE> struct NoiseWords { static constexpr int value = NX / 2 + (NOISE == NOISE_JUMP ? 1 : 0); };
 
-// The words of step t, on their own (probe, plant, materialised-noise generator, odd last step).
+// The words of step t, on their own (probe, plant, materialised-noise generator, ragged last steps).
 template <int WD>
 __device__ __forceinline__ void step_words(const Params& p, uint32_t k, uint32_t m, uint32_t t, uint32_t c3,
                                            uint32_t (&w)[WD]) {
-  static_assert(WD == 4 || WD == 6 || WD == 8, "words per step");
+  static_assert(WD == 2 || WD == 3 || WD == 4, "words per step");
   if constexpr (WD == 4) {
     const uint4 a = philox4x32_10(k, m, t, c3, p.rk);
     w[0] = a.x; w[1] = a.y; w[2] = a.z; w[3] = a.w;
-  } else if constexpr (WD == 8) {
-    const uint4 a = philox4x32_10(k, m, 2u * t, c3, p.rk), b = philox4x32_10(k, m, 2u * t + 1u, c3, p.rk);
-    w[0] = a.x; w[1] = a.y; w[2] = a.z; w[3] = a.w; w[4] = b.x; w[5] = b.y; w[6] = b.z; w[7] = b.w;
+  } else if constexpr (WD == 2) {
+    const uint4 a = philox4x32_10(k, m, t >> 1, c3, p.rk);
+    const bool odd = (t & 1u) != 0u;
+    w[0] = odd ? a.z : a.x; w[1] = odd ? a.w : a.y;
   } else {
-    const uint32_t c = (3u * t) >> 1;   // (6 t) >> 2
-    const uint4 a = philox4x32_10(k, m, c, c3, p.rk), b = philox4x32_10(k, m, c + 1u, c3, p.rk);
-    const bool odd = (t & 1u) != 0u;    // odd steps start at output 2 of their first call
-    w[0] = odd ? a.z : a.x; w[1] = odd ? a.w : a.y; w[2] = odd ? b.x : a.z; w[3] = odd ? b.y : a.w;
-    w[4] = odd ? b.z : b.x; w[5] = odd ? b.w : b.y;
+    const uint32_t n0 = 3u * t, c = n0 >> 2, o = n0 & 3u;   // first word = output o of call c
+    const uint4 a = philox4x32_10(k, m, c, c3, p.rk);
+    const uint32_t av[4] = {a.x, a.y, a.z, a.w};
+    uint32_t bv[4] = {0u, 0u, 0u, 0u};
+    if (o >= 2u) {   // the step runs over into the next call
+      const uint4 b = philox4x32_10(k, m, c + 1u, c3, p.rk);
+      bv[0] = b.x; bv[1] = b.y; bv[2] = b.z; bv[3] = b.w;
+    }
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      const uint32_t n = o + (uint32_t)i;
+      uint32_t v = 0u;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) v = (n == (uint32_t)j) ? av[j] : ((n == (uint32_t)(j + 4)) ? bv[j] : v);
+      w[i] = v;
+    }
   }
 }
 
@@ -130,14 +152,14 @@ template <int NX, int NOISE>
 __device__ __forceinline__ void noise_from_words(const Params& p, const uint32_t (&w)[NoiseWords<NX, NOISE>::value],
                                                  float (&z)[NX]) {
 #pragma unroll
-  for (int i = 0; i < NX; i += 2) {
-    if constexpr (NOISE == NOISE_UNIFORM) { z[i] = sym_uniform(w[i]); z[i + 1] = sym_uniform(w[i + 1]); }
-    else box_muller_fast(w[i], w[i + 1], z[i], z[i + 1]);
+  for (int j = 0; j < NX / 2; ++j) {
+    if constexpr (NOISE == NOISE_UNIFORM) sym_uniform16(w[j], z[2 * j], z[2 * j + 1]);
+    else box_muller16_fast(w[j], z[2 * j], z[2 * j + 1]);
   }
   if constexpr (NOISE == NOISE_JUMP) {
     // jump of unit length in a uniformly random direction z/|z| (the common factor of the Gaussian
     // draws cancels; its sign is in wscale), with probability noise_p[0]  (G29)
-    const float uj = __uint2float_rn(w[NX] >> 9) * 1.1920928955078125e-07f;
+    const float uj = unit16(__byte_perm(w[NX / 2], 0x3F800000u, 0x7632));
     float n2 = 0.0f;
 #pragma unroll
     for (int i = 0; i < NX; ++i) n2 = fmaf(z[i], z[i], n2);

@@ -394,30 +394,72 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
         }
         advance(t, a);
       }
-    } else if constexpr (NoiseWords<NX, NOISE>::value == 6) {
-      // 1.5 Philox calls per step: two steps share three calls; the spare half of the middle call is carried
+    } else if constexpr (NoiseWords<NX, NOISE>::value == 2) {
+      // n_x = 4: one Philox call serves two steps (16 bits per uniform, one word per Box-Muller pair)
       int t = 0;
       for (; t + 1 < p.T; t += 2) {
-        const uint32_t c = 3u * (uint32_t)(t >> 1);
         uint32_t carry[RC][2];
         float a[RC][NX];
 #pragma unroll
         for (int r = 0; r < RC; ++r) {
-          const uint4 qa = philox4x32_10(kg, m[r], c, c3, p.rk), qb = philox4x32_10(kg, m[r], c + 1u, c3, p.rk);
-          const uint32_t w[6] = {qa.x, qa.y, qa.z, qa.w, qb.x, qb.y};
-          carry[r][0] = qb.z; carry[r][1] = qb.w;
+          const uint4 q = philox4x32_10(kg, m[r], (uint32_t)(t >> 1), c3, p.rk);
+          const uint32_t w[2] = {q.x, q.y};
+          carry[r][0] = q.z; carry[r][1] = q.w;
           noise_from_words<NX, NOISE>(p, w, a[r]);
         }
         advance(t, a);
 #pragma unroll
         for (int r = 0; r < RC; ++r) {
-          const uint4 qc = philox4x32_10(kg, m[r], c + 2u, c3, p.rk);
-          const uint32_t w[6] = {carry[r][0], carry[r][1], qc.x, qc.y, qc.z, qc.w};
+          const uint32_t w[2] = {carry[r][0], carry[r][1]};
           noise_from_words<NX, NOISE>(p, w, a[r]);
         }
         advance(t + 1, a);
       }
-      if (t < p.T) {   // odd horizon: the last (even-indexed) step on its own
+      if (t < p.T) {   // odd horizon: the last (even-indexed) step takes the first half of its call
+        float a[RC][NX];
+#pragma unroll
+        for (int r = 0; r < RC; ++r) state_noise<NX, NOISE>(p, kg, m[r], (uint32_t)t, c3, a[r]);
+        advance(t, a);
+      }
+    } else if constexpr (NoiseWords<NX, NOISE>::value == 3) {
+      // three words per step (n_x = 6, or n_x = 4 with the jump trigger): three calls serve four steps
+      int t = 0;
+      for (; t + 3 < p.T; t += 4) {
+        const uint32_t c = 3u * (uint32_t)(t >> 2);
+        uint32_t carry[RC][3];
+        float a[RC][NX];
+#pragma unroll
+        for (int r = 0; r < RC; ++r) {
+          const uint4 qa = philox4x32_10(kg, m[r], c, c3, p.rk);
+          const uint32_t w[3] = {qa.x, qa.y, qa.z};
+          carry[r][0] = qa.w;
+          noise_from_words<NX, NOISE>(p, w, a[r]);
+        }
+        advance(t, a);
+#pragma unroll
+        for (int r = 0; r < RC; ++r) {
+          const uint4 qb = philox4x32_10(kg, m[r], c + 1u, c3, p.rk);
+          const uint32_t w[3] = {carry[r][0], qb.x, qb.y};
+          carry[r][0] = qb.z; carry[r][1] = qb.w;
+          noise_from_words<NX, NOISE>(p, w, a[r]);
+        }
+        advance(t + 1, a);
+#pragma unroll
+        for (int r = 0; r < RC; ++r) {
+          const uint4 qc = philox4x32_10(kg, m[r], c + 2u, c3, p.rk);
+          const uint32_t w[3] = {carry[r][0], carry[r][1], qc.x};
+          carry[r][0] = qc.y; carry[r][1] = qc.z; carry[r][2] = qc.w;
+          noise_from_words<NX, NOISE>(p, w, a[r]);
+        }
+        advance(t + 2, a);
+#pragma unroll
+        for (int r = 0; r < RC; ++r) {
+          const uint32_t w[3] = {carry[r][0], carry[r][1], carry[r][2]};
+          noise_from_words<NX, NOISE>(p, w, a[r]);
+        }
+        advance(t + 3, a);
+      }
+      for (; t < p.T; ++t) {   // up to three ragged steps on their own
         float a[RC][NX];
 #pragma unroll
         for (int r = 0; r < RC; ++r) state_noise<NX, NOISE>(p, kg, m[r], (uint32_t)t, c3, a[r]);
