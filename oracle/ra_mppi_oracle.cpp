@@ -85,13 +85,17 @@ void orc_box_muller(uint32_t ra, uint32_t rb, double z[2]) {
   z[1] = rho * std::sin(2.0 * kPi * u2);
 }
 
-/* Box-Muller pair from ONE Philox word, 16 bits per uniform (state-noise streams; D:RNG layout):
- * u1 = ((w >> 16) + 1/2) 2^-16 in (0,1), u2 = (w & 0xFFFF) 2^-16 in [0,1), both exactly representable in fp32 and
- * fp64.  |z| <= sqrt(2 * 17 ln 2) = 4.855 (truncated mass 1.2e-6 per draw); E z^2 = 1 - 5.3e-6, E z^4 = 3 - 2.1e-4
- * on this lattice (exact sums, pinned in tests/test_oracle_rng.py). */
+/* Box-Muller pair from ONE Philox word (state-noise streams; D:RNG layout):
+ * radius uniform  u1 = ((w & 0xFFFF) + 1/2) 2^-16 in (0,1)   (the low half of the word),
+ * angle uniform   u2 = (w >> 9) 2^-23 in [0,1)               (the top 23 bits of the word),
+ * both exactly representable in fp32 and fp64.  The two fields share bits 9..15 (the top 7 bits of u1 are the
+ * bottom 7 bits of u2): for every radius the 2^16 remaining angles are equally spaced over the full turn, so the
+ * pair has exactly the mixed moments of (radius lattice) x (uniform angle) and the 2^32 words still map to 2^32
+ * distinct points.  |z| <= sqrt(2 * 17 ln 2) = 4.855 (truncated mass 1.2e-6 per draw); E z^2 = 1 - 5.3e-6,
+ * E z^4 = 3 - 2.1e-4 on this lattice (exact sums, pinned in tests/test_oracle_rng.py). */
 void orc_box_muller16(uint32_t w, double z[2]) {
-  const double u1 = ((double)(w >> 16) + 0.5) * (1.0 / 65536.0);
-  const double u2 = (double)(w & 0xFFFFu) * (1.0 / 65536.0);
+  const double u1 = ((double)(w & 0xFFFFu) + 0.5) * (1.0 / 65536.0);
+  const double u2 = (double)(w >> 9) * (1.0 / 8388608.0);
   const double rho = std::sqrt(-2.0 * std::log(u1));
   z[0] = rho * std::cos(2.0 * kPi * u2);
   z[1] = rho * std::sin(2.0 * kPi * u2);

@@ -76,7 +76,7 @@ void   orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t 
 void   orc_counter(uint32_t k, uint32_t m, uint32_t t, uint32_t J, uint32_t j,
                    uint32_t stream, uint64_t iteration, uint32_t ctr[4]);
 void   orc_box_muller(uint32_t ra, uint32_t rb, double z[2]);   /* 23-bit uniforms, two words (control draw eps) */
-void   orc_box_muller16(uint32_t w, double z[2]);                /* 16-bit uniforms, one word (state noise)     */
+void   orc_box_muller16(uint32_t w, double z[2]);                /* one word: 16-bit radius, 23-bit angle (state noise) */
 /* the n_x noise values added to the state at step t of realisation (k,m)     */
 void   orc_state_noise(const orc_problem* p, uint32_t k, uint32_t m, uint32_t t,
                        uint32_t stream, uint64_t iteration, double w[6]);

@@ -114,42 +114,54 @@ def _draws(p, n_calls):
 
 
 def test_box_muller16_end_points():
-    """State-noise normals: ONE word per pair, 16 bits per uniform:
-    u1 = (hi + 1/2) 2^-16 in (0,1) from the high half, u2 = lo 2^-16 from the low half."""
+    """State-noise normals: ONE word per pair: radius uniform u1 = (lo16 + 1/2) 2^-16 in (0,1)
+    from the low half, angle uniform u2 = (w >> 9) 2^-23 from the top 23 bits."""
     rho_max = np.sqrt(2 * 17 * np.log(2.0))                   # u1 = 2^-17
     z = O.box_muller16(0x00000000)
     assert z[0] == pytest.approx(rho_max, rel=1e-15) and z[1] == 0.0
-    z = O.box_muller16(0x00004000)                             # u2 = 1/4 -> angle pi/2
+    z = O.box_muller16(0x40000000)                             # u2 = 1/4 -> angle pi/2
     assert abs(z[0]) < 1e-15 and z[1] == pytest.approx(rho_max, rel=1e-15)
-    z = O.box_muller16(0x00008000)                             # u2 = 1/2 -> angle pi
+    z = O.box_muller16(0x80000000)                             # u2 = 1/2 -> angle pi
     assert z[0] == pytest.approx(-rho_max, rel=1e-15) and abs(z[1]) < 1e-15
-    z = O.box_muller16(0xFFFF0000)                             # u1 = 1 - 2^-17: the smallest radius, never exactly 0
-    assert z[0] == pytest.approx(np.sqrt(-2 * np.log1p(-2.0**-17)), rel=1e-12) and z[0] > 0
-    z = O.box_muller16(0x7FFF0000)                             # u1 = (32767.5) 2^-16
-    assert z[0] == pytest.approx(np.sqrt(-2 * np.log(32767.5 / 65536)), rel=1e-15)
-    # the halves are not swapped: changing the low half rotates, changing the high half rescales
-    a, b, c = O.box_muller16(0x12340000), O.box_muller16(0x12344000), O.box_muller16(0x56780000)
-    assert np.hypot(*a) == pytest.approx(np.hypot(*b), rel=1e-15) and np.hypot(*a) != pytest.approx(np.hypot(*c), rel=1e-3)
-    assert a[1] == 0.0 and c[1] == 0.0 and abs(b[0]) < 1e-15
+    z = O.box_muller16(0x0000FFFF)                             # u1 = 1 - 2^-17: the smallest radius, never exactly 0
+    rho_min = np.sqrt(-2 * np.log1p(-2.0**-17))
+    assert np.hypot(*z) == pytest.approx(rho_min, rel=1e-12) and np.hypot(*z) > 0
+    assert np.arctan2(z[1], z[0]) == pytest.approx(2 * np.pi * (0xFFFF >> 9) / 2.0**23, rel=1e-9)   # the shared bits turn it
+    z = O.box_muller16(0x00007FFF)
+    assert np.hypot(*z) == pytest.approx(np.sqrt(-2 * np.log(32767.5 / 65536)), rel=1e-15)
+    # roles: the high half only rotates; bits 0..8 only rescale; bits 9..15 do both
+    a, b = O.box_muller16(0x00000123), O.box_muller16(0x56780123)
+    assert np.hypot(*a) == pytest.approx(np.hypot(*b), rel=1e-15) and a[1] == 0.0 and b[1] != 0.0
+    a, b = O.box_muller16(0x12340000), O.box_muller16(0x123401FF)
+    assert np.arctan2(a[1], a[0]) == pytest.approx(np.arctan2(b[1], b[0]), rel=1e-14) and np.hypot(*a) > np.hypot(*b)
+    a, b = O.box_muller16(0x12340000), O.box_muller16(0x12340200)
+    assert np.arctan2(b[1], b[0]) - np.arctan2(a[1], a[0]) == pytest.approx(2 * np.pi * 2.0**-23, rel=1e-6)
 
 
 def test_box_muller16_exact_lattice_moments():
-    """The 2^32 words map to a polar lattice; its moments are exact finite sums: E z^2 = 1 - 5.3e-6,
-    E z^4 = 3 - 2.1e-4, |z| <= 4.855 (the numbers DESIGN.md states for the 16-bit layout).  The radial sum is over
-    all 65536 radii; the angular sums over 65536 equally spaced angles are exact by symmetry
-    (mean cos^2 = 1/2, mean cos^4 = 3/8)."""
-    hi = np.arange(65536, dtype=np.uint64)
-    rho = np.array([np.hypot(*O.box_muller16(int(h) << 16)) for h in hi[::257]])       # sampled radii via the oracle
-    r2_all = -2.0 * np.log((hi.astype(np.float64) + 0.5) / 65536.0)
+    """The 2^32 words map to 2^32 points of a polar lattice; its moments are exact finite sums: E z^2 = 1 - 5.3e-6,
+    E z^4 = 3 - 2.1e-4, |z| <= 4.855 (the numbers DESIGN.md states).  The radial sum runs over all 65536 radii.  For
+    every radius the 65536 free angle bits give equally spaced angles over the full turn (offset by the shared bits), so
+    the angular means are exact by symmetry (mean cos = mean cos sin = 0, mean cos^2 = 1/2, mean cos^4 = 3/8)."""
+    lo = np.arange(65536, dtype=np.uint64)
+    rho = np.array([np.hypot(*O.box_muller16(int(h))) for h in lo[::257]])            # sampled radii via the oracle
+    r2_all = -2.0 * np.log((lo.astype(np.float64) + 0.5) / 65536.0)
     assert np.allclose(rho**2, r2_all[::257], rtol=1e-13)
     Ez2, Ez4 = r2_all.mean() / 2.0, (r2_all**2).mean() * 3.0 / 8.0
     assert Ez2 == pytest.approx(1.0 - 5.29e-6, abs=2e-8) and Ez4 == pytest.approx(3.0 - 2.106e-4, abs=1e-6)
     assert np.sqrt(r2_all.max()) == pytest.approx(4.8546, abs=1e-4)
-    lo = np.arange(0, 65536, 97)
-    ang = np.array([O.box_muller16(0x80000000 | int(l)) for l in lo])
-    r0 = np.sqrt(-2.0 * np.log(32768.5 / 65536.0))
-    assert np.allclose(ang[:, 0], r0 * np.cos(2 * np.pi * lo / 65536.0), atol=1e-15)
-    assert np.allclose(ang[:, 1], r0 * np.sin(2 * np.pi * lo / 65536.0), atol=1e-15)
+    # angles of one radius (low half fixed, all shared bits included): equally spaced, full turn, exact symmetry
+    for low in (0x0000, 0x8001, 0xFE37):
+        hi = np.arange(0, 65536, 64)
+        pts = np.array([O.box_muller16((int(h) << 16) | low) for h in hi])
+        r0 = np.sqrt(-2.0 * np.log((low + 0.5) / 65536.0))
+        th = 2 * np.pi * (((hi.astype(np.uint64) << 16) | low) >> 9).astype(np.float64) / 2.0**23
+        assert np.allclose(pts[:, 0], r0 * np.cos(th), atol=1e-14) and np.allclose(pts[:, 1], r0 * np.sin(th), atol=1e-14)
+        assert abs(pts[:, 0].mean()) < 1e-13 and abs((pts[:, 0] * pts[:, 1]).mean()) < 1e-13
+        assert (pts[:, 0] ** 2).mean() == pytest.approx(r0 * r0 / 2, rel=1e-12)
+    # distinct words -> distinct points (the shared bits lose nothing)
+    ws = np.random.default_rng(3).integers(0, 2**32, 4000)
+    assert len({tuple(O.box_muller16(int(w))) for w in ws}) == len(set(int(w) for w in ws))
 
 
 def test_normal_moments():
