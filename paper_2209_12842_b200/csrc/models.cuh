@@ -38,21 +38,25 @@ __device__ __forceinline__ void sincos_cw(float x, float& s, float& c) {
   s = (q & 2) ? -sn : sn;
 }
 
-// sin/cos of the yaw angle inside the K*M*T noisy rollouts: two-term Cody-Waite reduction to
-// [-pi, pi] (exact for |x| < pi, where j = 0) and MUFU.SIN / MUFU.COS (max abs error 2^-21.4 there).
-// Per Euler step that is <= dt v 4e-7 ~ 1e-7 m of position, below the half-ulp rounding (2.4e-7 m at
-// |X| in [4,8) m) that the fp32 position sum makes anyway; 7 instructions instead of 25.
+// sin/cos of the yaw angle inside the K*M*T noisy rollouts: MUFU.SIN / MUFU.COS on the angle itself (SASS: one
+// FMUL.RZ by 1/(2 pi) feeding both, the unit works in turns and drops whole turns exactly).  The rollout kernel
+// starts every realisation from a yaw reduced to [-pi, pi) (reduce_yaw below), so within the horizon |psi| stays at a
+// few turns at most: the multiply is then good to 2^-24 |psi| (<= 4e-7 rad per turn of winding) on top of the unit's
+// 2^-21.4 abs error -- per Euler step <= dt v 1e-6 ~ 2e-7 m of position, at the half-ulp (2.4e-7 m for |X| in [4,8) m)
+// that the fp32 position sum rounds by anyway; 3 instructions instead of 25 (round 1 reduced every step: 7).
 // The K*T nominal rollout and the plant keep sincos_cw.
-#ifndef RA_DYN_SINCOS_MUFU
-#define RA_DYN_SINCOS_MUFU 1
-#endif
 __device__ __forceinline__ void sincos_mufu(float x, float& s, float& c) {
-  const float jm = fmaf(x, 0.159154943f, 12582912.0f);
-  const float j = jm - 12582912.0f;
-  float r = fmaf(j, -6.28125f, x);
-  r = fmaf(j, -1.9353071795864769e-3f, r);
-  s = __sinf(r);
-  c = __cosf(r);
+  s = __sinf(x);
+  c = __cosf(x);
+}
+
+// psi = psi_rel + n 2 pi with psi_rel in [-pi, pi]: once per thread at rollout start; restore_yaw undoes it for output.
+__device__ __forceinline__ float reduce_yaw(float psi, float& n_turns) {
+  n_turns = rintf(psi * 0.159154943f);
+  return fmaf(n_turns, -1.9353071795864769e-3f, fmaf(n_turns, -6.28125f, psi));
+}
+__device__ __forceinline__ float restore_yaw(float psi_rel, float n_turns) {
+  return fmaf(n_turns, 6.28125f, fmaf(n_turns, 1.9353071795864769e-3f, psi_rel));
 }
 
 // atan2(y, x) for x > 0 (the single-track model floors vx at a positive value): one MUFU.RCP and
@@ -102,7 +106,7 @@ template <int DYN, bool FAST = false>
 __device__ __forceinline__ void dynamics_step(const Params& p, float (&x)[StateDim<DYN>::value],
                                               const float4 ce) {
   float s, c;
-  if constexpr (FAST && RA_DYN_SINCOS_MUFU) sincos_mufu(x[2], s, c);
+  if constexpr (FAST) sincos_mufu(x[2], s, c);
   else sincos_cw(x[2], s, c);
   if constexpr (DYN == DYN_BICYCLE) {
     const float dv = p.dt * x[3];

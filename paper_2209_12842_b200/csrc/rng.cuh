@@ -70,25 +70,25 @@ __device__ __forceinline__ void box_muller(uint32_t ra, uint32_t rb, float& z0, 
   z1 = rho * (neg ? -sn : sn);
 }
 
-// Box-Muller pair for the state-noise streams (K*M*T*n_x/2 evaluations per iteration) from ONE Philox word with 16 bits
-// per uniform: u1 = ((w >> 16) + 1/2) 2^-16 in (0,1), u2 = (w & 0xFFFF) 2^-16 in [0,1), both
-// exact in fp32; log2 / sqrt / sin / cos on the MUFU unit (lg2.approx, sqrt.approx, sin.approx, cos.approx).
-// Error budget: |dz| <= ~2e-6 |z| + 2e-7 / max(rho, 1e-3); scaled by sigma_w <= 0.05 that is
-// <= 1e-7 m per step, below the fp32 rounding of the positions themselves.
-//   u1: PRMT builds the float 1 + hi 2^-23 (bytes 0x3F80 : hi16), one FFMA scales it: (1 + hi 2^-23) 128 - (128 - 2^-17)
-//       = (hi + 1/2) 2^-16 exactly (only relative accuracy matters under the logarithm).
-//   angle = 2 pi (u2 - 1/2) in [-pi, pi) where MUFU.SIN/COS are most accurate; here the uniform must sit at the TOP of
-//       the mantissa (x = 1 + lo 2^-16 in [1,2)) so that 2 pi x - 3 pi cancels against 2 pi, not against 2 pi 2^7:
-//       one shift, one funnel shift, one FFMA.  The half-turn offset flips both signs.
+// Box-Muller pair for the state-noise streams (K*M*T*n_x/2 evaluations per iteration) from ONE Philox word
+// (DESIGN.md "RNG layout"): radius uniform u1 = ((w & 0xFFFF) + 1/2) 2^-16 in (0,1), angle uniform u2 = (w >> 9) 2^-23
+// in [0,1), both exact in fp32; log2 / sqrt / sin / cos on the MUFU unit (lg2.approx, sqrt.approx, sin.approx,
+// cos.approx).  Error budget: |dz| <= ~2e-6 |z| + 2e-7 / max(rho, 1e-3); scaled by
+// sigma_w <= 0.05 that is <= 1e-7 m per step, below the fp32 rounding of the positions themselves.
+//   u1: PRMT builds the float 1 + lo 2^-23 (bytes 0x3F80 : lo16), one FFMA scales it: (1 + lo 2^-23) 128 - (128 - 2^-17)
+//       = (lo + 1/2) 2^-16 exactly (only relative accuracy matters under the logarithm).
+//   angle = 2 pi (u2 - 1/2) in [-pi, pi) where MUFU.SIN/COS are most accurate: one funnel shift drops the top 23 bits
+//       of the word into the mantissa of x = 1 + u2 in [1,2), one FFMA forms 2 pi x - 3 pi (the cancellation is against
+//       2 pi, so the angle is good to 5e-7 rad).  The half-turn offset flips both signs.
 // Returns the UNSCALED pair (a0, a1) = sqrt(-log2 u1) (cos, sin)(angle); the normals are z = -sqrt(2 ln 2) a, and
 // that constant is folded into Params::wscale together with sigma_w, so the caller's x += wscale * a is one FFMA
-// per component.
+// per component.  12 instructions per pair: 2 on the ALU pipe, 6 on the FMA pipe, 4 MUFU.
 __device__ __forceinline__ void box_muller16_fast(uint32_t w, float& a0, float& a1) {
-  const float u1 = fmaf(__uint_as_float(__byte_perm(w, 0x3F800000u, 0x7632)), 128.0f, -127.99999237060546875f);
+  const float u1 = fmaf(__uint_as_float(__byte_perm(w, 0x3F800000u, 0x7610)), 128.0f, -127.99999237060546875f);
   float lg, s;
   asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lg) : "f"(u1));
   asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(s) : "f"(-lg));
-  const float th = fmaf(__uint_as_float(__funnelshift_r(w << 16, 0x7Fu, 9)), 6.283185307179586f, -9.42477796076938f);
+  const float th = fmaf(__uint_as_float(__funnelshift_r(w, 0x7Fu, 9)), 6.283185307179586f, -9.42477796076938f);
   a0 = s * __cosf(th);
   a1 = s * __sinf(th);
 }

@@ -201,7 +201,7 @@ __device__ __forceinline__ float warp_max_f32(float v) {
 // risk_p[0] once after the horizon loop.
 template <int RISK, int RC, int NX>
 __device__ __forceinline__ void risk_accumulate(const Params& p, const float4* circ_s, int n_circ_pad, int lane,
-                                                const MapFrame& mf, float x0X, float x0Y,
+                                                const MapFrame& mf, float x0X, float x0Y, float yaw_turns,
                                                 const float (&x)[RC][NX], float (&L)[RC]) {
   if constexpr (RISK == RISK_CIRCLES || RISK == RISK_NOMINAL) {
     // RISK_NOMINAL: l = q of the paper's racing costs: smooth part per lane, then the
@@ -268,7 +268,7 @@ __device__ __forceinline__ void risk_accumulate(const Params& p, const float4* c
       float val = 0.0f;
 #pragma unroll
       for (int i = 0; i < NX; ++i) val = (i == idx) ? x[r][i] : val;
-      val += (idx == 0) ? x0X : ((idx == 1) ? x0Y : 0.0f);
+      val = (idx == 2) ? restore_yaw(val, yaw_turns) : val + ((idx == 0) ? x0X : ((idx == 1) ? x0Y : 0.0f));
       L[r] = fmaf(p.risk_p[0], val, L[r]);
     }
   }
@@ -352,6 +352,9 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
 #pragma unroll
   for (int i = 2; i < NX; ++i) x_init[i] = x0g[i];
   if constexpr (DYN == DYN_SINGLE_TRACK) x_init[3] = fmaxf(x_init[3], p.dyn_p[6]);
+  // the models see the yaw only through sin / cos: integrate it from [-pi, pi) and add the whole turns back on output
+  float yaw_turns;
+  x_init[2] = reduce_yaw(x_init[2], yaw_turns);
 
   const uint32_t c3 = iteration_field(p, STREAM_W);
   const uint32_t kg = (uint32_t)(k + p.k_off);   // global sample index in the Philox counter
@@ -370,7 +373,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
     // x~_{t+1} = F(x~_t, u_t) + w_t   (6) PAPER.md:63 with w_t = wscale (.) a
     auto advance = [&](int t, const float (&a)[RC][NX]) {
       const float4 ce = ce_s[t];
-      risk_accumulate<RISK, RC, NX>(p, circ_s, n_circ_s, lane, mf, x0X, x0Y, x, L);
+      risk_accumulate<RISK, RC, NX>(p, circ_s, n_circ_s, lane, mf, x0X, x0Y, yaw_turns, x, L);
 #pragma unroll
       for (int r = 0; r < RC; ++r) {
         dynamics_step<DYN, true>(p, x[r], ce);
@@ -484,8 +487,9 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
         if (xT_out) {
           float* o = xT_out + ((size_t)k * p.M + m[r]) * NX;
           o[0] = x0X + x[r][0]; o[1] = x0Y + x[r][1];
+          o[2] = restore_yaw(x[r][2], yaw_turns);
 #pragma unroll
-          for (int i = 2; i < NX; ++i) o[i] = x[r][i];
+          for (int i = 3; i < NX; ++i) o[i] = x[r][i];
         }
       }
     }
