@@ -25,14 +25,31 @@ inline cudaError_t set_func_attr_once(std::atomic<int>* slot, int device, Kernel
   return e;
 }
 
+// Kernel launch with or without programmatic dependent launch (PDL): with `pdl` the kernel may be scheduled while
+// the previous kernel of the stream is still draining (after all its CTAs have executed griddepcontrol.launch_dependents
+// or exited) and must execute griddepcontrol.wait before it touches that kernel's results.  Works in eager streams and
+// under stream capture (the edge becomes a programmatic graph edge).
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_kernel(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream,
+                                 bool pdl, Args&&... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = pdl ? 1u : 0u;
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 // noise: NOISE_GAUSSIAN / NOISE_UNIFORM / NOISE_JUMP / 3 (materialised); rc in {1,2,4};
-// half: two samples per warp (M <= 16, rc must be 1).
+// half: two samples per warp (M <= 16, rc must be 1); pdl: launch as a programmatic dependent of the previous kernel.
 using RolloutLaunchFn = cudaError_t (*)(const Params& p, int noise, int rc, bool half, const float* d_x0,
-                                        float* d_L, float* d_xT, cudaStream_t stream);
+                                        float* d_L, float* d_xT, cudaStream_t stream, bool pdl);
 
 #define RA_DECLARE_ROLLOUT(D, R) \
   cudaError_t launch_rollout_##D##_##R(const Params& p, int noise, int rc, bool half, const float* d_x0, \
-                                       float* d_L, float* d_xT, cudaStream_t stream);
+                                       float* d_L, float* d_xT, cudaStream_t stream, bool pdl);
 RA_DECLARE_ROLLOUT(0, 0)
 RA_DECLARE_ROLLOUT(0, 1)
 RA_DECLARE_ROLLOUT(0, 2)

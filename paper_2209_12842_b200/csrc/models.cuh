@@ -91,7 +91,7 @@ __device__ __forceinline__ float4 control_effect(const Params& p, float u0, floa
   const float d = clampf(u0, p.u_min[0], p.u_max[0]);
   const float a = clampf(u1, p.u_min[1], p.u_max[1]);
   if constexpr (DYN == DYN_BICYCLE) {
-    return make_float4(p.dt * tanf(d) / p.dyn_p[0], p.dt * a, 0.0f, 0.0f);
+    return make_float4(p.dyn_q[0] * tanf(d), p.dt * a, 0.0f, 0.0f);   // dyn_q[0] = dt / L (host, fp64)
   } else {
     float s, c;
     sincos_cw(d, s, c);

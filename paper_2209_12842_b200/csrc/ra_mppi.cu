@@ -34,11 +34,13 @@ struct ra_mppi_ctx {
   float* d_cvar = nullptr;
   double* d_pen = nullptr;
   double* d_split = nullptr;   // [kMaxUpdateSplits][2+2T] partials of the update's sample ranges
+  unsigned int* d_done = nullptr;   // ticket counter of the update kernel's CTAs (its last CTA combines and re-arms it)
   float* d_w_mat = nullptr;
   LoopState* d_loop = nullptr;
   // closed-loop graph cache
   // host-buffer staging (ra_mppi_step_host) and optional kernel timing
   float* d_stage = nullptr;  // [nx + 2T]
+  bool pdl = true;     // programmatic dependent launch of the kernels that follow a kernel on the caller's stream
   bool timing = false;
   bool timed = false;  // ev_k0 / ev_k1 hold a rollout-kernel interval recorded outside a stream capture
   cudaEvent_t ev_k0 = nullptr, ev_k1 = nullptr;
@@ -53,7 +55,7 @@ struct ra_mppi_ctx {
 
 namespace {
 
-constexpr int kMaxUpdateSplits = 8;
+constexpr int kMaxUpdateSplits = 64;
 
 ra_status fail(ra_mppi_ctx* c, ra_status s, const std::string& msg) {
   if (c) c->err = msg;
@@ -297,11 +299,14 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
     p.carveout = need <= 57 * 1024 ? 25 : (need <= 114 * 1024 ? 50 : 100);
   }
   p.nx = cfg->dyn == RA_DYN_SINGLE_TRACK ? 6 : 4;
+  p.dyn = cfg->dyn; p.noise_kind = cfg->noise_kind;
   p.dt = cfg->dt;
   std::memcpy(p.dyn_p, cfg->dyn_p, sizeof p.dyn_p);
   if (cfg->dyn == RA_DYN_SINGLE_TRACK) {
     p.dyn_q[0] = (float)(1.0 / (double)cfg->dyn_p[0]);
     p.dyn_q[1] = (float)(1.0 / (double)cfg->dyn_p[1]);
+  } else {
+    p.dyn_q[0] = (float)((double)cfg->dt / (double)cfg->dyn_p[0]);   // dt / L of the yaw update
   }
   std::memcpy(p.nom_p, cfg->nom_p, sizeof p.nom_p);
   std::memcpy(p.risk_p, cfg->risk_p, sizeof p.risk_p);
@@ -335,10 +340,14 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
   if (dev_alloc(&c->d_u_raw, KT) != cudaSuccess || dev_alloc(&c->d_ce, KT) != cudaSuccess ||
       dev_alloc(&c->d_S, (size_t)cfg->K) != cudaSuccess || dev_alloc(&c->d_cvar, (size_t)cfg->K) != cudaSuccess ||
       dev_alloc(&c->d_pen, (size_t)cfg->K) != cudaSuccess || dev_alloc(&c->d_split, (size_t)kMaxUpdateSplits * (2 + 2 * cfg->T)) != cudaSuccess || dev_alloc(&c->d_loop, 1) != cudaSuccess ||
+      dev_alloc(&c->d_done, 1) != cudaSuccess ||
       dev_alloc(&c->d_stage, (size_t)(8 + 2 * cfg->T)) != cudaSuccess)
     return bail(RA_ENOMEM);
   p.u_raw = c->d_u_raw; p.ce = c->d_ce; p.S = c->d_S; p.cvar = c->d_cvar; p.pen = c->d_pen;
-  if (cudaMemset(c->d_loop, 0, sizeof(LoopState)) != cudaSuccess) return bail(RA_ECUDA);
+  if (cudaMemset(c->d_loop, 0, sizeof(LoopState)) != cudaSuccess || cudaMemset(c->d_done, 0, sizeof(unsigned int)) != cudaSuccess ||
+      cudaMemset(c->d_cvar, 0, (size_t)cfg->K * sizeof(float)) != cudaSuccess ||
+      cudaMemset(c->d_pen, 0, (size_t)cfg->K * sizeof(double)) != cudaSuccess)   // A = 0 steps never write them
+    return bail(RA_ECUDA);
   if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
       cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess)
@@ -365,7 +374,7 @@ ra_status ra_mppi_destroy(ra_mppi_ctx* c) {
   if (c->side) cudaStreamDestroy(c->side);
   if (c->ev_k0) cudaEventDestroy(c->ev_k0);
   if (c->ev_k1) cudaEventDestroy(c->ev_k1);
-  cudaFree(c->d_S); cudaFree(c->d_cvar); cudaFree(c->d_pen); cudaFree(c->d_split); cudaFree(c->d_w_mat); cudaFree(c->d_loop);
+  cudaFree(c->d_S); cudaFree(c->d_cvar); cudaFree(c->d_pen); cudaFree(c->d_split); cudaFree(c->d_w_mat); cudaFree(c->d_loop); cudaFree(c->d_done);
   delete c;
   return RA_OK;
 }
@@ -404,14 +413,14 @@ ra_status ra_mppi_query_counts(const ra_mppi_config* cfg, int32_t* h_k_tail, int
 namespace {
 
 cudaError_t launch_sample(const ra_mppi_ctx* c, const Params& p, const float* d_v, cudaStream_t s) {
-  const int grid = (p.K + kSampleKB - 1) / kSampleKB;
+  const dim3 grid((p.K + kSampleKB - 1) / kSampleKB, (p.T * kSampleKB + kSampleThreads - 1) / kSampleThreads);
   if (c->cfg.dyn == 0) sample_kernel<0><<<grid, kSampleThreads, 0, s>>>(p, d_v);
   else sample_kernel<1><<<grid, kSampleThreads, 0, s>>>(p, d_v);
-  return cudaGetLastError();
+  return cudaGetLastError();   // a plain launch: the first kernel of a step depends on everything before it
 }
 
 cudaError_t launch_nominal(const ra_mppi_ctx* c, const Params& p, const float* d_x0, const float* d_v,
-                           cudaStream_t s) {
+                           cudaStream_t s, bool pdl) {
   const int grid = (p.K + kNominalThreads - 1) / kNominalThreads;
   const int dyn = c->cfg.dyn, nom = c->cfg.nominal;
 #define RA_NOMK(D, N)                                                                                          \
@@ -420,12 +429,11 @@ cudaError_t launch_nominal(const ra_mppi_ctx* c, const Params& p, const float* d
     if (const cudaError_t e = set_func_attr_once(carveout_set, p.device, nominal_kernel<D, N>,                  \
                                                  cudaFuncAttributePreferredSharedMemoryCarveout, p.carveout))  \
       return e;                                                                                                \
-    nominal_kernel<D, N><<<grid, kNominalThreads, 0, s>>>(p, d_x0, d_v);                                       \
+    return launch_kernel(nominal_kernel<D, N>, dim3(grid), dim3(kNominalThreads), 0, s, pdl, p, d_x0, d_v);    \
   } while (0)
   if (dyn == 0) { if (nom == 0) RA_NOMK(0, 0); else if (nom == 1) RA_NOMK(0, 1); else RA_NOMK(0, 2); }
   else { if (nom == 0) RA_NOMK(1, 0); else if (nom == 1) RA_NOMK(1, 1); else RA_NOMK(1, 2); }
 #undef RA_NOMK
-  return cudaGetLastError();
 }
 
 template <int NX>
@@ -446,10 +454,9 @@ ra_status enqueue_costs(ra_mppi_ctx* c, const Params& p, const float* d_x0, cons
   // A = 0 is the baseline MPPI of section II: S~ = S by (14)-(16), so unless the caller
   // asks for the risk diagnostics the M noisy rollouts are not needed at all.
   if (c->cfg.A == 0.0f && !diagnostics) {
+    // cvar / pen stay zero: written once at create and by nothing else on this path
     RA_CUDA(c, launch_sample(c, p, d_v, s));
-    RA_CUDA(c, launch_nominal(c, p, d_x0, d_v, s));
-    RA_CUDA(c, cudaMemsetAsync(c->d_cvar, 0, (size_t)p.K * sizeof(float), s));
-    RA_CUDA(c, cudaMemsetAsync(c->d_pen, 0, (size_t)p.K * sizeof(double), s));
+    RA_CUDA(c, launch_nominal(c, p, d_x0, d_v, s, c->pdl));
     return RA_OK;
   }
   if (c->cfg.noise_mode == RA_NOISE_MATERIALISED)
@@ -458,58 +465,52 @@ ra_status enqueue_costs(ra_mppi_ctx* c, const Params& p, const float* d_x0, cons
   // fork: the K*T nominal rollout needs only the sampled controls and hides under the K*M*T noisy ones
   RA_CUDA(c, cudaEventRecord(c->ev_fork, s));
   RA_CUDA(c, cudaStreamWaitEvent(c->side, c->ev_fork, 0));
-  RA_CUDA(c, launch_nominal(c, p, d_x0, d_v, c->side));
+  RA_CUDA(c, launch_nominal(c, p, d_x0, d_v, c->side, false));
   RA_CUDA(c, cudaEventRecord(c->ev_join, c->side));
   // the timing pair is recorded on live streams only: an event recorded during capture has no elapsed time
   cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
   if (c->timing) RA_CUDA(c, cudaStreamIsCapturing(s, &cap));
   const bool time_it = c->timing && cap == cudaStreamCaptureStatusNone;
   if (time_it) RA_CUDA(c, cudaEventRecord(c->ev_k0, s));
-  RA_CUDA(c, c->rollout(p, c->noise_variant, c->rc, c->half, d_x0, d_L, d_xT, s));
+  // A plain launch, on purpose: as a programmatic dependent of the sampling kernel the rollout CTAs become resident
+  // before the nominal kernel on the side stream is released, fill every SM (2 CTAs x 256 threads x 128 registers) and
+  // push the nominal rollout behind the whole first wave -- measured on B200: C1 step 0.051 -> 0.068 ms, closed loop
+  // p50 0.152 -> 0.162 ms (profiles/r2).  The weights/update kernel behind it is the programmatic dependent.
+  RA_CUDA(c, c->rollout(p, c->noise_variant, c->rc, c->half, d_x0, d_L, d_xT, s, false));
   if (time_it) { RA_CUDA(c, cudaEventRecord(c->ev_k1, s)); c->timed = true; }
   RA_CUDA(c, cudaStreamWaitEvent(s, c->ev_join, 0));   // join
   return RA_OK;
 }
 
-// Alg.1 l.31: weights (17) and update (4) from the context scratch.  T CTAs alone leave most SMs idle, so the
-// samples are cut into ranges (enough for one CTA per SM, at least 2048 samples each) that are combined like the
-// shards of the K-sharded step.
+// Alg.1 l.31: weights (17) and update (4) from the context scratch.  One CTA per (horizon step, sample range); a range
+// is what one CTA caches in registers (kUpdateCached samples per thread), so the kernel is a single wave of small CTAs
+// whose ranges are combined like the shards of the K-sharded step.
 int update_splits(const ra_mppi_ctx* c) {
-  const Params& p = c->p;
-  const int by_sms = std::min(kMaxUpdateSplits, (c->n_sm + p.T - 1) / p.T);
-  return std::max(1, std::min(by_sms, p.K / 2048));
+  const int per_cta = kUpdateThreads * kUpdateCached;
+  return std::max(1, std::min(kMaxUpdateSplits, (c->p.K + per_cta - 1) / per_cta));
 }
 
-ra_status enqueue_update(ra_mppi_ctx* c, const Params& p, float* d_v_out, cudaStream_t s) {
-  const int splits = update_splits(c);
-  if (splits == 1) {
-    weights_update_kernel<double><<<p.T, kUpdateThreads, 0, s>>>(
-        p, p.S, p.pen, p.u_raw, 1LL, (long long)p.K, d_v_out, nullptr, nullptr, nullptr);
-  } else {
-    weights_update_kernel<double><<<dim3(p.T, splits), kUpdateThreads, 0, s>>>(
-        p, p.S, p.pen, p.u_raw, 1LL, (long long)p.K, nullptr, nullptr, nullptr, c->d_split);
-    RA_CUDA(c, cudaGetLastError());
-    combine_partials_kernel<<<1, 256, 0, s>>>(p, c->d_split, splits, d_v_out);
-  }
-  RA_CUDA(c, cudaGetLastError());
+ra_status enqueue_update(ra_mppi_ctx* c, const Params& p, float* d_v_out, cudaStream_t s, UpdateTail tail) {
+  // a programmatic dependent of the rollout kernel (of the nominal kernel when A = 0); the join with the side stream
+  // before it is a full dependency.  A timed step keeps plain launches.
+  RA_CUDA(c, launch_kernel(weights_update_kernel<double>, dim3(p.T, update_splits(c)), dim3(kUpdateThreads), 0, s,
+                           c->pdl && !c->timing, p, (const double*)p.S, (const double*)p.pen, (const float2*)p.u_raw, 1LL,
+                           (long long)p.K, d_v_out, (float*)nullptr, (float*)nullptr, c->d_split, c->d_done, tail));
   return RA_OK;
 }
 
 // The shard's share of (17)/(4) for the K-sharded step.
 ra_status enqueue_partial(ra_mppi_ctx* c, const Params& p, double* d_partial, cudaStream_t s) {
-  weights_update_kernel<double><<<p.T, kUpdateThreads, 0, s>>>(
-      p, p.S, p.pen, p.u_raw, 1LL, (long long)p.K, nullptr, nullptr, nullptr, d_partial);
-  RA_CUDA(c, cudaGetLastError());
+  RA_CUDA(c, launch_kernel(weights_update_kernel<double>, dim3(p.T, 1), dim3(kUpdateThreads), 0, s, c->pdl && !c->timing, p,
+                           (const double*)p.S, (const double*)p.pen, (const float2*)p.u_raw, 1LL, (long long)p.K,
+                           (float*)nullptr, (float*)nullptr, (float*)nullptr, d_partial, (unsigned int*)nullptr,
+                           UpdateTail{nullptr, nullptr, nullptr}));
   return RA_OK;
 }
 
-cudaError_t launch_plant(const ra_mppi_ctx* c, const Params& p, float* d_x0, float* d_v, float* d_u,
-                         float* d_log, LoopState* loop, cudaStream_t s) {
-  const int dyn = c->cfg.dyn, nk = c->cfg.noise_kind;
-#define RA_PLANT(D, N) plant_shift_kernel<D, N><<<1, 128, 0, s>>>(p, d_x0, d_v, d_u, d_log, loop)
-  if (dyn == 0) { if (nk == 0) RA_PLANT(0, 0); else if (nk == 1) RA_PLANT(0, 1); else RA_PLANT(0, 2); }
-  else { if (nk == 0) RA_PLANT(1, 0); else if (nk == 1) RA_PLANT(1, 1); else RA_PLANT(1, 2); }
-#undef RA_PLANT
+cudaError_t launch_plant(const Params& p, float* d_x0, float* d_v, float* d_u, float* d_log, LoopState* loop,
+                         cudaStream_t s) {
+  plant_shift_kernel<<<1, 128, 0, s>>>(p, d_x0, d_v, d_u, d_log, loop);
   return cudaGetLastError();
 }
 
@@ -531,7 +532,7 @@ ra_status ra_mppi_step(ra_mppi_ctx* c, const float* d_x0, float* d_v, uint64_t i
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const Params p = with_iteration(c, iteration);
   if (ra_status st = enqueue_costs(c, p, d_x0, d_v, nullptr, nullptr, s, false)) return st;
-  return enqueue_update(c, p, d_v, s);
+  return enqueue_update(c, p, d_v, s, UpdateTail{nullptr, nullptr, nullptr});
 }
 
 ra_status ra_mppi_step_partial(ra_mppi_ctx* c, const float* d_x0, const float* d_v, uint64_t iteration,
@@ -583,7 +584,8 @@ ra_status ra_mppi_weights_update(ra_mppi_ctx* c, const float* d_S_tilde, const f
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const Params p = with_iteration(c, 0);
   weights_update_kernel<float><<<p.T, kUpdateThreads, 0, s>>>(
-      p, d_S_tilde, nullptr, reinterpret_cast<const float2*>(d_u), (long long)p.T, 1LL, d_v_plus, d_w, d_stats, nullptr);
+      p, d_S_tilde, nullptr, reinterpret_cast<const float2*>(d_u), (long long)p.T, 1LL, d_v_plus, d_w, d_stats, nullptr,
+      nullptr, UpdateTail{nullptr, nullptr, nullptr});
   RA_CUDA(c, cudaGetLastError());
   return RA_OK;
 }
@@ -594,7 +596,7 @@ ra_status ra_mppi_plant_shift(ra_mppi_ctx* c, float* d_x0, float* d_v, float* d_
   if (!d_x0 || !d_v) return fail(c, RA_EINVAL, "null device pointer");
   RA_ON_DEVICE(c);
   const Params p = with_iteration(c, iteration);
-  RA_CUDA(c, launch_plant(c, p, d_x0, d_v, d_u_applied, nullptr, nullptr, static_cast<cudaStream_t>(stream)));
+  RA_CUDA(c, launch_plant(p, d_x0, d_v, d_u_applied, nullptr, nullptr, static_cast<cudaStream_t>(stream)));
   return RA_OK;
 }
 
@@ -650,9 +652,8 @@ ra_status ra_mppi_export_costs_f64(ra_mppi_ctx* c, double* d_S64, double* d_S_ti
 
 int32_t ra_mppi_launches_per_step(const ra_mppi_ctx* c) {
   if (!c) return 0;
-  const int update = update_splits(c) > 1 ? 2 : 1;   // weights/update (+ combine of its sample ranges)
-  if (c->cfg.A == 0.0f) return 2 + update;   // baseline MPPI: sampling, nominal rollout, weights/update
-  return 3 + update + (c->cfg.noise_mode == RA_NOISE_MATERIALISED ? 1 : 0);   // + noisy rollouts (+ noise generator)
+  if (c->cfg.A == 0.0f) return 3;   // baseline MPPI: sampling, nominal rollout, weights/update
+  return 4 + (c->cfg.noise_mode == RA_NOISE_MATERIALISED ? 1 : 0);   // + noisy rollouts (+ noise generator)
 }
 
 ra_status ra_mppi_philox(ra_mppi_ctx* c, const uint32_t* d_ctr, int32_t n, uint32_t* d_out, void* stream) {
@@ -710,7 +711,8 @@ ra_status ra_mppi_closed_loop(ra_mppi_ctx* c, float* d_x0, float* d_v, uint64_t 
   ra_status st = RA_OK;
   std::vector<cudaEvent_t> ev;
   do {
-    // (re)capture one iteration: step kernels + plant/shift, all reading the device-resident counter
+    // (re)capture one iteration: sampling, nominal || noisy rollouts, weights/update with the plant/shift tail, all reading
+    // the device-resident counter
     if (!c->graph_exec || c->g_x0 != d_x0 || c->g_v != d_v || c->g_log != d_log) {
       if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
       Params p = c->p;
@@ -719,8 +721,8 @@ ra_status ra_mppi_closed_loop(ra_mppi_ctx* c, float* d_x0, float* d_v, uint64_t 
       cudaGraph_t graph = nullptr;
       if (cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { st = fail(c, RA_ECUDA, "begin capture"); break; }
       st = enqueue_costs(c, p, d_x0, d_v, nullptr, nullptr, s, false);
-      if (st == RA_OK) st = enqueue_update(c, p, d_v, s);
-      if (st == RA_OK) st = cuda_fail(c, launch_plant(c, p, d_x0, d_v, nullptr, d_log, c->d_loop, s), "plant");
+      // the last CTA of the weights/update kernel applies v+_0 to the plant and shifts v: no separate kernels
+      if (st == RA_OK) st = enqueue_update(c, p, d_v, s, UpdateTail{d_x0, d_log, c->d_loop});
       cudaError_t e = cudaStreamEndCapture(s, &graph);
       if (st != RA_OK) { if (graph) cudaGraphDestroy(graph); break; }
       if (e != cudaSuccess) { st = cuda_fail(c, e, "end capture"); break; }

@@ -22,11 +22,12 @@ struct Params {
   int R_total;  // realisation slots of G lanes per sample = ceil(M / G)
   int wps;      // warps per control sample in the rollout kernel (1, 2, 4 or 8)
   int nx;
+  int dyn, noise_kind;  // model and noise kind (runtime copies for the kernels that are not templated on them)
   int carveout; // host only: preferred shared-memory carveout (percent) of the two concurrent rollout kernels
   int device;   // host only: CUDA device ordinal of the context (per-device kernel attributes)
   float dt;
   float dyn_p[8];
-  float dyn_q[2];   // single-track: 1/m, 1/Iz
+  float dyn_q[2];   // single-track: 1/m, 1/Iz; bicycle: dt/L
   float u_min[2], u_max[2];
   float sigma_eps[2];
   float ctrl_w[2];  // gamma / sigma_eps^2 (0 where sigma_eps == 0)   (3) PAPER.md:47
@@ -56,6 +57,12 @@ struct Params {
   const unsigned long long* d_iter;
   unsigned long long iter_imm;
 };
+
+// Programmatic dependent launch (launchers.h: launch_kernel): a kernel started early waits here for the previous
+// kernel of its stream to finish and flush; a kernel lets its successor start being scheduled once every CTA has
+// passed launch_dependents.  Both are no-ops for plain launches.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
 
 __device__ __forceinline__ uint32_t iteration_field(const Params& p, uint32_t stream) {
   const unsigned long long it = p.d_iter ? *p.d_iter : p.iter_imm;

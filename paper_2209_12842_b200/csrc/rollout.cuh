@@ -29,26 +29,25 @@ constexpr int NOISE_MATERIALISED = 3;  // rollout-kernel variant that reads w fr
 // Parallel over (k, t): Philox + accurate Box-Muller + tan / sincos of the clamped control, once per
 // (k, t).  Writes u_raw[T][K] (for the update (4)) and the control effects ce[K][T] (for both rollouts).
 // ---------------------------------------------------------------------------------------
-constexpr int kSampleThreads = 128;
-constexpr int kSampleKB = 16;  // control samples per CTA
+constexpr int kSampleThreads = 256;
+constexpr int kSampleKB = 16;  // control samples per CTA row: 16 consecutive k make one 128-byte segment of u_raw[t][.]
 
+// One (k, t) draw per thread (the kernel is a dependent chain -- Philox, log, sqrt, tan -- so it is laid out for
+// latency, not for work per thread): blockIdx.x picks 16 consecutive samples, blockIdx.y a chunk of their T * 16 draws.
 template <int DYN>
 __global__ void __launch_bounds__(kSampleThreads) sample_kernel(const __grid_constant__ Params p,
                                                                 const float* __restrict__ v) {
-  const int k0 = blockIdx.x * kSampleKB;
-  const uint32_t c3 = iteration_field(p, STREAM_EPS);
-  for (int idx = threadIdx.x; idx < p.T * kSampleKB; idx += blockDim.x) {
-    const int t = idx / kSampleKB, kl = idx % kSampleKB, k = k0 + kl;
-    if (k >= p.K) continue;
-    const uint4 r = philox4x32_10((uint32_t)(k + p.k_off), 0u, (uint32_t)t, c3, p.rk);
-    float z0, z1;
-    box_muller(r.x, r.y, z0, z1);
-    const bool with_mean = k + p.k_off < p.K0;
-    const float u0 = fmaf(p.sigma_eps[0], z0, with_mean ? __ldg(v + 2 * t) : 0.0f);
-    const float u1 = fmaf(p.sigma_eps[1], z1, with_mean ? __ldg(v + 2 * t + 1) : 0.0f);
-    p.u_raw[(size_t)t * p.K + k] = make_float2(u0, u1);
-    p.ce[(size_t)k * p.T + t] = control_effect<DYN>(p, u0, u1);
-  }
+  const int idx = blockIdx.y * kSampleThreads + threadIdx.x;
+  const int t = idx / kSampleKB, k = blockIdx.x * kSampleKB + idx % kSampleKB;
+  if (t >= p.T || k >= p.K) return;
+  const uint4 r = philox4x32_10((uint32_t)(k + p.k_off), 0u, (uint32_t)t, iteration_field(p, STREAM_EPS), p.rk);
+  float z0, z1;
+  box_muller(r.x, r.y, z0, z1);
+  const bool with_mean = k + p.k_off < p.K0;
+  const float u0 = fmaf(p.sigma_eps[0], z0, with_mean ? __ldg(v + 2 * t) : 0.0f);
+  const float u1 = fmaf(p.sigma_eps[1], z1, with_mean ? __ldg(v + 2 * t + 1) : 0.0f);
+  p.u_raw[(size_t)t * p.K + k] = make_float2(u0, u1);
+  p.ce[(size_t)k * p.T + t] = control_effect<DYN>(p, u0, u1);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -67,6 +66,8 @@ __global__ void __launch_bounds__(kNominalThreads) nominal_kernel(const __grid_c
                                                                   const float* __restrict__ x0g,
                                                                   const float* __restrict__ v) {
   constexpr int NX = StateDim<DYN>::value;
+  pdl_launch_dependents();
+  pdl_wait();                // baseline-MPPI steps (A = 0) launch this kernel as a dependent of the sampling kernel
   const int k = blockIdx.x * kNominalThreads + threadIdx.x;
   if (k >= p.K) return;
   const float x0X = x0g[0], x0Y = x0g[1];
@@ -313,6 +314,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
   float4* ce_all = smem4 + n_circ_s;                                   // [ce_slots][T] control effects
   uint32_t* keys_all = reinterpret_cast<uint32_t*>(ce_all + (size_t)ce_slots * p.T);
 
+  pdl_launch_dependents();   // the weights/update kernel may be scheduled behind the last wave of this grid
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const float x0X = x0g[0], x0Y = x0g[1];
   if constexpr (kUsesCircles) {

@@ -14,7 +14,7 @@ namespace ra {
 namespace {
 
 template <int NOISE, int RC, bool HALF>
-cudaError_t launch(const Params& p, const float* d_x0, float* d_L, float* d_xT, cudaStream_t stream) {
+cudaError_t launch(const Params& p, const float* d_x0, float* d_L, float* d_xT, cudaStream_t stream, bool pdl) {
   const int samples_per_cta = HALF ? 2 * kRolloutWarps : kRolloutWarps / p.wps;
   const int grid = (p.K + samples_per_cta - 1) / samples_per_cta;
   const int ce_slots = HALF ? 2 * kRolloutWarps : kRolloutWarps / p.wps;
@@ -31,18 +31,17 @@ cudaError_t launch(const Params& p, const float* d_x0, float* d_L, float* d_xT, 
   static std::atomic<int> carveout_set[kMaxDevices];
   if (const cudaError_t e = set_func_attr_once(carveout_set, p.device, kernel, cudaFuncAttributePreferredSharedMemoryCarveout, p.carveout))
     return e;
-  kernel<<<grid, kRolloutThreads, smem, stream>>>(p, d_x0, d_L, d_xT);
-  return cudaGetLastError();
+  return launch_kernel(kernel, dim3(grid), dim3(kRolloutThreads), smem, stream, pdl, p, d_x0, d_L, d_xT);
 }
 
 template <int NOISE>
 cudaError_t launch_noise(const Params& p, int rc, bool half, const float* d_x0, float* d_L, float* d_xT,
-                         cudaStream_t stream) {
-  if (half) return launch<NOISE, 1, true>(p, d_x0, d_L, d_xT, stream);
+                         cudaStream_t stream, bool pdl) {
+  if (half) return launch<NOISE, 1, true>(p, d_x0, d_L, d_xT, stream, pdl);
   switch (rc) {
-    case 1: return launch<NOISE, 1, false>(p, d_x0, d_L, d_xT, stream);
-    case 2: return launch<NOISE, 2, false>(p, d_x0, d_L, d_xT, stream);
-    case 4: return launch<NOISE, 4, false>(p, d_x0, d_L, d_xT, stream);
+    case 1: return launch<NOISE, 1, false>(p, d_x0, d_L, d_xT, stream, pdl);
+    case 2: return launch<NOISE, 2, false>(p, d_x0, d_L, d_xT, stream, pdl);
+    case 4: return launch<NOISE, 4, false>(p, d_x0, d_L, d_xT, stream, pdl);
     default: return cudaErrorInvalidValue;
   }
 }
@@ -54,12 +53,12 @@ cudaError_t launch_noise(const Params& p, int rc, bool half, const float* d_x0, 
 
 cudaError_t RA_CAT(RA_INST_DYN, RA_INST_RISK)(const Params& p, int noise, int rc, bool half,
                                                const float* d_x0, float* d_L, float* d_xT,
-                                               cudaStream_t stream) {
+                                               cudaStream_t stream, bool pdl) {
   switch (noise) {
-    case NOISE_GAUSSIAN: return launch_noise<NOISE_GAUSSIAN>(p, rc, half, d_x0, d_L, d_xT, stream);
-    case NOISE_UNIFORM: return launch_noise<NOISE_UNIFORM>(p, rc, half, d_x0, d_L, d_xT, stream);
-    case NOISE_JUMP: return launch_noise<NOISE_JUMP>(p, rc, half, d_x0, d_L, d_xT, stream);
-    case NOISE_MATERIALISED: return launch_noise<NOISE_MATERIALISED>(p, rc, half, d_x0, d_L, d_xT, stream);
+    case NOISE_GAUSSIAN: return launch_noise<NOISE_GAUSSIAN>(p, rc, half, d_x0, d_L, d_xT, stream, pdl);
+    case NOISE_UNIFORM: return launch_noise<NOISE_UNIFORM>(p, rc, half, d_x0, d_L, d_xT, stream, pdl);
+    case NOISE_JUMP: return launch_noise<NOISE_JUMP>(p, rc, half, d_x0, d_L, d_xT, stream, pdl);
+    case NOISE_MATERIALISED: return launch_noise<NOISE_MATERIALISED>(p, rc, half, d_x0, d_L, d_xT, stream, pdl);
     default: return cudaErrorInvalidValue;
   }
 }

@@ -6,7 +6,8 @@
 
 namespace ra {
 
-constexpr int kUpdateThreads = 1024;
+constexpr int kUpdateThreads = 256;   // small CTAs: 64 registers each (samples cached in registers), several per SM, one wave
+constexpr int kUpdateCached = 8;      // samples per thread held in registers across the min reduction
 
 template <typename T, typename Op>
 __device__ __forceinline__ T block_reduce(T v, T* smem, Op op, T identity) {
@@ -23,14 +24,119 @@ __device__ __forceinline__ T block_reduce(T v, T* smem, Op op, T identity) {
   return v;  // every thread holds the result
 }
 
+// Device-resident loop state for graph replay.
+struct LoopState {
+  unsigned long long iter;     // Philox iteration index of the next step
+  unsigned long long log_idx;  // row of the closed-loop log to write next
+};
+
+// ---------------------------------------------------------------------------------------
+// A10.  ExecuteCommand(v+_0) on the simulated plant (the disturbed dynamics (6) with the PLANT stream),
+// v <- shift(v+) (Alg.1 l.32-33 PAPER.md:218-220 + BASELINE config 4's warm-start shift), iteration++.
+// Executed by ONE CTA, all of its threads (it synchronises): the body of plant_shift_kernel and the tail of the
+// weights/update kernel inside the captured closed loop, so both give the same bits.
+// ---------------------------------------------------------------------------------------
+template <int DYN, int NOISE>
+__device__ __forceinline__ void plant_shift_cta(const Params& p, float* x0g, float* v, float* u_applied, float* log,
+                                                LoopState* loop) {
+  constexpr int NX = StateDim<DYN>::value;
+  // shift: read everything, then write (T <= RA_MAX_T = 128 <= 2 * blockDim for every caller)
+  float2 nxt[2];
+  float2* v2 = reinterpret_cast<float2*>(v);
+  int cnt = 0;
+  for (int t = threadIdx.x; t < p.T && cnt < 2; t += blockDim.x) nxt[cnt++] = v2[min(t + 1, p.T - 1)];
+  const float2 v0 = v2[0];
+  __syncthreads();
+  cnt = 0;
+  for (int t = threadIdx.x; t < p.T && cnt < 2; t += blockDim.x) v2[t] = nxt[cnt++];
+
+  if (threadIdx.x == 0) {
+    float x[NX];
+    const float x0X = x0g[0], x0Y = x0g[1];
+    x[0] = 0.0f; x[1] = 0.0f;
+#pragma unroll
+    for (int i = 2; i < NX; ++i) x[i] = x0g[i];
+    if constexpr (DYN == DYN_SINGLE_TRACK) x[3] = fmaxf(x[3], p.dyn_p[6]);
+    const float4 ce = control_effect<DYN>(p, v0.x, v0.y);
+    float z[NX];
+    state_noise<NX, NOISE>(p, 0u, 0u, 0u, iteration_field(p, STREAM_PLANT), z);
+    dynamics_step<DYN>(p, x, ce);
+#pragma unroll
+    for (int i = 0; i < NX; ++i) x[i] = fmaf(p.wscale[i], z[i], x[i]);
+    if constexpr (DYN == DYN_SINGLE_TRACK) x[3] = fmaxf(x[3], p.dyn_p[6]);
+    x[0] += x0X; x[1] += x0Y;
+#pragma unroll
+    for (int i = 0; i < NX; ++i) x0g[i] = x[i];
+    if (u_applied) { u_applied[0] = v0.x; u_applied[1] = v0.y; }
+    if (log) {
+      float* row = log + (loop ? loop->log_idx : 0ull) * (NX + 2);
+#pragma unroll
+      for (int i = 0; i < NX; ++i) row[i] = x[i];
+      row[NX] = v0.x; row[NX + 1] = v0.y;
+    }
+    if (loop) { loop->iter += 1ull; loop->log_idx += 1ull; }
+  }
+}
+
+// the same, picking the (model, noise kind) instantiation at run time
+__device__ __noinline__ void plant_shift_any(const Params& p, float* x0g, float* v, float* u_applied, float* log,
+                                             LoopState* loop) {
+  switch (p.dyn * 3 + p.noise_kind) {
+    case 0: plant_shift_cta<0, 0>(p, x0g, v, u_applied, log, loop); break;
+    case 1: plant_shift_cta<0, 1>(p, x0g, v, u_applied, log, loop); break;
+    case 2: plant_shift_cta<0, 2>(p, x0g, v, u_applied, log, loop); break;
+    case 3: plant_shift_cta<1, 0>(p, x0g, v, u_applied, log, loop); break;
+    case 4: plant_shift_cta<1, 1>(p, x0g, v, u_applied, log, loop); break;
+    default: plant_shift_cta<1, 2>(p, x0g, v, u_applied, log, loop); break;
+  }
+}
+
+__global__ void __launch_bounds__(128) plant_shift_kernel(const __grid_constant__ Params p, float* x0g, float* v,
+                                                          float* u_applied, float* log, LoopState* loop) {
+  plant_shift_any(p, x0g, v, u_applied, log, loop);
+}
+
+// Exchange step of (17)/(4) over sample ranges or shards: partials [n][2+2T] = {beta_g, Z_g, N_g[T][2]}
+// -> v+ = clamp(sum_g s_g N_g / sum_g s_g Z_g), s_g = exp(-(beta_g - beta)/lambda), beta = min_g beta_g,
+// which is (17)/(4) over the union of the parts (factor exp(-(beta_g-beta)/lambda) out of every w~_k).
+// Fixed summation order over g => every rank / every replay computes bitwise the same v+; fp64 until the final
+// divide.  Executed by one CTA, thread = (t, i).  The partials may have been written by other CTAs of the running
+// grid, hence the L2 loads (__ldcg).
+__device__ __forceinline__ void combine_partials_cta(const Params& p, const double* partials, int n_parts,
+                                                     float* v_out) {
+  const int stride = 2 + 2 * p.T;
+  double beta = INFINITY;
+  for (int g = 0; g < n_parts; ++g) beta = fmin(beta, __ldcg(partials + (size_t)g * stride));
+  for (int j = threadIdx.x; j < 2 * p.T; j += blockDim.x) {
+    double Z = 0.0, n = 0.0;
+    for (int g = 0; g < n_parts; ++g) {
+      const double* pg = partials + (size_t)g * stride;
+      const double s = (double)exp2f((float)(__ldcg(pg) - beta) * p.neg_log2e_over_lambda);
+      Z = fma(s, __ldcg(pg + 1), Z);
+      n = fma(s, __ldcg(pg + 2 + j), n);
+    }
+    v_out[j] = clampf((float)(n / Z), p.u_min[j & 1], p.u_max[j & 1]);
+  }
+}
+
+__global__ void combine_partials_kernel(const __grid_constant__ Params p, const double* __restrict__ partials,
+                                        int n_parts, float* __restrict__ v_out) {
+  combine_partials_cta(p, partials, n_parts, v_out);
+}
+
 // ---------------------------------------------------------------------------------------
 // A8 + A9.  One CTA per (horizon step t, sample range blockIdx.y of gridDim.y).  Each CTA recomputes
 // beta~ = min_k S~_k over its range (values from L2), then w~_k = exp(-(S~_k - beta~)/lambda), Z = sum w~, and
-// v+_t = clamp(sum_k w~_k u^k_t / Z)   (17) PAPER.md:134, (5) :55, (4) :51.  With gridDim.y = 1 the CTA writes
-// v+ itself; with `partial` set it writes its range's {beta, Z, N_t} for combine_partials_kernel (the same
-// exchange the K-sharded step uses), which lets T * gridDim.y CTAs cover all SMs when T alone does not.
-// u is addressed as u[k*su_k + t*su_t] so both the internal [T][K] scratch and a caller's
-// [K][T] array work.  Reduction order is fixed => bitwise reproducible.
+// N_t = sum_k w~_k u^k_t   (17) PAPER.md:134, (5) :55, (4) :51.  T CTAs alone leave most SMs idle, so the samples are
+// cut into gridDim.y ranges.  Three uses:
+//   * ra_mppi_step: the CTA writes its range's {beta, Z, N_t} into `partial` (context scratch); the LAST CTA of the grid
+//     to finish (an atomic ticket in *done) combines the ranges into v+ = clamp(N / Z) -- in a fixed order, so the
+//     result does not depend on which CTA that was -- and, inside the captured closed loop (tail.x0g != nullptr), goes on
+//     to apply v+_0 to the plant and shift v (A10): one kernel instead of three on the latency path of an iteration;
+//   * ra_mppi_step_partial (K-sharded step): `partial` is the caller's, done == nullptr: the CTA just writes its share;
+//   * ra_mppi_weights_update (caller's S~ and u, gridDim.y = 1, partial == nullptr): the CTA writes v+_t itself.
+// u is addressed as u[k*su_k + t*su_t] so both the internal [T][K] scratch and a caller's [K][T] array work.
+// Reduction order is fixed => bitwise reproducible.
 // ---------------------------------------------------------------------------------------
 // S~_k (16): the caller's array (ST = float), or S + J_C from the context scratch (ST = double, pen != nullptr)
 template <typename ST>
@@ -39,26 +145,60 @@ __device__ __forceinline__ ST s_tilde_at(const ST* __restrict__ S, const double*
   else return S[k];
 }
 
+struct UpdateTail {          // closed-loop tail of the update kernel (all null outside ra_mppi_closed_loop)
+  float* x0g;                // [n_x] state, advanced by the plant
+  float* log;                // closed-loop log or nullptr
+  LoopState* loop;
+};
+
 template <typename ST>
 __global__ void __launch_bounds__(kUpdateThreads)
 weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S_tilde,
                       const double* __restrict__ pen, const float2* __restrict__ u, long long su_k, long long su_t,
-                      float* __restrict__ v_out, float* __restrict__ w_out,
-                      float* __restrict__ stats, double* __restrict__ partial) {
+                      float* v_out, float* __restrict__ w_out, float* __restrict__ stats, double* partial,
+                      unsigned int* done, UpdateTail tail) {
   __shared__ ST red_s[32];
   __shared__ double red_f[96];
+  __shared__ bool is_last;
+  pdl_wait();   // launched as a programmatic dependent of the rollout kernel: its costs are read from here on
   const int t = blockIdx.x;
   const int k_chunk = (p.K + gridDim.y - 1) / gridDim.y;
   const int k_begin = blockIdx.y * k_chunk, k_end = min(p.K, k_begin + k_chunk);
-  if (partial) partial += (size_t)blockIdx.y * (2 + 2 * p.T);
+  double* my_partial = partial ? partial + (size_t)blockIdx.y * (2 + 2 * p.T) : nullptr;
+  // The kernel is a chain of memory round trips, so each thread fetches the costs AND the controls of its first
+  // kCached samples in one go and keeps them in registers across the min; the host cuts K into ranges of at most
+  // kCached * blockDim samples, and anything beyond (a caller's single range) takes the two-pass route through L1.
+  constexpr int kCached = kUpdateCached;
+  ST sc[kCached];
+  float2 uc[kCached];
   ST bmin = (ST)INFINITY;
-  for (int k = k_begin + threadIdx.x; k < k_end; k += blockDim.x) bmin = min(bmin, s_tilde_at<ST>(S_tilde, pen, k));
+#pragma unroll
+  for (int j = 0; j < kCached; ++j) {
+    const int k = k_begin + threadIdx.x + j * (int)blockDim.x;
+    sc[j] = (ST)INFINITY;
+    uc[j] = make_float2(0.0f, 0.0f);
+    if (k < k_end) {
+      sc[j] = s_tilde_at<ST>(S_tilde, pen, k);
+      uc[j] = __ldg(u + (long long)k * su_k + (long long)t * su_t);
+    }
+    bmin = min(bmin, sc[j]);
+  }
+  const int k_rest = k_begin + kCached * (int)blockDim.x;
+  for (int k = k_rest + threadIdx.x; k < k_end; k += blockDim.x) bmin = min(bmin, s_tilde_at<ST>(S_tilde, pen, k));
   const ST beta = block_reduce<ST>(bmin, red_s, [](ST a, ST b) { return a < b ? a : b; }, (ST)INFINITY);
 
   // Z and the two numerators are summed in fp64: with soft weights (ESS >> 1) and K = 65536 an fp32 sum would
-  // spend a visible part of the 1e-4 budget of v+ on its own rounding.  Each w~ is an fp32 exp2 of an fp32 argument.
+  // spend a visible part of the 1e-4 budget of v+ on its own rounding.  Each w~ is an fp32 exp2 of an fp32 argument
+  // (an empty slot holds S~ = +inf, hence weight exactly 0).
   double Z = 0.0, n0 = 0.0, n1 = 0.0;
-  for (int k = k_begin + threadIdx.x; k < k_end; k += blockDim.x) {
+#pragma unroll
+  for (int j = 0; j < kCached; ++j) {
+    const float w = exp2f((float)(sc[j] - beta) * p.neg_log2e_over_lambda);
+    Z += (double)w;
+    n0 = fma((double)w, (double)uc[j].x, n0);
+    n1 = fma((double)w, (double)uc[j].y, n1);
+  }
+  for (int k = k_rest + threadIdx.x; k < k_end; k += blockDim.x) {
     const float w = exp2f((float)(s_tilde_at<ST>(S_tilde, pen, k) - beta) * p.neg_log2e_over_lambda);
     const float2 uk = __ldg(u + (long long)k * su_k + (long long)t * su_t);
     Z += (double)w;
@@ -86,11 +226,29 @@ weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S
       n1 += __shfl_xor_sync(0xFFFFFFFFu, n1, o);
     }
   }
-  if (partial) {   // K-sharded step: the shard's unnormalised share {beta_g, Z_g, N_g[T][2]}
+  // one range, no closed-loop tail: this CTA owns v+_t outright, no exchange needed
+  if (my_partial && done && gridDim.y == 1 && !tail.x0g) my_partial = nullptr;
+  if (my_partial) {   // the range's / shard's unnormalised share {beta_g, Z_g, N_g[T][2]}
     if (threadIdx.x == 0) {
-      if (t == 0) { partial[0] = (double)beta; partial[1] = Z; }
-      partial[2 + 2 * t] = n0;
-      partial[3 + 2 * t] = n1;
+      if (t == 0) { my_partial[0] = (double)beta; my_partial[1] = Z; }
+      my_partial[2 + 2 * t] = n0;
+      my_partial[3 + 2 * t] = n1;
+    }
+    if (!done) return;
+    // last CTA to finish combines: its ticket is the last one, so every other CTA's partials are in L2
+    if (threadIdx.x == 0) {
+      __threadfence();
+      const unsigned int ticket = atomicAdd(done, 1u);
+      is_last = ticket == gridDim.x * gridDim.y - 1u;
+      if (is_last) *done = 0u;   // armed for the next launch
+      __threadfence();
+    }
+    __syncthreads();
+    if (!is_last) return;
+    combine_partials_cta(p, partial, (int)gridDim.y, v_out);
+    if (tail.x0g) {
+      __syncthreads();           // v+ complete before it is applied and shifted
+      plant_shift_any(p, tail.x0g, v_out, nullptr, tail.log, tail.loop);
     }
     return;
   }
@@ -103,28 +261,6 @@ weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S
     const float invZ = (float)(1.0 / Z);
     for (int k = threadIdx.x; k < p.K; k += blockDim.x)
       w_out[k] = exp2f((float)(s_tilde_at<ST>(S_tilde, pen, k) - beta) * p.neg_log2e_over_lambda) * invZ;
-  }
-}
-
-// Exchange step of the K-sharded iteration: partials [n][2+2T] = {beta_g, Z_g, N_g[T][2]} of the shards
-// -> v+ = clamp(sum_g s_g N_g / sum_g s_g Z_g), s_g = exp(-(beta_g - beta)/lambda), beta = min_g beta_g,
-// which is (17)/(4) over the union of the shards (factor exp(-(beta_g-beta)/lambda) out of every w~_k).
-// Fixed summation order over g => every rank computes bitwise the same v+; fp64 until the final divide.
-// One CTA, thread = (t, i).
-__global__ void combine_partials_kernel(const __grid_constant__ Params p, const double* __restrict__ partials,
-                                        int n_parts, float* __restrict__ v_out) {
-  const int stride = 2 + 2 * p.T;
-  double beta = INFINITY;
-  for (int g = 0; g < n_parts; ++g) beta = fmin(beta, partials[(size_t)g * stride]);
-  for (int j = threadIdx.x; j < 2 * p.T; j += blockDim.x) {
-    double Z = 0.0, n = 0.0;
-    for (int g = 0; g < n_parts; ++g) {
-      const double* pg = partials + (size_t)g * stride;
-      const double s = (double)exp2f((float)(pg[0] - beta) * p.neg_log2e_over_lambda);
-      Z = fma(s, pg[1], Z);
-      n = fma(s, pg[2 + j], n);
-    }
-    v_out[j] = clampf((float)(n / Z), p.u_min[j & 1], p.u_max[j & 1]);
   }
 }
 
@@ -154,60 +290,6 @@ __global__ void export_costs_f64_kernel(const __grid_constant__ Params p, double
   if (k >= p.K) return;
   if (S) S[k] = p.S[k];
   if (S_tilde) S_tilde[k] = p.S[k] + p.pen[k];
-}
-
-// Device-resident loop state for graph replay.
-struct LoopState {
-  unsigned long long iter;     // Philox iteration index of the next step
-  unsigned long long log_idx;  // row of the closed-loop log to write next
-};
-
-// ---------------------------------------------------------------------------------------
-// A10.  ExecuteCommand(v+_0) on the simulated plant (the disturbed dynamics (6) with the
-// PLANT stream), v <- shift(v+) (Alg.1 l.32-33 PAPER.md:218-220 + BASELINE config 4's
-// warm-start shift), iteration++.  One CTA.
-// ---------------------------------------------------------------------------------------
-template <int DYN, int NOISE>
-__global__ void __launch_bounds__(128) plant_shift_kernel(const __grid_constant__ Params p, float* x0g,
-                                                          float* v, float* u_applied, float* log,
-                                                          LoopState* loop) {
-  constexpr int NX = StateDim<DYN>::value;
-  // shift: read everything, then write
-  float2 nxt[2];
-  float2* v2 = reinterpret_cast<float2*>(v);
-  int cnt = 0;
-  for (int t = threadIdx.x; t < p.T; t += blockDim.x) nxt[cnt++] = v2[min(t + 1, p.T - 1)];
-  const float2 v0 = v2[0];
-  __syncthreads();
-  cnt = 0;
-  for (int t = threadIdx.x; t < p.T; t += blockDim.x) v2[t] = nxt[cnt++];
-
-  if (threadIdx.x == 0) {
-    float x[NX];
-    const float x0X = x0g[0], x0Y = x0g[1];
-    x[0] = 0.0f; x[1] = 0.0f;
-#pragma unroll
-    for (int i = 2; i < NX; ++i) x[i] = x0g[i];
-    if constexpr (DYN == DYN_SINGLE_TRACK) x[3] = fmaxf(x[3], p.dyn_p[6]);
-    const float4 ce = control_effect<DYN>(p, v0.x, v0.y);
-    float z[NX];
-    state_noise<NX, NOISE>(p, 0u, 0u, 0u, iteration_field(p, STREAM_PLANT), z);
-    dynamics_step<DYN>(p, x, ce);
-#pragma unroll
-    for (int i = 0; i < NX; ++i) x[i] = fmaf(p.wscale[i], z[i], x[i]);
-    if constexpr (DYN == DYN_SINGLE_TRACK) x[3] = fmaxf(x[3], p.dyn_p[6]);
-    x[0] += x0X; x[1] += x0Y;
-#pragma unroll
-    for (int i = 0; i < NX; ++i) x0g[i] = x[i];
-    if (u_applied) { u_applied[0] = v0.x; u_applied[1] = v0.y; }
-    if (log) {
-      float* row = log + (loop ? loop->log_idx : 0ull) * (NX + 2);
-#pragma unroll
-      for (int i = 0; i < NX; ++i) row[i] = x[i];
-      row[NX] = v0.x; row[NX + 1] = v0.y;
-    }
-    if (loop) { loop->iter += 1ull; loop->log_idx += 1ull; }
-  }
 }
 
 // Parity hooks: raw Philox words and state-noise draws exactly as the rollout kernel makes them.
