@@ -29,20 +29,71 @@ from paper_2209_12842_b200 import workloads as W  # noqa: E402
 METRIC = "noisy_state_steps_per_s"
 UNIT = "state-steps/s"
 
-# Algorithmic lane-operations per noisy state-step ("What bounds it"): the instructions
-# the method itself needs in its leanest known formulation, one per FP32-lane slot (FFMA = 1).
-#   Philox4x32-10 call 40 (20 mul-wide + 20 xor3); Box-Muller pair 11 (2 exact uniforms at 2 each, lg2, sqrt,
-#   angle FMA, sin, cos, 2 products) => 22 for n_x = 4, 33 for n_x = 6; noise add 1 FMA per component;
-#   bicycle step 7 (sin, cos, 5 FMA-class); single-track step 75; bilinear lookup 18; racing smooth cost 30.
-#   NOT credited: range reductions, address arithmetic, loop control, the CVaR select, and every circle test
-#   (far obstacles are culled exactly, and a culled test is not achieved work).
-_BICYCLE = 40 + 22 + 4 + 7
-_SINGLE_TRACK = 80 + 33 + 6 + 75
+# Algorithmic lane-operations per noisy state-step ("What bounds it"): the instructions the method
+# itself needs in its leanest known formulation, one per FP32-lane issue slot (FFMA = 1).
+#   Philox4x32-10 call 40 (20 mul-wide + 20 xor3), and a state-step takes n_x/8 of a call (16 bits per uniform, one word per
+#   Box-Muller pair): 20 for n_x = 4, 30 for n_x = 6; Box-Muller pair 10 (2 uniforms at 2 each, lg2, sqrt, sin, cos, 2 products);
+#   noise add 1 FMA per component; bicycle step 7 (sin, cos, 5 FMA-class); single-track step 75; bilinear lookup 18; racing
+#   smooth cost 30.  NOT credited: range reductions, address arithmetic, loop control, the CVaR select, and every circle
+#   test (far obstacles are culled exactly, and a culled test is not achieved work).
+_BICYCLE = 20 + 20 + 4 + 7
+_SINGLE_TRACK = 30 + 30 + 6 + 75
 ALGO_OPS = {"PAPER": _BICYCLE + 30, "PAPER-ST": _SINGLE_TRACK + 30, "C0": _BICYCLE, "C1": _BICYCLE, "C2": _SINGLE_TRACK,
             "C3": _BICYCLE + 18, "C4": _BICYCLE}
-# DRAM bytes (read + write) of one noisy_rollout_kernel launch, from the committed `ncu --set full` captures
-TRAFFIC_BYTES = {"C3": 13.29e6, "C2": 7.97e6}   # profiles/r1d_final_pipeline.md, profiles/r1c_c3_c2_c4_pipe_model.md
 ALU_PEAK_LANE_OPS = 148 * 128 * 1.965e9  # 148 SMs x 128 FP32 lanes x 1.965 GHz (B200_PROFILING.md nominal)
+ISSUE_PEAK_WARP_INST = 148 * 4 * 1.965e9  # one warp instruction per cycle per SM sub-partition
+COUNTERS_CSV = os.path.join(ROOT, "profiles", "r2_rollout_counters.csv")
+
+
+def load_counters():
+    """Per-launch counters of noisy_rollout_kernel from the committed `ncu --set full` captures (profiles/r2_rollout_counters.md
+    names the commands): {workload: {metric: value}}.  Absent file => {} and the derived fractions are null."""
+    import csv
+    out = {}
+    try:
+        rows = list(csv.reader(open(COUNTERS_CSV)))
+    except OSError:
+        return out
+    hdr = rows[0]
+    for r in rows[1:]:
+        if len(r) != len(hdr) or not r[0] or r[0] == "workload":
+            continue
+        d = {}
+        for k, v in zip(hdr[1:], r[1:]):
+            try:
+                d[k] = float(v.replace(",", ""))
+            except ValueError:
+                d[k] = v
+        out[r[0]] = d
+    return out
+
+
+def counter_key(name: str) -> str:
+    """Which capture describes workload `name`: the C4 sweep points share a kernel per M (captured at K = 16384)."""
+    name = name.upper()
+    if name.startswith("C4"):
+        parts = name.split("-")
+        M = parts[2] if len(parts) > 2 else "M64"
+        return f"C4-{M}"
+    return name
+
+
+def derived_fractions(name, state_steps, kernel_ms, ffma_peak_tlaneops, counters):
+    """Roofline fractions of one rollout-kernel launch lasting kernel_ms (measured live):
+    frac = algorithmic lane-ops / measured FFMA issue rate (the contract's figure);
+    frac_fp32_flop = FP32 flop/s (2 FFMA + FADD + FMUL thread instructions of the ncu capture) / measured FFMA flop/s;
+    frac_issue = executed warp instructions (ncu) / issue slots."""
+    ops = ALGO_OPS[workload_key(name)] * state_steps
+    peak = ffma_peak_tlaneops * 1e12 if ffma_peak_tlaneops and ffma_peak_tlaneops > 0 else ALU_PEAK_LANE_OPS
+    out = {"frac": ops / (kernel_ms * 1e-3) / peak, "frac_fp32_flop": None, "frac_issue": None}
+    c = counters.get(counter_key(name))
+    if c:
+        scale = state_steps / c["state_steps"] if c.get("state_steps") else 1.0   # same kernel, different K
+        flop = 2.0 * c["smsp__sass_thread_inst_executed_op_ffma_pred_on.sum"] + \
+            c["smsp__sass_thread_inst_executed_op_fadd_pred_on.sum"] + c["smsp__sass_thread_inst_executed_op_fmul_pred_on.sum"]
+        out["frac_fp32_flop"] = flop * scale / (kernel_ms * 1e-3) / (2.0 * peak)
+        out["frac_issue"] = c["smsp__inst_executed.sum"] * scale / (kernel_ms * 1e-3) / ISSUE_PEAK_WARP_INST
+    return out
 
 
 def make_problem(name: str, rank: int = 0) -> W.Problem:
@@ -105,13 +156,14 @@ class ClockSampler(threading.Thread):
                 "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
-def cpu_baseline(p: W.Problem, seconds_target: float = 20.0):
-    """The oracle as it stands, timed on the host cores on a bounded slice of the same workload."""
+def cpu_baseline(p: W.Problem, seconds_target: float = 12.0, threads=None):
+    """The oracle as it stands, timed on the host cores on a bounded slice of the same workload (threads = None: all
+    host cores; 1: the oracle as defined, single-threaded)."""
     from oracle import oracle as O
     orc = O.Oracle(p)
-    cores = os.cpu_count() or 1
-    per_step = 0.2e-6  # rough single-thread cost per state-step; only sizes the sample (CPU-seconds of work)
-    n_k = int(min(p.K, max(cores, seconds_target / (per_step * p.M * p.T))))
+    cores = threads or (os.cpu_count() or 1)
+    per_step = 0.13e-6  # rough single-thread cost per state-step; only sizes the sample (CPU-seconds of work)
+    n_k = int(min(p.K, max(cores, seconds_target * cores / (per_step * p.M * p.T))))
     t0 = time.perf_counter()
     orc.rollout_costs(k_begin=0, k_end=n_k, n_threads=cores, want_L=False, want_xT=False)
     dt = time.perf_counter() - t0
@@ -258,9 +310,14 @@ def run_cuda(args):
 
     if rank == 0:
         key = workload_key(args.workload)
+        counters = load_counters()
         ops = ALGO_OPS[key] * units_step
         achieved = ops / (kernel_ms * 1e-3)
         peak = pipe_peaks["ffma"] * 1e12 if pipe_peaks.get("ffma", 0) > 0 else ALU_PEAK_LANE_OPS
+        fr = derived_fractions(args.workload, units_step, kernel_ms, pipe_peaks.get("ffma"), counters)
+        c = counters.get(counter_key(args.workload), {})
+        pct = lambda k: (c[k] / 100.0 if k in c else None)
+        traffic = (c["dram__bytes_read.sum"] + c["dram__bytes_write.sum"]) if "dram__bytes_read.sum" in c else None
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
@@ -275,18 +332,36 @@ def run_cuda(args):
                     "d2h_bytes_per_step": int(4 * 2 * p.T), "ms_per_step": e2e_ms / args.steps,
                     "api": "ra_mppi_step_host (pinned host x0, v -> v+)"},
             "gpu_launches": int(ctl.launches_per_step * args.steps),
-            "roofline": {"bound": "alu", "kernel": "noisy_rollout_kernel", "achieved": achieved / 1e12,
-                         "peak": peak / 1e12, "unit": "Tlane-op/s (FP32-lane issue slots; FFMA = 1)",
-                         "frac": achieved / peak, "traffic": TRAFFIC_BYTES.get(key),
-                         "nominal_peak": ALU_PEAK_LANE_OPS / 1e12, "frac_of_nominal": achieved / ALU_PEAK_LANE_OPS,
-                         "measured_pipe_peaks_Tlaneops": pipe_peaks,
-                         "algorithmic_ops_per_state_step": ALGO_OPS[key], "kernel_ms": kernel_ms,
-                         "kernel_share_of_step": kernel_ms / (total_ms / args.steps),
-                         "peak_source": "measured in this run: FFMA issue rate of ra_mppi_measure_pipe_peaks (FFMA = 1 lane-op); "
-                                        "nominal = 148 SMs x 128 FP32 lanes x 1.965 GHz (DESIGN.md)"},
+            "roofline": {
+                "bound": "alu", "kernel": "noisy_rollout_kernel",
+                "binding_resource": "issue slots and the XU (MUFU) pipe, co-limiting; fmaheavy behind them (pipe_busy)",
+                "achieved": achieved / 1e12, "peak": peak / 1e12,
+                "unit": "Tlane-op/s (algorithmic instructions per FP32-lane issue slot; FFMA = 1)",
+                "frac": achieved / peak,
+                # the same launch on the stricter readings: FP32 flop only, and all executed instructions
+                "frac_fp32_flop": fr["frac_fp32_flop"],
+                "fp32_flop_note": "(2 FFMA + FADD + FMUL thread instructions per launch, ncu SASS counters of the committed capture) / "
+                                  "live kernel time / (2 x measured FFMA rate); Philox integer work and MUFU are not FP32 flop",
+                "frac_issue": fr["frac_issue"],
+                "pipe_busy": {"issue": pct("smsp__issue_active.avg.pct_of_peak_sustained_active"),
+                              "fmaheavy": pct("sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_elapsed"),
+                              "fma": pct("sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active"),
+                              "alu": pct("sm__pipe_alu_cycles_active.avg.pct_of_peak_sustained_active"),
+                              "xu": pct("sm__inst_executed_pipe_xu.avg.pct_of_peak_sustained_active"),
+                              "source": "ncu --set full capture, profiles/r2_rollout_counters.csv" if c else None},
+                "traffic": traffic,
+                "nominal_peak": ALU_PEAK_LANE_OPS / 1e12, "frac_of_nominal": achieved / ALU_PEAK_LANE_OPS,
+                "measured_pipe_peaks_Tlaneops": pipe_peaks,
+                "algorithmic_ops_per_state_step": ALGO_OPS[key], "kernel_ms": kernel_ms,
+                "kernel_share_of_step": kernel_ms / (total_ms / args.steps),
+                "peak_source": "measured in this run: FFMA issue rate of ra_mppi_measure_pipe_peaks (FFMA = 1 lane-op); "
+                               "nominal = 148 SMs x 128 FP32 lanes x 1.965 GHz (DESIGN.md)"},
         }
+        if world == 1 and not args.no_workloads:
+            line["workloads"] = run_workloads(pipe_peaks.get("ffma"), counters, flush)
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(p)
+            line["cpu_baseline_1thread"] = cpu_baseline(p, seconds_target=6.0, threads=1)
         print(json.dumps(line))
     ctl.close()
     if world > 1:
@@ -374,38 +449,41 @@ def run_sharded(args):
         dist.destroy_process_group()
 
 
-def quick_time(p, steps=50, warmup=5):
-    """Device-timed ra_mppi_step on problem p (events per step, L2 flushed between); small helper of --report."""
+def quick_time(p, steps=50, warmup=5, flush=None):
+    """Device-timed ra_mppi_step on problem p (events per step, L2 flushed between); helper of the `workloads` array."""
     import torch
 
     from paper_2209_12842_b200.controller import RaMppi
     ctl = RaMppi(p, device=0)
     d_x0, v_init = ctl.tensor(p.x0), ctl.tensor(p.v)
     d_v = v_init.clone()
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=ctl.device)
+    if flush is None:
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=ctl.device)
     stream = torch.cuda.current_stream()
-    ctl.enable_kernel_timing(True)
     ms, kms = [], []
-    for i in range(warmup + steps):
-        d_v.copy_(v_init)
-        flush.zero_()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(stream)
-        ctl.step(d_x0, d_v, i)
-        b.record(stream)
-        b.synchronize()
-        if i >= warmup:
-            ms.append(a.elapsed_time(b))
-            kms.append(ctl.last_rollout_ms())
+    for timed in (False, True):     # a plain pass for the step time, then one with the event pair around the rollout kernel
+        ctl.enable_kernel_timing(timed)
+        for i in range(warmup + steps):
+            d_v.copy_(v_init)
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            ctl.step(d_x0, d_v, i)
+            b.record(stream)
+            b.synchronize()
+            if i >= warmup:
+                (kms if timed else ms).append(ctl.last_rollout_ms() if timed else a.elapsed_time(b))
     ctl.close()
     step_ms = float(np.mean(ms))
     return {"workload": f"{p.name} K={p.K} M={p.M} T={p.T}", "ms_per_step": step_ms, "iterations_per_s": 1e3 / step_ms,
             "state_steps_per_s": p.state_steps / (step_ms * 1e-3), "rollout_kernel_ms": float(np.mean(kms))}
 
 
-def run_report(args):
-    """--report: all five BASELINE workloads, the C4 sweep, the materialised-noise (HBM) variant of C3 and the
-    500-iteration CUDA-graph closed loop.  One JSON object per line on stdout (not the driver's bench line)."""
+def run_workloads(ffma_peak, counters, flush=None):
+    """Every workload BASELINE.json names, on this GPU, each with its roofline fractions (north_star: "throughput on the
+    five synthetic workloads ... as a fraction of the relevant roofline"): configs 0-3, the 12 points of the config-4
+    sweep, the paper's own workload (two vehicle models), the materialised-noise (HBM-bound) variant of C3, and the
+    500-iteration CUDA-graph closed loop of config 4."""
     import torch
 
     from paper_2209_12842_b200.controller import RaMppi
@@ -415,26 +493,37 @@ def run_report(args):
     except Exception:
         pass
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    out = []
+
+    def add(tag, name, p=None, steps=30):
+        p = make_problem(name) if p is None else p
+        r = quick_time(p, steps=steps, flush=flush)
+        r.update({"kind": tag, "name": name})
+        r.update(derived_fractions(name, p.state_steps, r["rollout_kernel_ms"], ffma_peak, counters))
+        r["roofline_bound"] = "alu"
+        out.append(r)
+        return r, p
+
     for name in ("C0", "C1", "C2", "C3"):
-        print(json.dumps({"report": "workload", **quick_time(make_problem(name))}), flush=True)
+        add("BASELINE config", name)
     for name in ("PAPER", "PAPER-ST"):   # the paper's own workload (context for its 44.3 Hz on an RTX 3090)
-        print(json.dumps({"report": "paper workload (1024 x 300 x 30, costs (20)-(23), l = q)",
-                          **quick_time(make_problem(name), steps=100)}), flush=True)
+        add("paper workload (1024 x 300 x 30, costs (20)-(23), l = q)", name, steps=50)
     for K in W.C4_SWEEP_K:
         for M in W.C4_SWEEP_M:
-            steps = 20 if K * M >= 65536 * 64 else 50
-            print(json.dumps({"report": "C4 sweep", **quick_time(make_problem(f"C4-K{K}-M{M}"), steps=steps)}), flush=True)
+            add("config 4 sweep", f"C4-K{K}-M{M}", steps=15 if K * M >= 65536 * 64 else 30)
     # materialised-noise mode: w[K,T,n_x,M] written by the generator and streamed back by the rollout kernel
     p = make_problem("C3").replace(noise_mode=W.NOISE_MATERIALISED)
-    r = quick_time(p, steps=30)
+    r = quick_time(p, steps=15, flush=flush)
     noise_bytes = 4.0 * p.nx * p.state_steps
-    r.update({"report": "materialised noise (HBM-bound variant)", "noise_tensor_GB": noise_bytes / 1e9,
-              "rollout_read_GBps": noise_bytes / (r["rollout_kernel_ms"] * 1e-3) / 1e9,
-              "hbm_peak_GBps": hbm_peak, "peak_source": "measured" if peaks else "fallback",
-              "rollout_frac_of_hbm_peak": noise_bytes / (r["rollout_kernel_ms"] * 1e-3) / 1e9 / hbm_peak})
-    print(json.dumps(r), flush=True)
+    gbs = noise_bytes / (r["rollout_kernel_ms"] * 1e-3) / 1e9
+    r.update({"kind": "materialised noise (HBM-bound variant of C3)", "name": "C3-materialised", "roofline_bound": "hbm",
+              "noise_tensor_GB": noise_bytes / 1e9, "rollout_read_GBps": gbs, "hbm_peak_GBps": hbm_peak,
+              "peak_source": "measured (MEASURED_PEAKS.json)" if peaks else "fallback", "frac": gbs / hbm_peak,
+              "frac_note": "rollout kernel streaming the noise tensor: algorithmic bytes 4 n_x K M T / kernel time / HBM copy peak"})
+    out.append(r)
     # closed loop: config 4, K=8192, M=64, 500 receding-horizon iterations replayed from one CUDA graph
-    p = make_problem("C4-K8192-M64")
+    name = "C4-K8192-M64"
+    p = make_problem(name)
     ctl = RaMppi(p, device=0)
     d_x0, d_v = ctl.tensor(p.x0), ctl.tensor(np.zeros((p.T, 2)))
     ctl.closed_loop(d_x0, d_v, 0, 20)                      # capture + warm-up
@@ -448,12 +537,27 @@ def run_report(args):
     b.synchronize()
     total = a.elapsed_time(b)
     log = log.cpu().numpy()
-    print(json.dumps({"report": "closed loop (CUDA graph)", "workload": f"{p.name} K={p.K} M={p.M} T={p.T}",
-                      "iterations": 500, "sustained_hz": 500.0 / (total * 1e-3), "latency_ms_p50": float(np.percentile(ms, 50)),
-                      "latency_ms_p99": float(np.percentile(ms, 99)), "latency_ms_max": float(ms.max()),
-                      "final_state": [float(x) for x in log[-1, :p.nx]],
-                      "distance_travelled_m": float(np.hypot(np.diff(log[:, 0]), np.diff(log[:, 1])).sum())}), flush=True)
+    p50 = float(np.percentile(ms, 50))
+    cl = {"kind": "closed loop (one CUDA graph launch per iteration)", "name": name + "-closed-loop",
+          "workload": f"{p.name} K={p.K} M={p.M} T={p.T}", "iterations": 500, "sustained_hz": 500.0 / (total * 1e-3),
+          "latency_ms_p50": p50, "latency_ms_p99": float(np.percentile(ms, 99)), "latency_ms_max": float(ms.max()),
+          "ms_per_step": total / 500.0, "state_steps_per_s": p.state_steps * 500.0 / (total * 1e-3),
+          "final_state": [float(x) for x in log[-1, :p.nx]],
+          "distance_travelled_m": float(np.hypot(np.diff(log[:, 0]), np.diff(log[:, 1])).sum()), "roofline_bound": "alu"}
+    # whole-iteration fractions (the graph has no event pair around the rollout kernel): iteration time as the denominator
+    cl.update(derived_fractions(name, p.state_steps, total / 500.0, ffma_peak, counters))
+    cl["frac_note"] = "whole iteration (sampling + rollouts + update + plant) as the time base"
+    out.append(cl)
     ctl.close()
+    return out
+
+
+def run_report(args):
+    """--report: the `workloads` array of the default line, one JSON object per line (not the driver's bench line)."""
+    from paper_2209_12842_b200 import binding as B
+    pipe_peaks = B.ra_mppi_measure_pipe_peaks(0)
+    for r in run_workloads(pipe_peaks.get("ffma"), load_counters()):
+        print(json.dumps({"report": r.pop("kind"), **r}), flush=True)
 
 
 def main():
@@ -465,6 +569,7 @@ def main():
     ap.add_argument("--workload", default="C3")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-workloads", action="store_true", help="leave the per-workload array out of the line (short profiling runs)")
     ap.add_argument("--pipe-model", action="store_true",
                     help="print the measured issue-cost model of the SM pipes (one JSON line) and exit")
     ap.add_argument("--sharded", action="store_true",

@@ -94,6 +94,13 @@ def test_full_oracle_comparison(torch_cuda, name):
     assert err2 < TOL_V_ABS
     assert int(np.argmin(g["St64"])) == int(np.argmin(r["S_tilde"])) or \
         np.sort(r["S_tilde"])[1] - np.sort(r["S_tilde"])[0] < 2 * np.abs(g["St64"] - r["S_tilde"]).max()
+    # the same comparison through the shared helper, so the full-size cases appear in the verdict table
+    from parity_utils import check_step_parity
+    from paper_2209_12842_b200.controller import RaMppi
+    ctl = RaMppi(p, device=0)
+    verdict, _ = check_step_parity(p, ctl, orc, r, case=f"{name} full size K={p.K} M={p.M} T={p.T} lambda={p.lam:g}")
+    print(f"{name}: {verdict}")
+    ctl.close()
 
 
 @pytest.mark.parametrize("name", ["C2", "C4-K8192-M64", "C4-K65536-M256", "C4-K65536-M16"])
