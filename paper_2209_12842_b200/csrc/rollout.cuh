@@ -317,6 +317,35 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
   pdl_launch_dependents();   // the weights/update kernel may be scheduled behind the last wave of this grid
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const float x0X = x0g[0], x0Y = x0g[1];
+
+  const int sample_in_cta = warp / wps, ws = warp - sample_in_cta * wps;
+  const int sample = blockIdx.x * (kRolloutWarps / wps) + sample_in_cta;
+  const int k_raw = HALF ? sample * 2 + (lane >> 4) : sample;
+  const int sub = HALF ? (lane & 15) : lane;
+  const uint32_t mask = HALF ? (0xFFFFu << (lane & 16)) : 0xFFFFFFFFu;
+  const bool k_valid = k_raw < p.K;
+  const int k = k_valid ? k_raw : p.K - 1;
+  uint32_t* keys = keys_all + (size_t)sample_in_cta * p.R_total * 32;
+
+  // The T control effects of sample k (one contiguous row of ce[K][T], 16 T bytes) go to shared memory once, so the step
+  // loop reads them with a broadcast LDS instead of a dependent L2 load per step.  The row is moved by the TMA engine:
+  // one thread per row arms an mbarrier with the byte count and issues a 1-D bulk copy (cp.async.bulk, SASS UBLKCP); the
+  // copy runs while the CTA stages its obstacles, and the threads that use the row wait on the barrier's phase.
+  // Measured against an LDG/STS loop per warp: C3 step 0.393 -> 0.387 ms, other workloads equal (profiles/r2_tma_experiment.md).
+  __shared__ __align__(8) unsigned long long ce_bar[kCeSlotsMax];
+  const int ce_slot = HALF ? warp * 2 + (lane >> 4) : sample_in_cta;
+  const float4* ce_s = ce_all + (size_t)ce_slot * p.T;
+  if (ws == 0 && sub == 0) {
+    const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&ce_bar[ce_slot]);
+    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(ce_s);
+    const uint32_t bytes = (uint32_t)p.T * (uint32_t)sizeof(float4);
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+    asm volatile("fence.mbarrier_init.release.cluster;");
+    asm volatile("fence.proxy.async.shared::cta;");     // the barrier's initialisation is visible to the async proxy
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(p.ce + (size_t)k * p.T), "r"(bytes), "r"(bar) : "memory");
+  }
   if constexpr (kUsesCircles) {
     for (int i = threadIdx.x; i < n_circ_s; i += blockDim.x) {
       float4 c = make_float4(0.0f, 0.0f, 0.0f, 0.0f);   // padding: R^2 = 0 is never near
@@ -330,24 +359,12 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
   MapFrame mf{};
   if constexpr (RISK == RISK_COSTMAP) mf = make_map_frame(p, x0X, x0Y);
 
-  const int sample_in_cta = warp / wps, ws = warp - sample_in_cta * wps;
-  const int sample = blockIdx.x * (kRolloutWarps / wps) + sample_in_cta;
-  const int k_raw = HALF ? sample * 2 + (lane >> 4) : sample;
-  const int sub = HALF ? (lane & 15) : lane;
-  const uint32_t mask = HALF ? (0xFFFFu << (lane & 16)) : 0xFFFFFFFFu;
-  const bool k_valid = k_raw < p.K;
-  const int k = k_valid ? k_raw : p.K - 1;
-  uint32_t* keys = keys_all + (size_t)sample_in_cta * p.R_total * 32;
-
-  // The T control effects of sample k (one contiguous row of ce[K][T]) go to shared memory once, so the
-  // step loop reads them with a broadcast LDS instead of a dependent L2 load per step.
-  const float4* ce_s = ce_all + (size_t)(HALF ? warp * 2 + (lane >> 4) : sample_in_cta) * p.T;
-  if (ws == 0) {
-    float4* dst = const_cast<float4*>(ce_s);
-    const float4* src = p.ce + (size_t)k * p.T;
-    for (int t = sub; t < p.T; t += G) dst[t] = __ldg(src + t);
+  __syncthreads();   // obstacles staged; the barriers are initialised for every thread that waits on one
+  {
+    const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&ce_bar[ce_slot]);
+    asm volatile("{\n\t.reg .pred P1;\n\tRA_WAIT_CE:\n\tmbarrier.try_wait.parity.shared::cta.b64 P1, [%0], 0;\n\t@!P1 bra RA_WAIT_CE;\n\t}"
+                 ::"r"(bar) : "memory");
   }
-  __syncthreads();
 
   float x_init[NX];
   x_init[0] = 0.0f; x_init[1] = 0.0f;
