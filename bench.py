@@ -358,7 +358,7 @@ def run_cuda(args):
                                "nominal = 148 SMs x 128 FP32 lanes x 1.965 GHz (DESIGN.md)"},
         }
         if world == 1 and not args.no_workloads:
-            line["workloads"] = run_workloads(pipe_peaks.get("ffma"), counters, flush)
+            line["workloads"] = run_workloads(pipe_peaks.get("ffma"), counters, flush, with_cpu=not args.no_cpu_baseline)
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(p)
             line["cpu_baseline_1thread"] = cpu_baseline(p, seconds_target=6.0, threads=1)
@@ -479,7 +479,7 @@ def quick_time(p, steps=50, warmup=5, flush=None):
             "state_steps_per_s": p.state_steps / (step_ms * 1e-3), "rollout_kernel_ms": float(np.mean(kms))}
 
 
-def run_workloads(ffma_peak, counters, flush=None):
+def run_workloads(ffma_peak, counters, flush=None, with_cpu=False):
     """Every workload BASELINE.json names, on this GPU, each with its roofline fractions (north_star: "throughput on the
     five synthetic workloads ... as a fraction of the relevant roofline"): configs 0-3, the 12 points of the config-4
     sweep, the paper's own workload (two vehicle models), the materialised-noise (HBM-bound) variant of C3, and the
@@ -505,7 +505,9 @@ def run_workloads(ffma_peak, counters, flush=None):
         return r, p
 
     for name in ("C0", "C1", "C2", "C3"):
-        add("BASELINE config", name)
+        r, p = add("BASELINE config", name)
+        if with_cpu:   # the oracle as defined (one thread) on a ~1 s slice of this config, beside the GPU number
+            r["cpu_oracle_1thread"] = cpu_baseline(p, seconds_target=1.0, threads=1)
     for name in ("PAPER", "PAPER-ST"):   # the paper's own workload (context for its 44.3 Hz on an RTX 3090)
         add("paper workload (1024 x 300 x 30, costs (20)-(23), l = q)", name, steps=50)
     for K in W.C4_SWEEP_K:

@@ -43,7 +43,8 @@ inline cudaError_t launch_kernel(void (*kernel)(KArgs...), dim3 grid, dim3 block
 }
 
 // noise: NOISE_GAUSSIAN / NOISE_UNIFORM / NOISE_JUMP / 3 (materialised); rc in {1,2,4};
-// half: two samples per warp (M <= 16, rc must be 1); pdl: launch as a programmatic dependent of the previous kernel.
+// half: half a warp per sample (M <= 16; rc in {1,2} = 2 rc samples per warp); pdl: launch as a programmatic dependent of the
+// previous kernel.
 using RolloutLaunchFn = cudaError_t (*)(const Params& p, int noise, int rc, bool half, const float* d_x0,
                                         float* d_L, float* d_xT, cudaStream_t stream, bool pdl);
 

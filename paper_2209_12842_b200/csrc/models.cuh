@@ -229,7 +229,8 @@ __device__ __forceinline__ float terminal_cost(const Params& p, float Xabs, floa
 struct MapFrame {
   float bxf, byf;            // fractional part of (x0 - origin)/res + 1/2
   float lox, hix, loy, hiy;  // clamp bounds of the fractional-frame coordinate
-  uint32_t base;             // (integer bias y) * (W+1) + (integer bias x), less the magic-number bits (mod 2^32)
+  uint32_t addr_lo, addr_hi; // address of the table entry at index "0 - magic-number bits" (mod 2^32 in the low word): the table lies
+                             // inside one 4 GiB window (ra_mppi_create), so an entry's address is addr_hi : (addr_lo + 16 idx), no carry
 };
 
 constexpr float kFloorMagic = 12582912.0f;     // 1.5 * 2^23
@@ -244,7 +245,11 @@ __device__ __forceinline__ MapFrame make_map_frame(const Params& p, float x0X, f
   f.lox = -fx; f.hix = (float)p.map_w - fx;
   f.loy = -fy; f.hiy = (float)p.map_h - fy;
   const uint32_t stride = (uint32_t)(p.map_w + 1);
-  f.base = (uint32_t)(int)fy * stride + (uint32_t)(int)fx - ((uint32_t)kFloorMagicBits * stride + (uint32_t)kFloorMagicBits);
+  // (integer bias y) * (W+1) + (integer bias x), less the magic-number bits the lookup leaves in jx, jy (mod 2^32)
+  const uint32_t base = (uint32_t)(int)fy * stride + (uint32_t)(int)fx - ((uint32_t)kFloorMagicBits * stride + (uint32_t)kFloorMagicBits);
+  const unsigned long long q0 = reinterpret_cast<unsigned long long>(p.quadmap);
+  f.addr_lo = (uint32_t)q0 + (base << 4);
+  f.addr_hi = (uint32_t)(q0 >> 32);
   return f;
 }
 
@@ -253,13 +258,12 @@ __device__ __forceinline__ float bilinear_weighted(const Params& p, const MapFra
   const float gy = fminf(fmaxf(fmaf(Yrel, p.map_inv_res, f.byf), f.loy), f.hiy);
   const float jx = __fadd_rd(gx, kFloorMagic), jy = __fadd_rd(gy, kFloorMagic);
   const float tx = gx - (jx - kFloorMagic), ty = gy - (jy - kFloorMagic);
-  // all index arithmetic is mod 2^32; the sum is the absolute table index in [0, (H+1)(W+1))
-  const uint32_t idx = __float_as_uint(jy) * (uint32_t)(p.map_w + 1) + __float_as_uint(jx) + f.base;
-  // byte address = table + 16 idx with two 32-bit adds on the ALU pipe (add.cc / addc) instead of a 64-bit
-  // IMAD.WIDE, which would hold the FMA pipe for four cycles (profiles/r1c); the table is < 4 GB (validated)
+  // all index arithmetic is mod 2^32: jy_bits * (W+1) + jx_bits + base is the absolute table index in [0, (H+1)(W+1)), and
+  // 16 times it, added to the low address word, cannot carry (the table lies inside one 4 GiB window).  One IMAD + one LEA per
+  // lookup; a 64-bit IMAD.WIDE here would hold the FMA pipe for four cycles (profiles/r1c).
+  const uint32_t idx = __float_as_uint(jy) * (uint32_t)(p.map_w + 1) + __float_as_uint(jx);
   const float4* addr;
-  asm("{\n\t.reg .u32 lo, hi;\n\tmov.b64 {lo, hi}, %1;\n\tadd.cc.u32 lo, lo, %2;\n\taddc.u32 hi, hi, 0;\n\tmov.b64 %0, {lo, hi};\n\t}"
-      : "=l"(addr) : "l"(p.quadmap), "r"(idx << 4));
+  asm("mov.b64 %0, {%1, %2};" : "=l"(addr) : "r"(f.addr_lo + (idx << 4)), "r"(f.addr_hi));
   const float4 q = __ldg(addr);
   return fmaf(ty, fmaf(tx, q.w, q.z), fmaf(tx, q.y, q.x));
 }

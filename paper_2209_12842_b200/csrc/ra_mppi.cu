@@ -27,7 +27,8 @@ struct ra_mppi_ctx {
   RolloutLaunchFn rollout = nullptr;
   // device allocations owned by the context
   float4* d_circles = nullptr;
-  float4* d_costmap = nullptr;  // quad-texel table
+  float4* d_costmap = nullptr;  // quad-texel table: allocation
+  float4* d_quadmap = nullptr;  // ... and the table inside it, placed so that it does not straddle a 4 GiB boundary
   float2* d_u_raw = nullptr;
   float4* d_ce = nullptr;
   double* d_S = nullptr;
@@ -223,10 +224,26 @@ ra_status upload_env(ra_mppi_ctx* c, const ra_mppi_env* env, bool first) {
         q[(size_t)jy * (Wd + 1) + jx] = make_float4((float)(w * c00), (float)(w * (c01 - c00)), (float)(w * (c10 - c00)),
                                                     (float)(w * (c11 - c10 - c01 + c00)));
       }
-    if (first && dev_alloc(&c->d_costmap, n) != cudaSuccess) return fail(c, RA_ENOMEM, "alloc costmap");
-    if (cuda_fail(c, cudaMemcpy(c->d_costmap, q.data(), n * sizeof(float4), cudaMemcpyHostToDevice), "copy costmap"))
+    if (first) {
+      // The kernel forms a lookup address as (high word of the table) : (low word + 16 idx) with one 32-bit add, so the
+      // table must lie inside one 4 GiB-aligned window (its size is < 4 GiB, validated).  An allocation that straddles a
+      // boundary (about one in a thousand for a 4 MB table) is replaced by one of twice the size, which always holds an
+      // aligned copy.
+      const size_t bytes = n * sizeof(float4);
+      auto straddles = [bytes](const void* q0) { return ((reinterpret_cast<uintptr_t>(q0) & 0xFFFFFFFFull) + bytes) > (1ull << 32); };
+      if (dev_alloc(&c->d_costmap, n) != cudaSuccess) return fail(c, RA_ENOMEM, "alloc costmap");
+      c->d_quadmap = c->d_costmap;
+      if (straddles(c->d_costmap)) {
+        cudaFree(c->d_costmap); c->d_costmap = nullptr;
+        if (dev_alloc(&c->d_costmap, 2 * n) != cudaSuccess) return fail(c, RA_ENOMEM, "alloc costmap");
+        c->d_quadmap = c->d_costmap;
+        if (straddles(c->d_costmap))   // start the table at the boundary inside the allocation
+          c->d_quadmap = reinterpret_cast<float4*>((reinterpret_cast<uintptr_t>(c->d_costmap) + bytes) & ~0xFFFFFFFFull);
+      }
+    }
+    if (cuda_fail(c, cudaMemcpy(c->d_quadmap, q.data(), n * sizeof(float4), cudaMemcpyHostToDevice), "copy costmap"))
       return RA_ECUDA;
-    p.quadmap = c->d_costmap;
+    p.quadmap = c->d_quadmap;
     p.map_h = env->map_h; p.map_w = env->map_w;
     p.map_inv_res = (float)(1.0 / (double)env->map_res);
     p.map_ox = env->map_ox; p.map_oy = env->map_oy;
@@ -282,7 +299,10 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
   // so every warp runs one group: shorter CTAs fill the SMs at small K (the paper's 1024 x 300
   // workload: 5 groups -> 8 warps) and cut the wave tail at large K.
   p.wps = 1;
-  c->rc = 1;
+  // M <= 16: a warp carries 2 rc samples.  Two slots per lane halve the per-state-step share of the obstacle culling, but
+  // also the number of warps: measured on B200 (profiles/r2), rc = 2 wins from K = 65536 (0.308 -> 0.281 ms) and loses below
+  // K = 16384 (0.093 -> 0.098 ms; K = 1024: 0.034 -> 0.045 ms), where the GPU is not full.
+  c->rc = (c->half && cfg->K >= 32768) ? 2 : 1;
   if (!c->half) {
     c->rc = (p.R_total >= 4 && p.R_total % 4 == 0) ? 4 : (p.R_total >= 2 ? 2 : 1);
     const int groups = (p.R_total + c->rc - 1) / c->rc;
@@ -292,9 +312,10 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
     // shared-memory carveout (percent of the 228 KB unified L1) that holds three rollout CTAs; the nominal-rollout
     // kernel asks for the same split so both kernels can share an SM
     const bool circ = cfg->risk == RA_RISK_CIRCLES || cfg->nominal == RA_NOM_RACING;
-    const size_t ce_slots = c->half ? 2 * kRolloutWarps : kRolloutWarps / p.wps;
+    const size_t ce_slots = c->half ? 2 * c->rc * kRolloutWarps : kRolloutWarps / p.wps;
     const size_t smem_cta = (circ && env ? (size_t)((env->n_circles + 31) & ~31) * sizeof(float4) : 0) +
-                            ce_slots * cfg->T * sizeof(float4) + (size_t)kRolloutWarps * p.R_total * 32 * sizeof(uint32_t);
+                            ce_slots * cfg->T * sizeof(float4) +
+                            (size_t)kRolloutWarps * (c->half ? c->rc : p.R_total) * 32 * sizeof(uint32_t);
     const size_t need = 3 * (smem_cta + 1024);
     p.carveout = need <= 57 * 1024 ? 25 : (need <= 114 * 1024 ? 50 : 100);
   }

@@ -307,9 +307,12 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
   const int n_circ_s = kUsesCircles ? ((p.n_circles + 31) & ~31) : 0;   // padded to whole 32-obstacle batches
   // wps warps share one control sample when K alone cannot fill the GPU (small K, large M):
   // warp ws of the sample takes the realisation chunks ws, ws + wps, ...; the CVaR select runs in
-  // warp 0 of the sample after a CTA barrier.  HALF (two samples per warp) always has wps = 1.
+  // warp 0 of the sample after a CTA barrier.
+  // HALF (M <= 16): a sample needs only half a warp, so a warp carries 2 RC samples -- lanes 0-15 / 16-31 of
+  // realisation slot r belong to samples 2r / 2r+1 of the warp -- and always has wps = 1.  (With one slot per lane the
+  // per-step obstacle culling, ~120 warp-instructions whatever RC is, is spread over half as many state-steps.)
   const int wps = HALF ? 1 : p.wps;
-  constexpr int kCeSlotsMax = HALF ? 2 * kRolloutWarps : kRolloutWarps;
+  constexpr int kCeSlotsMax = HALF ? 2 * RC * kRolloutWarps : kRolloutWarps;
   const int ce_slots = HALF ? kCeSlotsMax : kRolloutWarps / wps;
   float4* ce_all = smem4 + n_circ_s;                                   // [ce_slots][T] control effects
   uint32_t* keys_all = reinterpret_cast<uint32_t*>(ce_all + (size_t)ce_slots * p.T);
@@ -320,12 +323,23 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
 
   const int sample_in_cta = warp / wps, ws = warp - sample_in_cta * wps;
   const int sample = blockIdx.x * (kRolloutWarps / wps) + sample_in_cta;
-  const int k_raw = HALF ? sample * 2 + (lane >> 4) : sample;
   const int sub = HALF ? (lane & 15) : lane;
   const uint32_t mask = HALF ? (0xFFFFu << (lane & 16)) : 0xFFFFFFFFu;
-  const bool k_valid = k_raw < p.K;
-  const int k = k_valid ? k_raw : p.K - 1;
-  uint32_t* keys = keys_all + (size_t)sample_in_cta * p.R_total * 32;
+  // sample of realisation slot r of this lane: the warp's one sample, or (HALF) sample 2r + (lane >> 4) of the warp's 2 RC
+  int k_of[RC];
+  bool k_valid_of[RC];
+  const float4* ce_of[RC];     // its control-effect row in shared memory
+  uint32_t* keys_of[RC];       // its key row(s): [R_total][32], or (HALF) one row of 32 shared by the two samples of slot r
+  int ce_slot_of[RC];
+#pragma unroll
+  for (int r = 0; r < RC; ++r) {
+    const int k_raw = HALF ? ((blockIdx.x * kRolloutWarps + warp) * RC + r) * 2 + (lane >> 4) : sample;
+    k_valid_of[r] = k_raw < p.K;
+    k_of[r] = k_valid_of[r] ? k_raw : p.K - 1;
+    ce_slot_of[r] = HALF ? (warp * RC + r) * 2 + (lane >> 4) : sample_in_cta;
+    ce_of[r] = ce_all + (size_t)ce_slot_of[r] * p.T;
+    keys_of[r] = keys_all + (HALF ? (size_t)(warp * RC + r) * 32 : (size_t)sample_in_cta * p.R_total * 32);
+  }
 
   // The T control effects of sample k (one contiguous row of ce[K][T], 16 T bytes) go to shared memory once, so the step
   // loop reads them with a broadcast LDS instead of a dependent L2 load per step.  The row is moved by the TMA engine:
@@ -333,18 +347,19 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
   // copy runs while the CTA stages its obstacles, and the threads that use the row wait on the barrier's phase.
   // Measured against an LDG/STS loop per warp: C3 step 0.393 -> 0.387 ms, other workloads equal (profiles/r2_tma_experiment.md).
   __shared__ __align__(8) unsigned long long ce_bar[kCeSlotsMax];
-  const int ce_slot = HALF ? warp * 2 + (lane >> 4) : sample_in_cta;
-  const float4* ce_s = ce_all + (size_t)ce_slot * p.T;
   if (ws == 0 && sub == 0) {
-    const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&ce_bar[ce_slot]);
-    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(ce_s);
-    const uint32_t bytes = (uint32_t)p.T * (uint32_t)sizeof(float4);
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
-    asm volatile("fence.mbarrier_init.release.cluster;");
-    asm volatile("fence.proxy.async.shared::cta;");     // the barrier's initialisation is visible to the async proxy
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(dst), "l"(p.ce + (size_t)k * p.T), "r"(bytes), "r"(bar) : "memory");
+#pragma unroll
+    for (int r = 0; r < (HALF ? RC : 1); ++r) {
+      const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&ce_bar[ce_slot_of[r]]);
+      const uint32_t dst = (uint32_t)__cvta_generic_to_shared(ce_of[r]);
+      const uint32_t bytes = (uint32_t)p.T * (uint32_t)sizeof(float4);
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+      asm volatile("fence.mbarrier_init.release.cluster;");
+      asm volatile("fence.proxy.async.shared::cta;");     // the barrier's initialisation is visible to the async proxy
+      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                   ::"r"(dst), "l"(p.ce + (size_t)k_of[r] * p.T), "r"(bytes), "r"(bar) : "memory");
+    }
   }
   if constexpr (kUsesCircles) {
     for (int i = threadIdx.x; i < n_circ_s; i += blockDim.x) {
@@ -360,8 +375,9 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
   if constexpr (RISK == RISK_COSTMAP) mf = make_map_frame(p, x0X, x0Y);
 
   __syncthreads();   // obstacles staged; the barriers are initialised for every thread that waits on one
-  {
-    const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&ce_bar[ce_slot]);
+#pragma unroll
+  for (int r = 0; r < (HALF ? RC : 1); ++r) {
+    const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&ce_bar[ce_slot_of[r]]);
     asm volatile("{\n\t.reg .pred P1;\n\tRA_WAIT_CE:\n\tmbarrier.try_wait.parity.shared::cta.b64 P1, [%0], 0;\n\t@!P1 bra RA_WAIT_CE;\n\t}"
                  ::"r"(bar) : "memory");
   }
@@ -376,7 +392,9 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
   x_init[2] = reduce_yaw(x_init[2], yaw_turns);
 
   const uint32_t c3 = iteration_field(p, STREAM_W);
-  const uint32_t kg = (uint32_t)(k + p.k_off);   // global sample index in the Philox counter
+  uint32_t kg[RC];                               // global sample index in the Philox counter
+#pragma unroll
+  for (int r = 0; r < RC; ++r) kg[r] = (uint32_t)(k_of[HALF ? r : 0] + p.k_off);
 
   for (int chunk = ws * RC; chunk < p.R_total; chunk += wps * RC) {
     float x[RC][NX], L[RC];
@@ -384,17 +402,20 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
 #pragma unroll
     for (int r = 0; r < RC; ++r) {
       L[r] = 0.0f;
-      m[r] = (uint32_t)((chunk + r) * G + sub);
+      m[r] = HALF ? (uint32_t)sub : (uint32_t)((chunk + r) * G + sub);
 #pragma unroll
       for (int i = 0; i < NX; ++i) x[r][i] = x_init[i];
     }
     // one transition of all RC realisations of this lane: l(x~_t) at the pre-step state, then
     // x~_{t+1} = F(x~_t, u_t) + w_t   (6) PAPER.md:63 with w_t = wscale (.) a
     auto advance = [&](int t, const float (&a)[RC][NX]) {
-      const float4 ce = ce_s[t];
+      float4 ce_shared;
+      if constexpr (!HALF) ce_shared = ce_of[0][t];   // the slots share a sample: one broadcast LDS per step
       risk_accumulate<RISK, RC, NX>(p, circ_s, n_circ_s, lane, mf, x0X, x0Y, yaw_turns, x, L);
 #pragma unroll
       for (int r = 0; r < RC; ++r) {
+        float4 ce;
+        if constexpr (HALF) ce = ce_of[r][t]; else ce = ce_shared;
         dynamics_step<DYN, true>(p, x[r], ce);
 #pragma unroll
         for (int i = 0; i < NX; ++i)
@@ -410,7 +431,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
           // a slot past R_total (RC does not divide the slot count) has m >= M_pad: clamp it into the row so
           // the load stays inside w_mat; the slot's results are discarded below
           const uint32_t mc = min(m[r], (uint32_t)(p.M_pad - 1));
-          const float* wp = p.w_mat + (((size_t)k * p.T + t) * NX) * p.M_pad + mc;
+          const float* wp = p.w_mat + (((size_t)k_of[r] * p.T + t) * NX) * p.M_pad + mc;
 #pragma unroll
           for (int i = 0; i < NX; ++i) a[r][i] = __ldg(wp + (size_t)i * p.M_pad);
         }
@@ -424,7 +445,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
         float a[RC][NX];
 #pragma unroll
         for (int r = 0; r < RC; ++r) {
-          const uint4 q = philox4x32_10(kg, m[r], (uint32_t)(t >> 1), c3, p.rk);
+          const uint4 q = philox4x32_10(kg[r], m[r], (uint32_t)(t >> 1), c3, p.rk);
           const uint32_t w[2] = {q.x, q.y};
           carry[r][0] = q.z; carry[r][1] = q.w;
           noise_from_words<NX, NOISE>(p, w, a[r]);
@@ -440,7 +461,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
       if (t < p.T) {   // odd horizon: the last (even-indexed) step takes the first half of its call
         float a[RC][NX];
 #pragma unroll
-        for (int r = 0; r < RC; ++r) state_noise<NX, NOISE>(p, kg, m[r], (uint32_t)t, c3, a[r]);
+        for (int r = 0; r < RC; ++r) state_noise<NX, NOISE>(p, kg[r], m[r], (uint32_t)t, c3, a[r]);
         advance(t, a);
       }
     } else if constexpr (NoiseWords<NX, NOISE>::value == 3) {
@@ -452,7 +473,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
         float a[RC][NX];
 #pragma unroll
         for (int r = 0; r < RC; ++r) {
-          const uint4 qa = philox4x32_10(kg, m[r], c, c3, p.rk);
+          const uint4 qa = philox4x32_10(kg[r], m[r], c, c3, p.rk);
           const uint32_t w[3] = {qa.x, qa.y, qa.z};
           carry[r][0] = qa.w;
           noise_from_words<NX, NOISE>(p, w, a[r]);
@@ -460,7 +481,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
         advance(t, a);
 #pragma unroll
         for (int r = 0; r < RC; ++r) {
-          const uint4 qb = philox4x32_10(kg, m[r], c + 1u, c3, p.rk);
+          const uint4 qb = philox4x32_10(kg[r], m[r], c + 1u, c3, p.rk);
           const uint32_t w[3] = {carry[r][0], qb.x, qb.y};
           carry[r][0] = qb.z; carry[r][1] = qb.w;
           noise_from_words<NX, NOISE>(p, w, a[r]);
@@ -468,7 +489,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
         advance(t + 1, a);
 #pragma unroll
         for (int r = 0; r < RC; ++r) {
-          const uint4 qc = philox4x32_10(kg, m[r], c + 2u, c3, p.rk);
+          const uint4 qc = philox4x32_10(kg[r], m[r], c + 2u, c3, p.rk);
           const uint32_t w[3] = {carry[r][0], carry[r][1], qc.x};
           carry[r][0] = qc.y; carry[r][1] = qc.z; carry[r][2] = qc.w;
           noise_from_words<NX, NOISE>(p, w, a[r]);
@@ -484,7 +505,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
       for (; t < p.T; ++t) {   // up to three ragged steps on their own
         float a[RC][NX];
 #pragma unroll
-        for (int r = 0; r < RC; ++r) state_noise<NX, NOISE>(p, kg, m[r], (uint32_t)t, c3, a[r]);
+        for (int r = 0; r < RC; ++r) state_noise<NX, NOISE>(p, kg[r], m[r], (uint32_t)t, c3, a[r]);
         advance(t, a);
       }
     } else {
@@ -492,16 +513,18 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
       for (int t = 0; t < p.T; ++t) {
         float a[RC][NX];
 #pragma unroll
-        for (int r = 0; r < RC; ++r) state_noise<NX, NOISE>(p, kg, m[r], (uint32_t)t, c3, a[r]);
+        for (int r = 0; r < RC; ++r) state_noise<NX, NOISE>(p, kg[r], m[r], (uint32_t)t, c3, a[r]);
         advance(t, a);
       }
     }
 #pragma unroll
     for (int r = 0; r < RC; ++r) {
-      const bool valid = (chunk + r) < p.R_total && (int)m[r] < p.M;
+      const bool slot_ok = HALF || (chunk + r) < p.R_total;
+      const bool valid = slot_ok && (int)m[r] < p.M;
       if constexpr (RISK == RISK_CIRCLES) L[r] *= p.risk_p[0];   // risk_accumulate sums unweighted penetrations
-      if (chunk + r < p.R_total) keys[(chunk + r) * 32 + lane] = valid ? float_key(L[r]) : 0u;
-      if (valid && k_valid) {
+      if (slot_ok) keys_of[r][(HALF ? 0 : (chunk + r) * 32) + lane] = valid ? float_key(L[r]) : 0u;
+      if (valid && k_valid_of[r]) {
+        const int k = k_of[r];
         if (L_out) L_out[(size_t)k * p.M + m[r]] = L[r];
         if (xT_out) {
           float* o = xT_out + ((size_t)k * p.M + m[r]) * NX;
@@ -520,15 +543,18 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
     __syncwarp();
   }
 
-  float Lbar = 0.0f;
-  float cvar = cvar_select<G>(keys, p.R_total, lane, p.k_tail, p.M, mask, p.B != 1.0f, &Lbar);
-  // (18)-(19) PAPER.md:144-148: L_a = B (L - Lbar) + Lbar is affine-monotone for B > 0, so
-  // CVaR(L_a) = B (CVaR(L) - Lbar) + Lbar.
-  if (p.B != 1.0f) cvar = fmaf(p.B, cvar - Lbar, Lbar);
-  if (sub == 0 && k_valid) {
-    // soft filter (14)-(16) PAPER.md:120-130, strict threshold (15)
-    p.cvar[k] = cvar;
-    p.pen[k] = (cvar > p.C_u) ? (double)(p.A * cvar) : 0.0;   // J_C of (14); S~ = S + J_C is formed by its readers
+#pragma unroll
+  for (int r = 0; r < (HALF ? RC : 1); ++r) {   // HALF: the two samples of every slot; otherwise the warp's one sample
+    float Lbar = 0.0f;
+    float cvar = cvar_select<G>(keys_of[r], p.R_total, lane, p.k_tail, p.M, mask, p.B != 1.0f, &Lbar);
+    // (18)-(19) PAPER.md:144-148: L_a = B (L - Lbar) + Lbar is affine-monotone for B > 0, so
+    // CVaR(L_a) = B (CVaR(L) - Lbar) + Lbar.
+    if (p.B != 1.0f) cvar = fmaf(p.B, cvar - Lbar, Lbar);
+    if (sub == 0 && k_valid_of[r]) {
+      // soft filter (14)-(16) PAPER.md:120-130, strict threshold (15)
+      p.cvar[k_of[r]] = cvar;
+      p.pen[k_of[r]] = (cvar > p.C_u) ? (double)(p.A * cvar) : 0.0;   // J_C of (14); S~ = S + J_C is formed by its readers
+    }
   }
 }
 

@@ -15,11 +15,12 @@ namespace {
 
 template <int NOISE, int RC, bool HALF>
 cudaError_t launch(const Params& p, const float* d_x0, float* d_L, float* d_xT, cudaStream_t stream, bool pdl) {
-  const int samples_per_cta = HALF ? 2 * kRolloutWarps : kRolloutWarps / p.wps;
+  const int samples_per_cta = HALF ? 2 * RC * kRolloutWarps : kRolloutWarps / p.wps;
   const int grid = (p.K + samples_per_cta - 1) / samples_per_cta;
-  const int ce_slots = HALF ? 2 * kRolloutWarps : kRolloutWarps / p.wps;
+  const int ce_slots = samples_per_cta;
+  const int key_rows = kRolloutWarps * (HALF ? RC : p.R_total);
   const size_t smem = ((RA_INST_RISK == RISK_CIRCLES || RA_INST_RISK == RISK_NOMINAL) ? (size_t)((p.n_circles + 31) & ~31) * sizeof(float4) : 0) +
-                      (size_t)ce_slots * p.T * sizeof(float4) + (size_t)kRolloutWarps * p.R_total * 32 * sizeof(uint32_t);
+                      (size_t)ce_slots * p.T * sizeof(float4) + (size_t)key_rows * 32 * sizeof(uint32_t);
   auto kernel = noisy_rollout_kernel<RA_INST_DYN, RA_INST_RISK, NOISE, RC, HALF>;
   if (smem > 48 * 1024) {   // worst case (1024 circles, T = 128, M = 512) is 65 KB
     static std::atomic<int> smem_set[kMaxDevices];
@@ -37,7 +38,10 @@ cudaError_t launch(const Params& p, const float* d_x0, float* d_L, float* d_xT, 
 template <int NOISE>
 cudaError_t launch_noise(const Params& p, int rc, bool half, const float* d_x0, float* d_L, float* d_xT,
                          cudaStream_t stream, bool pdl) {
-  if (half) return launch<NOISE, 1, true>(p, d_x0, d_L, d_xT, stream, pdl);
+  if (half) {   // M <= 16: half a warp per sample, 2 rc samples per warp
+    if (rc == 2) return launch<NOISE, 2, true>(p, d_x0, d_L, d_xT, stream, pdl);
+    return rc == 1 ? launch<NOISE, 1, true>(p, d_x0, d_L, d_xT, stream, pdl) : cudaErrorInvalidValue;
+  }
   switch (rc) {
     case 1: return launch<NOISE, 1, false>(p, d_x0, d_L, d_xT, stream, pdl);
     case 2: return launch<NOISE, 2, false>(p, d_x0, d_L, d_xT, stream, pdl);

@@ -118,7 +118,8 @@ def test_iteration_enters_the_counter(torch_cuda, iteration):
 
 # ------------------------------------------------------------------ edge cases
 @pytest.mark.parametrize("K,M,T", [(1, 1, 1), (3, 1, 7), (5, 2, 3), (9, 17, 5), (33, 20, 9), (17, 50, 11),
-                                    (6, 300, 30), (4, 512, 8), (2, 96, 128), (31, 33, 2)])
+                                    (6, 300, 30), (4, 512, 8), (2, 96, 128), (31, 33, 2),
+                                    (32771, 9, 6), (32769, 16, 3)])   # M <= 16 with four samples per warp (K >= 32768), ragged K
 def test_ragged_and_extreme_sizes(torch_cuda, K, M, T):
     p = W.small(W.config0(near_obstacle=True), K=K, M=M, T=T)
     p = _with_v(p.replace(sigma_w=[0.05, 0.05, 0.02, 0.1]))
