@@ -328,7 +328,7 @@ def run_cuda(args):
             "iterations_per_s": world * args.steps / (total_ms * 1e-3),
             "wall_ms_per_step_incl_flush": 1e3 * t_wall / args.steps,
             "clocks": sampler.summary(),
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(4 * (p.nx + 2 * p.T)),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(4 * (8 + 2 * p.T)),
                     "d2h_bytes_per_step": int(4 * 2 * p.T), "ms_per_step": e2e_ms / args.steps,
                     "api": "ra_mppi_step_host (pinned host x0, v -> v+)"},
             "gpu_launches": int(ctl.launches_per_step * args.steps),

@@ -157,9 +157,10 @@ ra_status ra_mppi_plant_shift(ra_mppi_ctx* ctx, float* d_x0, float* d_v, float* 
 ra_status ra_mppi_closed_loop(ra_mppi_ctx* ctx, float* d_x0, float* d_v, uint64_t iteration0,
                               int32_t n_iter, float* d_log, float* h_ms, void* cuda_stream);
 
-/* ra_mppi_step with HOST buffers: h_x0 [n_x] and h_v [T,2] (in: v, out: v+) are copied to the
- * context's device staging buffers, the step runs, v+ is copied back, and the call returns after
- * the stream has drained.  Pinned host memory makes the copies asynchronous; pageable works.  */
+/* ra_mppi_step with HOST buffers: h_x0 [n_x] and h_v [T,2] (in: v, out: v+) go through the context's pinned
+ * staging buffer (one host-to-device copy of iteration, x0 and v together, the step, one device-to-host copy of v+),
+ * submitted as one CUDA graph captured on first use; the call returns after the stream has drained with v+ in h_v.
+ * Any host memory works (pinned or pageable).  Results are bit-identical to ra_mppi_step on device buffers.       */
 ra_status ra_mppi_step_host(ra_mppi_ctx* ctx, const float* h_x0, float* h_v, uint64_t iteration,
                             void* cuda_stream);
 

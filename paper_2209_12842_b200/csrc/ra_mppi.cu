@@ -40,7 +40,13 @@ struct ra_mppi_ctx {
   LoopState* d_loop = nullptr;
   // closed-loop graph cache
   // host-buffer staging (ra_mppi_step_host) and optional kernel timing
-  float* d_stage = nullptr;  // [nx + 2T]
+  // ra_mppi_step_host: staging buffer [8 + 2T] floats = { iteration (u64), x0 (6 floats), v [T,2] } on the device and, pinned,
+  // on the host (one copy each way whatever memory the caller passes), and the whole call captured once as a CUDA graph
+  // (H2D copy, the step's kernels reading the iteration from the staging buffer, D2H copy): one launch call per step
+  float* d_stage = nullptr;
+  float* h_stage = nullptr;
+  cudaGraphExec_t host_graph = nullptr;
+  bool host_graph_failed = false;
   bool pdl = true;     // programmatic dependent launch of the kernels that follow a kernel on the caller's stream
   bool timing = false;
   bool timed = false;  // ev_k0 / ev_k1 hold a rollout-kernel interval recorded outside a stream capture
@@ -362,7 +368,8 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
       dev_alloc(&c->d_S, (size_t)cfg->K) != cudaSuccess || dev_alloc(&c->d_cvar, (size_t)cfg->K) != cudaSuccess ||
       dev_alloc(&c->d_pen, (size_t)cfg->K) != cudaSuccess || dev_alloc(&c->d_split, (size_t)kMaxUpdateSplits * (2 + 2 * cfg->T)) != cudaSuccess || dev_alloc(&c->d_loop, 1) != cudaSuccess ||
       dev_alloc(&c->d_done, 1) != cudaSuccess ||
-      dev_alloc(&c->d_stage, (size_t)(8 + 2 * cfg->T)) != cudaSuccess)
+      dev_alloc(&c->d_stage, (size_t)(8 + 2 * cfg->T)) != cudaSuccess ||
+      cudaHostAlloc(reinterpret_cast<void**>(&c->h_stage), (size_t)(8 + 2 * cfg->T) * sizeof(float), cudaHostAllocDefault) != cudaSuccess)
     return bail(RA_ENOMEM);
   p.u_raw = c->d_u_raw; p.ce = c->d_ce; p.S = c->d_S; p.cvar = c->d_cvar; p.pen = c->d_pen;
   if (cudaMemset(c->d_loop, 0, sizeof(LoopState)) != cudaSuccess || cudaMemset(c->d_done, 0, sizeof(unsigned int)) != cudaSuccess ||
@@ -388,8 +395,10 @@ ra_status ra_mppi_destroy(ra_mppi_ctx* c) {
   if (!c) return RA_OK;
   DeviceGuard on_device(c->cfg.device);
   if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+  if (c->host_graph) cudaGraphExecDestroy(c->host_graph);
   cudaFree(c->d_circles); cudaFree(c->d_costmap); cudaFree(c->d_u_raw); cudaFree(c->d_ce);
   cudaFree(c->d_stage);
+  if (c->h_stage) cudaFreeHost(c->h_stage);
   if (c->ev_fork) cudaEventDestroy(c->ev_fork);
   if (c->ev_join) cudaEventDestroy(c->ev_join);
   if (c->side) cudaStreamDestroy(c->side);
@@ -415,6 +424,7 @@ ra_status ra_mppi_set_env(ra_mppi_ctx* c, const ra_mppi_env* env) {
   // earlier launches may still read the old copies; a captured graph holds the old sizes in its kernel arguments
   RA_CUDA(c, cudaDeviceSynchronize());
   if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+  if (c->host_graph) { cudaGraphExecDestroy(c->host_graph); c->host_graph = nullptr; }
   return upload_env(c, env, false);
 }
 
@@ -626,14 +636,42 @@ ra_status ra_mppi_step_host(ra_mppi_ctx* c, const float* h_x0, float* h_v, uint6
   if (!h_x0 || !h_v) return fail(c, RA_EINVAL, "null host pointer");
   RA_ON_DEVICE(c);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
-  float* d_x0 = c->d_stage;
+  float* d_x0 = c->d_stage + 2;
   float* d_v = c->d_stage + 8;
-  const size_t nv = (size_t)2 * c->p.T * sizeof(float);
-  RA_CUDA(c, cudaMemcpyAsync(d_x0, h_x0, (size_t)c->p.nx * sizeof(float), cudaMemcpyHostToDevice, s));
-  RA_CUDA(c, cudaMemcpyAsync(d_v, h_v, nv, cudaMemcpyHostToDevice, s));
-  if (ra_status st = ra_mppi_step(c, d_x0, d_v, iteration, stream)) return st;
-  RA_CUDA(c, cudaMemcpyAsync(h_v, d_v, nv, cudaMemcpyDeviceToHost, s));
+  const size_t nv = (size_t)2 * c->p.T;
+  std::memcpy(c->h_stage, &iteration, sizeof(uint64_t));
+  std::memcpy(c->h_stage + 2, h_x0, (size_t)c->p.nx * sizeof(float));
+  std::memcpy(c->h_stage + 8, h_v, nv * sizeof(float));
+  // The whole call as one graph launch (captured on first use; a timed step and a failed capture take the call-by-call path)
+  if (!c->host_graph && !c->host_graph_failed && !c->timing) {
+    cudaStream_t cs = nullptr;
+    cudaGraph_t graph = nullptr;
+    ra_status st = RA_OK;
+    if (cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking) == cudaSuccess &&
+        cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+      Params p = c->p;
+      p.d_iter = reinterpret_cast<const unsigned long long*>(c->d_stage);
+      p.iter_imm = 0;
+      if (cudaMemcpyAsync(c->d_stage, c->h_stage, (8 + nv) * sizeof(float), cudaMemcpyHostToDevice, cs) != cudaSuccess) st = RA_ECUDA;
+      if (st == RA_OK) st = enqueue_costs(c, p, d_x0, d_v, nullptr, nullptr, cs, false);
+      if (st == RA_OK) st = enqueue_update(c, p, d_v, cs, UpdateTail{nullptr, nullptr, nullptr});
+      if (st == RA_OK && cudaMemcpyAsync(c->h_stage + 8, d_v, nv * sizeof(float), cudaMemcpyDeviceToHost, cs) != cudaSuccess) st = RA_ECUDA;
+      const cudaError_t e = cudaStreamEndCapture(cs, &graph);
+      if (st != RA_OK || e != cudaSuccess || cudaGraphInstantiate(&c->host_graph, graph, 0) != cudaSuccess) c->host_graph = nullptr;
+      if (graph) cudaGraphDestroy(graph);
+    }
+    if (cs) cudaStreamDestroy(cs);
+    if (!c->host_graph) { c->host_graph_failed = true; (void)cudaGetLastError(); }
+  }
+  if (c->host_graph && !c->timing) {
+    RA_CUDA(c, cudaGraphLaunch(c->host_graph, s));
+  } else {
+    RA_CUDA(c, cudaMemcpyAsync(c->d_stage, c->h_stage, (8 + nv) * sizeof(float), cudaMemcpyHostToDevice, s));
+    if (ra_status st = ra_mppi_step(c, d_x0, d_v, iteration, stream)) return st;
+    RA_CUDA(c, cudaMemcpyAsync(c->h_stage + 8, d_v, nv * sizeof(float), cudaMemcpyDeviceToHost, s));
+  }
   RA_CUDA(c, cudaStreamSynchronize(s));
+  std::memcpy(h_v, c->h_stage + 8, nv * sizeof(float));
   return RA_OK;
 }
 

@@ -10,17 +10,7 @@
 
 namespace ra {
 
-#ifndef RA_ROLLOUT_THREADS
-#define RA_ROLLOUT_THREADS 256
-#endif
-constexpr int kRolloutThreads = RA_ROLLOUT_THREADS;
-#define RA_PRAGMA_(x) _Pragma(#x)
-#define RA_PRAGMA(x) RA_PRAGMA_(x)
-#ifdef RA_T_UNROLL
-#define RA_T_LOOP_UNROLL RA_PRAGMA(unroll RA_T_UNROLL)
-#else
-#define RA_T_LOOP_UNROLL
-#endif
+constexpr int kRolloutThreads = 256;
 constexpr int kRolloutWarps = kRolloutThreads / 32;
 constexpr int NOISE_MATERIALISED = 3;  // rollout-kernel variant that reads w from HBM
 
@@ -56,10 +46,7 @@ __global__ void __launch_bounds__(kSampleThreads) sample_kernel(const __grid_con
 // S is accumulated in fp64 (K*T adds only) because the softmin weights of (17) are sensitive to
 // absolute errors in S~.  Independent of the noisy rollouts, so ra_mppi_step runs it beside them.
 // ---------------------------------------------------------------------------------------
-#ifndef RA_NOMINAL_THREADS
-#define RA_NOMINAL_THREADS 64
-#endif
-constexpr int kNominalThreads = RA_NOMINAL_THREADS;
+constexpr int kNominalThreads = 64;
 
 template <int DYN, int NOM>
 __global__ void __launch_bounds__(kNominalThreads) nominal_kernel(const __grid_constant__ Params p,
@@ -285,15 +272,9 @@ __device__ __forceinline__ void risk_accumulate(const Params& p, const float4* c
 // faster with 2 CTAs/SM than with 3 CTAs of 80 registers (C3 0.458 -> 0.445 ms); the bicycle + circles kernels
 // (87 registers at most) and everything with RC <= 2 are faster with 3 (C1, C4, M = 256 sweep points).
 // Throughput-, not latency-bound: 4-6 CTAs/SM are slower everywhere.
-#ifndef RA_MIN_CTAS_RC4
-#define RA_MIN_CTAS_RC4 2
-#endif
-#ifndef RA_MIN_CTAS_RC12
-#define RA_MIN_CTAS_RC12 3
-#endif
 template <int DYN, int RISK, int RC>
 constexpr int rollout_min_ctas() {
-  return (RC == 4 && (DYN == DYN_SINGLE_TRACK || RISK == RISK_COSTMAP)) ? RA_MIN_CTAS_RC4 : RA_MIN_CTAS_RC12;
+  return (RC == 4 && (DYN == DYN_SINGLE_TRACK || RISK == RISK_COSTMAP)) ? 2 : 3;
 }
 template <int DYN, int RISK, int NOISE, int RC, bool HALF>
 __global__ void __launch_bounds__(kRolloutThreads, rollout_min_ctas<DYN, RISK, RC>())
@@ -509,7 +490,6 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
         advance(t, a);
       }
     } else {
-      RA_T_LOOP_UNROLL
       for (int t = 0; t < p.T; ++t) {
         float a[RC][NX];
 #pragma unroll
