@@ -69,12 +69,14 @@ def load_counters():
 
 
 def counter_key(name: str) -> str:
-    """Which capture describes workload `name`: the C4 sweep points share a kernel per M (captured at K = 16384)."""
+    """Which capture describes workload `name`: the C4 sweep points share a kernel per M (captured at K = 16384), except
+    M = 16 from K = 32768, where a warp carries four samples instead of two (captured at K = 65536)."""
     name = name.upper()
     if name.startswith("C4"):
         parts = name.split("-")
+        K = int(parts[1][1:]) if len(parts) > 1 else 8192
         M = parts[2] if len(parts) > 2 else "M64"
-        return f"C4-{M}"
+        return f"C4-{M}-4PERWARP" if (M == "M16" and K >= 32768) else f"C4-{M}"
     return name
 
 
