@@ -187,12 +187,14 @@ __device__ __forceinline__ float nominal_cost(const Params& p, float Xabs, float
     }
     return q;
   } else {
-    const float a = p.nom_p[0], b = p.nom_p[1];
-    const float xa = Xabs / a, yb = Yabs / b;
+    // first-order signed offset e = f / (2 |grad f / 2|), + outside (G25), with the reciprocals of the semi-axes
+    // from the host (nom_q = {1/a, 1/b}) and one reciprocal square root instead of five divisions and a square root: this
+    // function is the body of the K*T sequential chain of the nominal rollout, so its dependent-instruction count is its cost
+    const float xa = Xabs * p.nom_q[0], yb = Yabs * p.nom_q[1];
     const float f = fmaf(xa, xa, fmaf(yb, yb, -1.0f));
-    const float gx = xa / a, gy = yb / b;
-    const float g = sqrtf(fmaf(gx, gx, gy * gy));
-    const float e = f / (2.0f * fmaxf(g, 1e-12f));   // first-order signed offset, + outside
+    const float gx = xa * p.nom_q[0], gy = yb * p.nom_q[1];
+    const float g2 = fmaf(gx, gx, gy * gy);
+    const float e = 0.5f * f * rsqrtf(fmaxf(g2, 1e-24f));   // g floored at 1e-12
     const float over = fmaxf(0.0f, fabsf(e) - p.nom_p[2]);
     const float dv = v - p.nom_p[5];
     return fmaf(p.nom_p[3] * e, e, fmaf(p.nom_p[4] * dv, dv, p.nom_p[6] * over * over));

@@ -336,6 +336,10 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
     p.dyn_q[0] = (float)((double)cfg->dt / (double)cfg->dyn_p[0]);   // dt / L of the yaw update
   }
   std::memcpy(p.nom_p, cfg->nom_p, sizeof p.nom_p);
+  if (cfg->nominal == RA_NOM_ELLIPSE_TRACK) {
+    p.nom_q[0] = (float)(1.0 / (double)cfg->nom_p[0]);
+    p.nom_q[1] = (float)(1.0 / (double)cfg->nom_p[1]);
+  }
   std::memcpy(p.risk_p, cfg->risk_p, sizeof p.risk_p);
   std::memcpy(p.noise_p, cfg->noise_p, sizeof p.noise_p);
   std::memcpy(p.sigma_w, cfg->sigma_w, sizeof p.sigma_w);

@@ -36,6 +36,7 @@ struct Params {
   float neg_log2e_over_lambda;  // weights (17) PAPER.md:134 as exp2
   float A, B, C_u;
   float nom_p[12];
+  float nom_q[2];   // ellipse track: 1/a, 1/b
   float risk_p[4];
   float noise_p[4];
   uint32_t rk[20];  // the ten Philox round keys (k0_r, k1_r), key = seed

@@ -65,12 +65,29 @@ __global__ void __launch_bounds__(kNominalThreads) nominal_kernel(const __grid_c
   if constexpr (DYN == DYN_SINGLE_TRACK) x[3] = fmaxf(x[3], p.dyn_p[6]);
   const float4* ce_k = p.ce + (size_t)k * p.T;
   double S = 0.0;
-  for (int t = 0; t < p.T; ++t) {
-    const float2 u = p.u_raw[(size_t)t * p.K + k];
-    const float ctrl = fmaf(p.ctrl_w[0] * __ldg(v + 2 * t), u.x, p.ctrl_w[1] * __ldg(v + 2 * t + 1) * u.y);  // gamma v^T Sigma^-1 u  (3)
-    const float q = nominal_cost<NOM>(p, x0X + x[0], x0Y + x[1], x[3]);
-    S += (double)q + (double)ctrl;
-    dynamics_step<DYN>(p, x, ce_k[t]);
+  // The step is a dependent chain, and its inputs (u, ce: two L2 loads per step) do not depend on it: fetch them a block
+  // of steps ahead, so the chain pays the load latency once per block instead of once per step (nominal kernel at
+  // K = 16384, T = 50: 36 -> 22 us with the shorter cost chain, -> 11 us with the blocked loads).
+  constexpr int kBlock = 8;
+  for (int t0 = 0; t0 < p.T; t0 += kBlock) {
+    float2 ub[kBlock];
+    float4 cb[kBlock];
+#pragma unroll
+    for (int j = 0; j < kBlock; ++j) {
+      const int t = min(t0 + j, p.T - 1);
+      ub[j] = p.u_raw[(size_t)t * p.K + k];
+      cb[j] = ce_k[t];
+    }
+#pragma unroll
+    for (int j = 0; j < kBlock; ++j) {
+      const int t = t0 + j;
+      if (t < p.T) {
+        const float ctrl = fmaf(p.ctrl_w[0] * __ldg(v + 2 * t), ub[j].x, p.ctrl_w[1] * __ldg(v + 2 * t + 1) * ub[j].y);  // gamma v^T Sigma^-1 u  (3)
+        const float q = nominal_cost<NOM>(p, x0X + x[0], x0Y + x[1], x[3]);
+        S += (double)q + (double)ctrl;
+        dynamics_step<DYN>(p, x, cb[j]);
+      }
+    }
   }
   S += (double)terminal_cost<NOM>(p, x0X + x[0], x0Y + x[1], x[3], x0X, x0Y);
   p.S[k] = S;
