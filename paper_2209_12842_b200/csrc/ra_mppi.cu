@@ -311,6 +311,11 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
   c->rc = (c->half && cfg->K >= 32768) ? 2 : 1;
   if (!c->half) {
     c->rc = (p.R_total >= 4 && p.R_total % 4 == 0) ? 4 : (p.R_total >= 2 ? 2 : 1);
+    // The costmap kernel prefers two slots per lane at 80 registers and 3 CTAs/SM (6 warps per scheduler instead of 4) now
+    // that it is co-limited by issue slots and the MUFU queue: C3 rollout 0.359 -> 0.343 ms.  The circle and single-track
+    // kernels keep four (their per-step culling and their dynamics amortise over the slots: RC = 2 costs them 4-6 %).
+    // The materialised-noise variant streams four rows per step and lane better (5.1 against 4.5 TB/s).
+    if (cfg->risk == RA_RISK_COSTMAP && cfg->dyn == RA_DYN_KINEMATIC_BICYCLE && cfg->noise_mode == RA_NOISE_FUSED && c->rc == 4) c->rc = 2;
     const int groups = (p.R_total + c->rc - 1) / c->rc;
     while (p.wps < 8 && p.wps < groups) p.wps *= 2;
   }
