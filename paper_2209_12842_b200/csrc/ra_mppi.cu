@@ -530,12 +530,19 @@ int update_splits(const ra_mppi_ctx* c) {
   return std::max(1, std::min(kMaxUpdateSplits, (c->p.K + per_cta - 1) / per_cta));
 }
 
+// steps of the horizon one update CTA takes: as many as keep the grid at about two CTAs per SM (at least one)
+int update_steps_per_cta(const ra_mppi_ctx* c, int splits) {
+  const int want = (c->p.T * splits) / (2 * std::max(c->n_sm, 1));
+  return std::max(1, std::min(kUpdateMaxSteps, want));
+}
+
 ra_status enqueue_update(ra_mppi_ctx* c, const Params& p, float* d_v_out, cudaStream_t s, UpdateTail tail) {
   // a programmatic dependent of the rollout kernel (of the nominal kernel when A = 0); the join with the side stream
   // before it is a full dependency.  A timed step keeps plain launches.
-  RA_CUDA(c, launch_kernel(weights_update_kernel<double>, dim3(p.T, update_splits(c)), dim3(kUpdateThreads), 0, s,
+  const int splits = update_splits(c), steps = update_steps_per_cta(c, splits);
+  RA_CUDA(c, launch_kernel(weights_update_kernel<double>, dim3((p.T + steps - 1) / steps, splits), dim3(kUpdateThreads), 0, s,
                            c->pdl && !c->timing, p, (const double*)p.S, (const double*)p.pen, (const float2*)p.u_raw, 1LL,
-                           (long long)p.K, d_v_out, (float*)nullptr, (float*)nullptr, c->d_split, c->d_done, tail));
+                           (long long)p.K, d_v_out, (float*)nullptr, (float*)nullptr, c->d_split, c->d_done, tail, steps));
   return RA_OK;
 }
 
@@ -544,7 +551,7 @@ ra_status enqueue_partial(ra_mppi_ctx* c, const Params& p, double* d_partial, cu
   RA_CUDA(c, launch_kernel(weights_update_kernel<double>, dim3(p.T, 1), dim3(kUpdateThreads), 0, s, c->pdl && !c->timing, p,
                            (const double*)p.S, (const double*)p.pen, (const float2*)p.u_raw, 1LL, (long long)p.K,
                            (float*)nullptr, (float*)nullptr, (float*)nullptr, d_partial, (unsigned int*)nullptr,
-                           UpdateTail{nullptr, nullptr, nullptr}));
+                           UpdateTail{nullptr, nullptr, nullptr}, 1));
   return RA_OK;
 }
 
@@ -625,7 +632,7 @@ ra_status ra_mppi_weights_update(ra_mppi_ctx* c, const float* d_S_tilde, const f
   const Params p = with_iteration(c, 0);
   weights_update_kernel<float><<<p.T, kUpdateThreads, 0, s>>>(
       p, d_S_tilde, nullptr, reinterpret_cast<const float2*>(d_u), (long long)p.T, 1LL, d_v_plus, d_w, d_stats, nullptr,
-      nullptr, UpdateTail{nullptr, nullptr, nullptr});
+      nullptr, UpdateTail{nullptr, nullptr, nullptr}, 1);
   RA_CUDA(c, cudaGetLastError());
   return RA_OK;
 }

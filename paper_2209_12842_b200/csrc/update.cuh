@@ -125,10 +125,11 @@ __global__ void combine_partials_kernel(const __grid_constant__ Params p, const 
 }
 
 // ---------------------------------------------------------------------------------------
-// A8 + A9.  One CTA per (horizon step t, sample range blockIdx.y of gridDim.y).  Each CTA recomputes
-// beta~ = min_k S~_k over its range (values from L2), then w~_k = exp(-(S~_k - beta~)/lambda), Z = sum w~, and
-// N_t = sum_k w~_k u^k_t   (17) PAPER.md:134, (5) :55, (4) :51.  T CTAs alone leave most SMs idle, so the samples are
-// cut into gridDim.y ranges.  Three uses:
+// A8 + A9.  One CTA per (group of steps_per_cta horizon steps, sample range blockIdx.y of gridDim.y).  Each CTA forms
+// beta~ = min_k S~_k over its range (values from L2), w~_k = exp(-(S~_k - beta~)/lambda) and Z = sum w~ ONCE, then
+// N_t = sum_k w~_k u^k_t for each of its steps   (17) PAPER.md:134, (5) :55, (4) :51.  The host picks the ranges (what a CTA
+// caches in registers) and then the group size so that the grid is about two CTAs per SM: at large K this stops every
+// step's CTA from re-reading the range's costs (K = 65536: 50 re-reads -> 9).  Three uses:
 //   * ra_mppi_step: the CTA writes its range's {beta, Z, N_t} into `partial` (context scratch); the LAST CTA of the grid
 //     to finish (an atomic ticket in *done) combines the ranges into v+ = clamp(N / Z) -- in a fixed order, so the
 //     result does not depend on which CTA that was -- and, inside the captured closed loop (tail.x0g != nullptr), goes on
@@ -151,22 +152,28 @@ struct UpdateTail {          // closed-loop tail of the update kernel (all null 
   LoopState* loop;
 };
 
+constexpr int kUpdateMaxSteps = 8;    // horizon steps one CTA may take (its samples' weights are formed once and reused)
+
 template <typename ST>
 __global__ void __launch_bounds__(kUpdateThreads)
 weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S_tilde,
                       const double* __restrict__ pen, const float2* __restrict__ u, long long su_k, long long su_t,
                       float* v_out, float* __restrict__ w_out, float* __restrict__ stats, double* partial,
-                      unsigned int* done, UpdateTail tail) {
+                      unsigned int* done, UpdateTail tail, int steps_per_cta) {
+  constexpr int kWarps = kUpdateThreads / 32;
   __shared__ ST red_s[32];
-  __shared__ double red_f[96];
+  __shared__ double sm_z[kWarps];
+  __shared__ double sm_n[kUpdateMaxSteps][2][kWarps];
   __shared__ bool is_last;
   pdl_wait();   // launched as a programmatic dependent of the rollout kernel: its costs are read from here on
-  const int t = blockIdx.x;
+  const int t_first = blockIdx.x * steps_per_cta;
+  const int n_t = min(steps_per_cta, p.T - t_first);
   const int k_chunk = (p.K + gridDim.y - 1) / gridDim.y;
   const int k_begin = blockIdx.y * k_chunk, k_end = min(p.K, k_begin + k_chunk);
   double* my_partial = partial ? partial + (size_t)blockIdx.y * (2 + 2 * p.T) : nullptr;
-  // The kernel is a chain of memory round trips, so each thread fetches the costs AND the controls of its first
-  // kCached samples in one go and keeps them in registers across the min; the host cuts K into ranges of at most
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  // The kernel is a chain of memory round trips, so each thread fetches the costs AND the first step's controls of its
+  // first kCached samples in one go and keeps them in registers across the min; the host cuts K into ranges of at most
   // kCached * blockDim samples, and anything beyond (a caller's single range) takes the two-pass route through L1.
   constexpr int kCached = kUpdateCached;
   ST sc[kCached];
@@ -179,7 +186,7 @@ weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S
     uc[j] = make_float2(0.0f, 0.0f);
     if (k < k_end) {
       sc[j] = s_tilde_at<ST>(S_tilde, pen, k);
-      uc[j] = __ldg(u + (long long)k * su_k + (long long)t * su_t);
+      uc[j] = __ldg(u + (long long)k * su_k + (long long)t_first * su_t);
     }
     bmin = min(bmin, sc[j]);
   }
@@ -187,55 +194,68 @@ weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S
   for (int k = k_rest + threadIdx.x; k < k_end; k += blockDim.x) bmin = min(bmin, s_tilde_at<ST>(S_tilde, pen, k));
   const ST beta = block_reduce<ST>(bmin, red_s, [](ST a, ST b) { return a < b ? a : b; }, (ST)INFINITY);
 
-  // Z and the two numerators are summed in fp64: with soft weights (ESS >> 1) and K = 65536 an fp32 sum would
-  // spend a visible part of the 1e-4 budget of v+ on its own rounding.  Each w~ is an fp32 exp2 of an fp32 argument
-  // (an empty slot holds S~ = +inf, hence weight exactly 0).
-  double Z = 0.0, n0 = 0.0, n1 = 0.0;
+  // w~_k once per sample (an empty slot holds S~ = +inf, hence weight exactly 0), reused for every step of this CTA.
+  // Z and the numerators are summed in fp64: with soft weights (ESS >> 1) and K = 65536 an fp32 sum would spend a
+  // visible part of the 1e-4 budget of v+ on its own rounding.  Each w~ is an fp32 exp2 of an fp32 argument.
+  float wc[kCached];
+  double Z = 0.0;
 #pragma unroll
   for (int j = 0; j < kCached; ++j) {
-    const float w = exp2f((float)(sc[j] - beta) * p.neg_log2e_over_lambda);
-    Z += (double)w;
-    n0 = fma((double)w, (double)uc[j].x, n0);
-    n1 = fma((double)w, (double)uc[j].y, n1);
+    wc[j] = exp2f((float)(sc[j] - beta) * p.neg_log2e_over_lambda);
+    Z += (double)wc[j];
   }
-  for (int k = k_rest + threadIdx.x; k < k_end; k += blockDim.x) {
-    const float w = exp2f((float)(s_tilde_at<ST>(S_tilde, pen, k) - beta) * p.neg_log2e_over_lambda);
-    const float2 uk = __ldg(u + (long long)k * su_k + (long long)t * su_t);
-    Z += (double)w;
-    n0 = fma((double)w, (double)uk.x, n0);
-    n1 = fma((double)w, (double)uk.y, n1);
-  }
-  // one fixed-order tree for the three sums (a single shared-memory exchange)
+  for (int k = k_rest + threadIdx.x; k < k_end; k += blockDim.x)
+    Z += (double)exp2f((float)(s_tilde_at<ST>(S_tilde, pen, k) - beta) * p.neg_log2e_over_lambda);
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    Z += __shfl_xor_sync(0xFFFFFFFFu, Z, o);
-    n0 += __shfl_xor_sync(0xFFFFFFFFu, n0, o);
-    n1 += __shfl_xor_sync(0xFFFFFFFFu, n1, o);
-  }
-  {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    if (lane == 0) { red_f[warp] = Z; red_f[32 + warp] = n0; red_f[64 + warp] = n1; }
-    __syncthreads();
-    Z = lane < nw ? red_f[lane] : 0.0;
-    n0 = lane < nw ? red_f[32 + lane] : 0.0;
-    n1 = lane < nw ? red_f[64 + lane] : 0.0;
+  for (int o = 16; o > 0; o >>= 1) Z += __shfl_xor_sync(0xFFFFFFFFu, Z, o);
+  if (lane == 0) sm_z[warp] = Z;
+  for (int tt = 0; tt < n_t; ++tt) {
+    const int t = t_first + tt;
+    float2 un[kCached];          // the next step's controls are fetched while this step's are summed
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      Z += __shfl_xor_sync(0xFFFFFFFFu, Z, o);
+    for (int j = 0; j < kCached; ++j) {
+      const int k = k_begin + threadIdx.x + j * (int)blockDim.x;
+      un[j] = (tt + 1 < n_t && k < k_end) ? __ldg(u + (long long)k * su_k + (long long)(t + 1) * su_t) : make_float2(0.0f, 0.0f);
+    }
+    double n0 = 0.0, n1 = 0.0;
+#pragma unroll
+    for (int j = 0; j < kCached; ++j) {
+      n0 = fma((double)wc[j], (double)uc[j].x, n0);
+      n1 = fma((double)wc[j], (double)uc[j].y, n1);
+      uc[j] = un[j];
+    }
+    for (int k = k_rest + threadIdx.x; k < k_end; k += blockDim.x) {
+      const float w = exp2f((float)(s_tilde_at<ST>(S_tilde, pen, k) - beta) * p.neg_log2e_over_lambda);
+      const float2 uk = __ldg(u + (long long)k * su_k + (long long)t * su_t);
+      n0 = fma((double)w, (double)uk.x, n0);
+      n1 = fma((double)w, (double)uk.y, n1);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {   // fixed-order tree inside the warp ...
       n0 += __shfl_xor_sync(0xFFFFFFFFu, n0, o);
       n1 += __shfl_xor_sync(0xFFFFFFFFu, n1, o);
     }
+    if (lane == 0) { sm_n[tt][0][warp] = n0; sm_n[tt][1][warp] = n1; }
   }
-  // one range, no closed-loop tail: this CTA owns v+_t outright, no exchange needed
+  __syncthreads();
+  // ... then over the warps, in order: thread (tt, i) finishes N_t[i]; every thread that needs Z forms the same sum
+  double Zt = 0.0;
+#pragma unroll
+  for (int w = 0; w < kWarps; ++w) Zt += sm_z[w];
+  const int my_tt = threadIdx.x >> 1, my_i = threadIdx.x & 1;
+  double N = 0.0;
+  if (my_tt < n_t) {
+#pragma unroll
+    for (int w = 0; w < kWarps; ++w) N += sm_n[my_tt][my_i][w];
+  }
+  // one range, no closed-loop tail: this CTA owns its v+_t outright, no exchange needed
   if (my_partial && done && gridDim.y == 1 && !tail.x0g) my_partial = nullptr;
   if (my_partial) {   // the range's / shard's unnormalised share {beta_g, Z_g, N_g[T][2]}
-    if (threadIdx.x == 0) {
-      if (t == 0) { my_partial[0] = (double)beta; my_partial[1] = Z; }
-      my_partial[2 + 2 * t] = n0;
-      my_partial[3 + 2 * t] = n1;
-    }
+    if (my_tt < n_t) my_partial[2 + 2 * (t_first + my_tt) + my_i] = N;
+    if (threadIdx.x == 0 && blockIdx.x == 0) { my_partial[0] = (double)beta; my_partial[1] = Zt; }
     if (!done) return;
     // last CTA to finish combines: its ticket is the last one, so every other CTA's partials are in L2
+    __syncthreads();             // this CTA's partial stores precede its ticket
     if (threadIdx.x == 0) {
       __threadfence();
       const unsigned int ticket = atomicAdd(done, 1u);
@@ -252,13 +272,10 @@ weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S
     }
     return;
   }
-  if (threadIdx.x == 0) {
-    v_out[2 * t] = clampf((float)(n0 / Z), p.u_min[0], p.u_max[0]);
-    v_out[2 * t + 1] = clampf((float)(n1 / Z), p.u_min[1], p.u_max[1]);
-    if (t == 0 && stats) { stats[0] = (float)beta; stats[1] = (float)Z; }
-  }
-  if (t == 0 && w_out) {
-    const float invZ = (float)(1.0 / Z);
+  if (my_tt < n_t) v_out[2 * (t_first + my_tt) + my_i] = clampf((float)(N / Zt), p.u_min[my_i], p.u_max[my_i]);
+  if (blockIdx.x == 0 && threadIdx.x == 0 && stats) { stats[0] = (float)beta; stats[1] = (float)Zt; }
+  if (blockIdx.x == 0 && w_out) {
+    const float invZ = (float)(1.0 / Zt);
     for (int k = threadIdx.x; k < p.K; k += blockDim.x)
       w_out[k] = exp2f((float)(s_tilde_at<ST>(S_tilde, pen, k) - beta) * p.neg_log2e_over_lambda) * invZ;
   }
