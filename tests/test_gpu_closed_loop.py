@@ -138,3 +138,38 @@ def test_step_is_capturable_in_a_caller_graph(torch_cuda):
     torch.cuda.synchronize()
     assert torch.equal(v_graph, v_eager)
     ctl.close()
+
+
+def test_step_host_graph_follows_set_env_and_timing_mode(torch_cuda):
+    """ra_mppi_step_host submits one captured graph per call: the capture must be dropped when the environment changes,
+    and the call-by-call path a timed step takes (plain launches, no programmatic dependent launch) must give the same bits."""
+    torch = torch_cuda
+    p = W.small(W.config1(), K=160, M=64, T=25)
+    p = p.replace(v=W.random_mean_control(p, 2))
+    moved = p.circles + np.array([0.1, -0.05, 0.02])
+    a, b = _ctl(p), _ctl(p.replace(circles=moved))
+    h_x0 = torch.tensor(np.asarray(p.x0, dtype=np.float32))
+    h_v0 = torch.tensor(np.asarray(p.v, dtype=np.float32))
+    va = h_v0.clone(); a.step_host(h_x0, va, 7)              # captures a's graph on the old environment
+    a.set_env(circles=moved)
+    va = h_v0.clone(); a.step_host(h_x0, va, 7)              # must re-capture
+    vb = h_v0.clone(); b.step_host(h_x0, vb, 7)
+    assert torch.equal(va, vb)
+    old = h_v0.clone(); _ctl(p).step_host(h_x0, old, 7)
+    assert not torch.equal(old, va)
+    # a second call replays the captured graph with a new iteration and new inputs
+    va2, vb2 = va.clone(), vb.clone()
+    a.step_host(h_x0, va2, 8); b.step(b.tensor(p.x0), (d := b.tensor(vb2.numpy())), 8)
+    torch.cuda.synchronize()
+    assert np.array_equal(va2.numpy(), d.cpu().numpy())
+    # timed steps (plain launches) == untimed steps (update kernel as a programmatic dependent of the rollout kernel)
+    d1, d2 = b.tensor(p.v), b.tensor(p.v)
+    b.step(b.tensor(p.x0), d1, 3)
+    b.enable_kernel_timing(True)
+    b.step(b.tensor(p.x0), d2, 3)
+    assert b.last_rollout_ms() > 0
+    vt = h_v0.clone(); b.step_host(h_x0, vt, 3)              # timing on: the call-by-call path
+    b.enable_kernel_timing(False)
+    torch.cuda.synchronize()
+    assert torch.equal(d1, d2) and np.array_equal(vt.numpy(), d1.cpu().numpy())
+    a.close(); b.close()
