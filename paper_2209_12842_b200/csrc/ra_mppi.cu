@@ -21,7 +21,7 @@ struct ra_mppi_ctx {
   ra_mppi_config cfg{};
   Params p{};
   int rc = 1;          // realisations interleaved per lane in the rollout kernel
-  bool half = false;   // two samples per warp
+  bool half = false;   // M <= 16: half a warp per sample (2 rc samples per warp)
   int noise_variant = 0;
   int n_sm = 0;        // multiprocessors of cfg.device (grid sizing of the small kernels)
   RolloutLaunchFn rollout = nullptr;
