@@ -66,13 +66,18 @@ _lib = None
 def load():
     """Load libra_mppi.so; raises if it has not been built (no fallback)."""
     global _lib
-    if _lib is not None:
-        return _lib
-    if not os.path.exists(LIB_PATH):
+    if _lib is None:
+        _lib = open_library(LIB_PATH)
+    return _lib
+
+
+def open_library(path):
+    """A configured ctypes handle of the library at `path` (the product library, or the checked build the tests use)."""
+    if not os.path.exists(path):
         raise RaMppiError(RA_ECUDA, "load",
-                          f"{LIB_PATH} is missing: run `python -m paper_2209_12842_b200.build` "
+                          f"{path} is missing: run `python -m paper_2209_12842_b200.build` "
                           "(or __graft_entry__.build()); there is no CPU fallback")
-    L = C.CDLL(LIB_PATH)
+    L = C.CDLL(path)
     vp, fp, u64, i32 = C.c_void_p, C.c_void_p, C.c_uint64, C.c_int32
     L.ra_mppi_create.argtypes = [C.POINTER(ra_mppi_config), C.POINTER(ra_mppi_env), C.POINTER(vp)]
     L.ra_mppi_set_env.argtypes = [vp, C.POINTER(ra_mppi_env)]
@@ -100,7 +105,6 @@ def load():
     for name in EXPORTS:
         if name not in ("ra_mppi_launches_per_step", "ra_mppi_last_error"):
             getattr(L, name).restype = C.c_int
-    _lib = L
     return L
 
 

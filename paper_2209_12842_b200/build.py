@@ -1,6 +1,9 @@
 """Build libra_mppi.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a.
 
-    python -m paper_2209_12842_b200.build [--force]
+    python -m paper_2209_12842_b200.build [--force] [--checked]
+
+--checked builds libra_mppi_checked.so, the same sources with -DRA_CHECKED: every kernel asserts its own indices
+(compute-sanitizer is closed on the GPU pool); tests/test_gpu_checked_build.py runs parity cases through it.
 
 The rollout kernel is instantiated per (dynamics, risk) pair in separate translation units
 so they compile in parallel.  No torch headers are involved: the library is plain CUDA.
@@ -26,21 +29,27 @@ def _sources():
     return [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC))] + [os.path.join(INCLUDE, "ra_mppi.h")]
 
 
-def _jobs():
-    jobs = [(os.path.join(CSRC, "ra_mppi.cu"), os.path.join(OBJ, "ra_mppi.o"), []),
-            (os.path.join(CSRC, "pipe_peaks.cu"), os.path.join(OBJ, "pipe_peaks.o"), [])]
+LIB_CHECKED = os.path.join(HERE, "libra_mppi_checked.so")
+
+
+def _jobs(obj_dir, defs0):
+    jobs = [(os.path.join(CSRC, "ra_mppi.cu"), os.path.join(obj_dir, "ra_mppi.o"), list(defs0)),
+            (os.path.join(CSRC, "pipe_peaks.cu"), os.path.join(obj_dir, "pipe_peaks.o"), list(defs0))]
     for d in (0, 1):
         for r in (0, 1, 2, 3):
-            jobs.append((os.path.join(CSRC, "rollout_inst.cu"), os.path.join(OBJ, f"rollout_{d}_{r}.o"),
-                         [f"-DRA_INST_DYN={d}", f"-DRA_INST_RISK={r}"]))
+            jobs.append((os.path.join(CSRC, "rollout_inst.cu"), os.path.join(obj_dir, f"rollout_{d}_{r}.o"),
+                         list(defs0) + [f"-DRA_INST_DYN={d}", f"-DRA_INST_RISK={r}"]))
     return jobs
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, checked: bool = False) -> str:
+    lib = LIB_CHECKED if checked else LIB
+    obj_dir = OBJ + "_checked" if checked else OBJ
+    jobs = _jobs(obj_dir, ["-DRA_CHECKED"] if checked else [])
     newest = max(os.path.getmtime(s) for s in _sources() + [os.path.abspath(__file__)])
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
-        return LIB
-    os.makedirs(OBJ, exist_ok=True)
+    if not force and os.path.exists(lib) and os.path.getmtime(lib) >= newest:
+        return lib
+    os.makedirs(obj_dir, exist_ok=True)
     extra = ["-Xptxas", "-v"] if verbose else []
 
     def compile_one(job):
@@ -52,15 +61,15 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return r.stderr
 
     with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
-        logs = list(ex.map(compile_one, _jobs()))
+        logs = list(ex.map(compile_one, jobs))
     if verbose:
-        with open(os.path.join(OBJ, "ptxas.log"), "w") as f:
+        with open(os.path.join(obj_dir, "ptxas.log"), "w") as f:
             f.write("\n".join(logs))
-    objs = [j[1] for j in _jobs()]
-    cmd = ["nvcc", "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB, *objs, "-lcudart"]
+    objs = [j[1] for j in jobs]
+    cmd = ["nvcc", "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", lib, *objs, "-lcudart"]
     subprocess.run(cmd, check=True)
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, checked="--checked" in sys.argv))

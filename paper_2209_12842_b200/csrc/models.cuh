@@ -266,6 +266,7 @@ __device__ __forceinline__ float bilinear_weighted(const Params& p, const MapFra
   const uint32_t idx = __float_as_uint(jy) * (uint32_t)(p.map_w + 1) + __float_as_uint(jx);
   const float4* addr;
   asm("mov.b64 %0, {%1, %2};" : "=l"(addr) : "r"(f.addr_lo + (idx << 4)), "r"(f.addr_hi));
+  RA_DEVICE_CHECK(addr >= p.quadmap && addr < p.quadmap + (size_t)(p.map_h + 1) * (p.map_w + 1));
   const float4 q = __ldg(addr);
   return fmaf(ty, fmaf(tx, q.w, q.z), fmaf(tx, q.y, q.x));
 }

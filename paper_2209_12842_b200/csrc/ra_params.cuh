@@ -2,6 +2,23 @@
 // Built once per context on the host (ra_mppi.cu) and passed to every kernel by value.
 #pragma once
 #include <cstdint>
+#include <cstdio>
+
+// Bounds checks of the checked build (python -m paper_2209_12842_b200.build --checked -> libra_mppi_checked.so, used by
+// tests/test_gpu_checked_build.py): compute-sanitizer is closed on the GPU pool, so the kernels carry their own index
+// assertions, compiled out of the product library.  A failed check prints its condition and traps the kernel.
+#ifdef RA_CHECKED
+#define RA_DEVICE_CHECK(cond)                                                                   \
+  do {                                                                                          \
+    if (!(cond)) {                                                                              \
+      printf("RA_DEVICE_CHECK failed: %s (%s:%d) block %d thread %d\n", #cond, __FILE__, __LINE__, \
+             (int)blockIdx.x, (int)threadIdx.x);                                                \
+      __trap();                                                                                 \
+    }                                                                                           \
+  } while (0)
+#else
+#define RA_DEVICE_CHECK(cond) do { } while (0)
+#endif
 
 namespace ra {
 
@@ -64,6 +81,12 @@ struct Params {
 // passed launch_dependents.  Both are no-ops for plain launches.
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+
+__device__ __forceinline__ uint32_t dynamic_smem_bytes() {
+  uint32_t n;
+  asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(n));
+  return n;
+}
 
 __device__ __forceinline__ uint32_t iteration_field(const Params& p, uint32_t stream) {
   const unsigned long long it = p.d_iter ? *p.d_iter : p.iter_imm;

@@ -36,6 +36,7 @@ __global__ void __launch_bounds__(kSampleThreads) sample_kernel(const __grid_con
   const bool with_mean = k + p.k_off < p.K0;
   const float u0 = fmaf(p.sigma_eps[0], z0, with_mean ? __ldg(v + 2 * t) : 0.0f);
   const float u1 = fmaf(p.sigma_eps[1], z1, with_mean ? __ldg(v + 2 * t + 1) : 0.0f);
+  RA_DEVICE_CHECK(t >= 0 && t < p.T && k >= 0 && k < p.K);
   p.u_raw[(size_t)t * p.K + k] = make_float2(u0, u1);
   p.ce[(size_t)k * p.T + t] = control_effect<DYN>(p, u0, u1);
 }
@@ -75,6 +76,7 @@ __global__ void __launch_bounds__(kNominalThreads) nominal_kernel(const __grid_c
 #pragma unroll
     for (int j = 0; j < kBlock; ++j) {
       const int t = min(t0 + j, p.T - 1);
+      RA_DEVICE_CHECK(t >= 0 && t < p.T && k < p.K);
       ub[j] = p.u_raw[(size_t)t * p.K + k];
       cb[j] = ce_k[t];
     }
@@ -231,11 +233,13 @@ __device__ __forceinline__ void risk_accumulate(const Params& p, const float4* c
     lox = warp_min_f32(lox); hix = warp_max_f32(hix);
     loy = warp_min_f32(loy); hiy = warp_max_f32(hiy);
     for (int base = 0; base < n_circ_pad; base += 32) {
+      RA_DEVICE_CHECK(base + lane < n_circ_pad);
       const float4 cb = circ_s[base + lane];  // (cx - x0X, cy - x0Y, r + margin, (r + margin)^2)
       const float ddx = fmaxf(fmaxf(lox - cb.x, cb.x - hix), 0.0f);
       const float ddy = fmaxf(fmaxf(loy - cb.y, cb.y - hiy), 0.0f);
       uint32_t cand = __ballot_sync(0xFFFFFFFFu, fmaf(ddx, ddx, ddy * ddy) < cb.w);
       while (cand) {
+        RA_DEVICE_CHECK(base + __ffs(cand) - 1 < n_circ_pad);
         const float4 c = circ_s[base + __ffs(cand) - 1];  // broadcast
         cand &= cand - 1u;
         float d2[RC];
@@ -316,6 +320,9 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
   uint32_t* keys_all = reinterpret_cast<uint32_t*>(ce_all + (size_t)ce_slots * p.T);
 
   pdl_launch_dependents();   // the weights/update kernel may be scheduled behind the last wave of this grid
+  // the three regions fit the dynamic shared memory the launcher asked for
+  RA_DEVICE_CHECK((size_t)n_circ_s * sizeof(float4) + (size_t)ce_slots * p.T * sizeof(float4) +
+                  (size_t)kRolloutWarps * (HALF ? RC : p.R_total) * 32 * sizeof(uint32_t) <= dynamic_smem_bytes());
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const float x0X = x0g[0], x0Y = x0g[1];
 
@@ -336,6 +343,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
     k_of[r] = k_valid_of[r] ? k_raw : p.K - 1;
     ce_slot_of[r] = HALF ? (warp * RC + r) * 2 + (lane >> 4) : sample_in_cta;
     ce_of[r] = ce_all + (size_t)ce_slot_of[r] * p.T;
+    RA_DEVICE_CHECK(ce_slot_of[r] >= 0 && ce_slot_of[r] < ce_slots && ce_slot_of[r] < kCeSlotsMax);
     keys_of[r] = keys_all + (HALF ? (size_t)(warp * RC + r) * 32 : (size_t)sample_in_cta * p.R_total * 32);
   }
 
@@ -429,6 +437,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
           // a slot past R_total (RC does not divide the slot count) has m >= M_pad: clamp it into the row so
           // the load stays inside w_mat; the slot's results are discarded below
           const uint32_t mc = min(m[r], (uint32_t)(p.M_pad - 1));
+          RA_DEVICE_CHECK(k_of[r] < p.K && t < p.T && (int)mc < p.M_pad);
           const float* wp = p.w_mat + (((size_t)k_of[r] * p.T + t) * NX) * p.M_pad + mc;
 #pragma unroll
           for (int i = 0; i < NX; ++i) a[r][i] = __ldg(wp + (size_t)i * p.M_pad);
@@ -519,9 +528,12 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
       const bool slot_ok = HALF || (chunk + r) < p.R_total;
       const bool valid = slot_ok && (int)m[r] < p.M;
       if constexpr (RISK == RISK_CIRCLES) L[r] *= p.risk_p[0];   // risk_accumulate sums unweighted penetrations
+      RA_DEVICE_CHECK(!slot_ok || (keys_of[r] + (HALF ? 0 : (chunk + r) * 32) + lane <
+                                   keys_all + (size_t)kRolloutWarps * (HALF ? RC : p.R_total) * 32));
       if (slot_ok) keys_of[r][(HALF ? 0 : (chunk + r) * 32) + lane] = valid ? float_key(L[r]) : 0u;
       if (valid && k_valid_of[r]) {
         const int k = k_of[r];
+        RA_DEVICE_CHECK(k >= 0 && k < p.K && (int)m[r] < p.M);
         if (L_out) L_out[(size_t)k * p.M + m[r]] = L[r];
         if (xT_out) {
           float* o = xT_out + ((size_t)k * p.M + m[r]) * NX;
@@ -549,6 +561,7 @@ noisy_rollout_kernel(const __grid_constant__ Params p, const float* __restrict__
     if (p.B != 1.0f) cvar = fmaf(p.B, cvar - Lbar, Lbar);
     if (sub == 0 && k_valid_of[r]) {
       // soft filter (14)-(16) PAPER.md:120-130, strict threshold (15)
+      RA_DEVICE_CHECK(k_of[r] >= 0 && k_of[r] < p.K);
       p.cvar[k_of[r]] = cvar;
       p.pen[k_of[r]] = (cvar > p.C_u) ? (double)(p.A * cvar) : 0.0;   // J_C of (14); S~ = S + J_C is formed by its readers
     }

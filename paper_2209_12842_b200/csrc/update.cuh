@@ -185,6 +185,7 @@ weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S
     sc[j] = (ST)INFINITY;
     uc[j] = make_float2(0.0f, 0.0f);
     if (k < k_end) {
+      RA_DEVICE_CHECK(k >= 0 && k < p.K && t_first < p.T);
       sc[j] = s_tilde_at<ST>(S_tilde, pen, k);
       uc[j] = __ldg(u + (long long)k * su_k + (long long)t_first * su_t);
     }
@@ -251,6 +252,7 @@ weights_update_kernel(const __grid_constant__ Params p, const ST* __restrict__ S
   // one range, no closed-loop tail: this CTA owns its v+_t outright, no exchange needed
   if (my_partial && done && gridDim.y == 1 && !tail.x0g) my_partial = nullptr;
   if (my_partial) {   // the range's / shard's unnormalised share {beta_g, Z_g, N_g[T][2]}
+    RA_DEVICE_CHECK(my_tt >= n_t || (t_first + my_tt < p.T && n_t <= kUpdateMaxSteps));
     if (my_tt < n_t) my_partial[2 + 2 * (t_first + my_tt) + my_i] = N;
     if (threadIdx.x == 0 && blockIdx.x == 0) { my_partial[0] = (double)beta; my_partial[1] = Zt; }
     if (!done) return;
