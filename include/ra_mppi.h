@@ -143,6 +143,46 @@ ra_status ra_mppi_export_costs_f64(ra_mppi_ctx* ctx, double* d_S64, double* d_S_
 ra_status ra_mppi_weights_update(ra_mppi_ctx* ctx, const float* d_S_tilde, const float* d_u,
                                  float* d_v_plus, float* d_w, float* d_stats, void* cuda_stream);
 
+/* Weights (17) PAPER.md:134 and update (4) PAPER.md:51 for callers that must not allocate device memory.
+ *
+ * Who this is for: code that runs where cudaMalloc is off limits -- a control loop that has already handed all of
+ * its device memory to a fixed pool, a plug-in loaded into a host process whose allocator it may not touch, a
+ * real-time thread in which an allocation (an implicit device synchronisation and an unbounded driver call) would
+ * break the deadline.  Such a caller cannot use a context either, because creating one allocates.  This call needs
+ * no context and calls no cudaMalloc, cudaFree or allocating library routine: the per-range partial sums and the
+ * ticket counter that the multi-range weights/update kernel exchanges through global memory live in a fixed array
+ * of RA_STATIC_SCRATCH_BYTES bytes compiled into the library.  Every GPU that loads the library holds that array
+ * until the process exits, used or not; that is the price, and why the limits below are modest.
+ *
+ *   K in 1..RA_STATIC_MAX_K samples, T in 1..RA_MAX_T steps, lambda > 0; u_min[2], u_max[2] HOST (the clamp of v+);
+ *   d_S_tilde [K] modified costs (16), d_u [K,T,2] sampled controls, d_v_plus [T,2] output: DEVICE pointers on the
+ *   CURRENT device (there is no context to name one).  Same arithmetic as the context's weights/update kernel
+ *   (fp32 exp2, fp64 sums, fixed summation order): results are reproducible run to run, and agree with the
+ *   context-based weights/update call to rounding (the samples are summed range by range instead of in one pass).
+ *
+ * Sizes beyond the limits are refused with RA_EUNSUPPORTED before anything is enqueued; RA_EINVAL for a null pointer,
+ * K or T < 1, a non-positive or non-finite lambda, u_min > u_max; RA_ECUDA when a CUDA call fails.  The reason is kept
+ * per calling thread and read with ra_mppi_weights_update_static_error.
+ *
+ * The first call on each device looks up the device address of the array (the array's name is only a host-side
+ * handle; kernels need the address the runtime reports for the device that is current) and the SM count.  That
+ * first call may make the runtime load the library's code onto the device, so make it once at start-up, outside
+ * any stream capture.  Later calls only enqueue a 4-byte memset (the ticket counter must start at zero whatever an
+ * earlier, possibly aborted, call left behind) and one kernel on `cuda_stream`, and do not synchronise.
+ *
+ * All calls on a device share the one array.  Two calls whose kernels can overlap on the GPU (different streams
+ * without an ordering between them, or two host threads) race on it and give wrong results: order them on one
+ * stream or with events.  The array keeps the previous call's partial sums; every entry a call reads it has first
+ * written itself, so nothing but the ticket needs clearing.                                                    */
+#define RA_STATIC_MAX_K 131072      /* 64 sample ranges of 2048                                               */
+#define RA_STATIC_SCRATCH_BYTES 132352 /* 64 x (2 + 2 x RA_MAX_T) fp64 partial sums + a 256-byte ticket slot    */
+ra_status ra_mppi_weights_update_static(int32_t K, int32_t T, float lambda, const float* u_min, const float* u_max,
+                                        const float* d_S_tilde, const float* d_u, float* d_v_plus,
+                                        void* cuda_stream);
+/* Why the calling thread's most recent ra_mppi_weights_update_static call failed ("" if it did not).  The text is
+ * owned by the library and valid until this thread's next call of that function.                                */
+const char* ra_mppi_weights_update_static_error(void);
+
 /* Closed-loop glue, Alg.1 l.32-33 on a simulated plant (BASELINE config 4):
  * d_x0 <- F~(d_x0, v+_0, w_plant(iteration)); d_u_applied [2] <- v+_0 (or NULL);
  * d_v[t] <- d_v[t+1], d_v[T-1] kept (warm-start shift).                                   */

@@ -54,6 +54,7 @@ class ra_mppi_env(C.Structure):
 
 EXPORTS = (
     "ra_mppi_create", "ra_mppi_set_env", "ra_mppi_step", "ra_mppi_rollout_costs", "ra_mppi_weights_update",
+    "ra_mppi_weights_update_static", "ra_mppi_weights_update_static_error",
     "ra_mppi_step_partial", "ra_mppi_combine_partials",
     "ra_mppi_step_host", "ra_mppi_enable_kernel_timing", "ra_mppi_last_rollout_ms",
     "ra_mppi_export_costs_f64", "ra_mppi_plant_shift", "ra_mppi_closed_loop", "ra_mppi_philox", "ra_mppi_state_noise",
@@ -86,6 +87,10 @@ def open_library(path):
     L.ra_mppi_step_partial.argtypes = [vp, fp, fp, u64, vp, vp]
     L.ra_mppi_combine_partials.argtypes = [vp, vp, i32, fp, vp]
     L.ra_mppi_weights_update.argtypes = [vp, fp, fp, fp, fp, fp, vp]
+    L.ra_mppi_weights_update_static.argtypes = [i32, i32, C.c_float, C.POINTER(C.c_float), C.POINTER(C.c_float),
+                                                fp, fp, fp, vp]
+    L.ra_mppi_weights_update_static_error.argtypes = []
+    L.ra_mppi_weights_update_static_error.restype = C.c_char_p
     L.ra_mppi_export_costs_f64.argtypes = [vp, vp, vp, vp]
     L.ra_mppi_step_host.argtypes = [vp, vp, vp, u64, vp]
     L.ra_mppi_enable_kernel_timing.argtypes = [vp, i32]
@@ -103,7 +108,7 @@ def open_library(path):
     L.ra_mppi_last_error.restype = C.c_char_p
     L.ra_mppi_destroy.argtypes = [vp]
     for name in EXPORTS:
-        if name not in ("ra_mppi_launches_per_step", "ra_mppi_last_error"):
+        if name not in ("ra_mppi_launches_per_step", "ra_mppi_last_error", "ra_mppi_weights_update_static_error"):
             getattr(L, name).restype = C.c_int
     return L
 
@@ -195,6 +200,23 @@ def ra_mppi_combine_partials(ctx, d_partials, n_parts, d_v_plus, stream=0):
 def ra_mppi_weights_update(ctx, d_S_tilde, d_u, d_v_plus, d_w=None, d_stats=None, stream=0):
     _check(ctx, load().ra_mppi_weights_update(ctx, d_S_tilde, d_u, d_v_plus, d_w, d_stats, stream),
            "ra_mppi_weights_update")
+
+
+RA_STATIC_MAX_K = 131072   # include/ra_mppi.h
+
+
+def ra_mppi_weights_update_static(K, T, lam, u_min, u_max, d_S_tilde, d_u, d_v_plus, stream=0):
+    """Weights (17) and update (4) with no context and no device allocation, for callers that may not call
+    cudaMalloc (a loop that gave all its device memory to a fixed pool, a plug-in inside someone else's process,
+    a real-time thread): the kernel's scratch is an array compiled into the library.  K <= RA_STATIC_MAX_K,
+    T <= 128; the device pointers belong to the CURRENT device.  Calls share that one array, so calls that can
+    overlap on the GPU must be ordered by the caller; make the first call on a device outside stream capture."""
+    lo, hi = (C.c_float * 2)(*map(float, u_min)), (C.c_float * 2)(*map(float, u_max))
+    L = load()
+    st = L.ra_mppi_weights_update_static(int(K), int(T), float(lam), lo, hi, d_S_tilde, d_u, d_v_plus, stream)
+    if st != RA_OK:
+        msg = L.ra_mppi_weights_update_static_error()
+        raise RaMppiError(st, "ra_mppi_weights_update_static", msg.decode() if msg else "")
 
 
 def ra_mppi_step_host(ctx, h_x0, h_v, iteration, stream=0):

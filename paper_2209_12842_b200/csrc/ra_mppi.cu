@@ -833,3 +833,119 @@ ra_status ra_mppi_closed_loop(ra_mppi_ctx* c, float* d_x0, float* d_v, uint64_t 
 }
 
 }  // extern "C"
+
+// =======================================================================================
+// ra_mppi_weights_update_static: weights (17) and update (4) without a context and without any device allocation
+// (include/ra_mppi.h says who needs that).  The kernel is the library's weights_update_kernel in its multi-range form:
+// every CTA writes its range's {beta, Z, N_t} into `partial`, takes a ticket from `done`, and the last CTA combines the
+// ranges.  Elsewhere those two buffers are cudaMalloc'ed by the context; here they are the array below.
+//
+// g_static_update_scratch is a __device__ variable: in HOST code its name is a stand-in the runtime uses to find the
+// per-device instance, not a device address.  Handing `g_static_update_scratch` (or &g_static_update_scratch[0])
+// to a kernel from host code would pass a host address: the kernel faults, or on a system where the GPU can read
+// host memory quietly works on the wrong bytes.  The device address comes from cudaGetSymbolAddress, per device, with
+// that device current (static_scratch_on_current_device below).
+// =======================================================================================
+namespace {
+constexpr size_t kStaticPartialBytes = sizeof(double) * kMaxUpdateSplits * (2 + 2 * RA_MAX_T);
+constexpr size_t kStaticTicketOffset = kStaticPartialBytes;            // the ticket sits behind the partial sums
+constexpr size_t kStaticScratchBytes = kStaticPartialBytes + 256;
+static_assert(kStaticScratchBytes == RA_STATIC_SCRATCH_BYTES, "include/ra_mppi.h states the size of the static scratch");
+static_assert(kStaticTicketOffset % 256 == 0, "ticket slot keeps the array's alignment");
+static_assert(RA_STATIC_MAX_K == kMaxUpdateSplits * kUpdateThreads * kUpdateCached,
+              "the limit is what kMaxUpdateSplits register-cached ranges hold");
+}  // namespace
+
+static __device__ __align__(256) unsigned char g_static_update_scratch[kStaticScratchBytes];
+
+namespace {
+
+struct StaticScratchSlot {
+  std::atomic<unsigned char*> base{nullptr};   // device address of g_static_update_scratch on this device
+  std::atomic<int> n_sm{0};
+};
+StaticScratchSlot g_static_slot[kMaxDevices];
+
+thread_local char g_static_error[256] = "";
+
+ra_status static_fail(ra_status st, const char* what, const char* detail = "") {
+  std::snprintf(g_static_error, sizeof g_static_error, "ra_mppi_weights_update_static: %s%s%s", what,
+                detail[0] ? ": " : "", detail);
+  return st;
+}
+
+// Once per device (ordinals past the table: every call): the array's address on the CURRENT device and its SM count.
+// Neither call allocates; the first may make the runtime load this library's module onto the device.
+ra_status static_scratch_on_current_device(unsigned char** base, int* n_sm) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return static_fail(RA_ECUDA, "cudaGetDevice", cudaGetErrorString(e));
+  const bool cached = dev >= 0 && dev < kMaxDevices;
+  if (cached) {
+    unsigned char* b = g_static_slot[dev].base.load(std::memory_order_acquire);
+    if (b) { *base = b; *n_sm = g_static_slot[dev].n_sm.load(std::memory_order_relaxed); return RA_OK; }
+  }
+  void* ptr = nullptr;
+  e = cudaGetSymbolAddress(&ptr, g_static_update_scratch);
+  if (e != cudaSuccess || !ptr)
+    return static_fail(RA_ECUDA, "cudaGetSymbolAddress(g_static_update_scratch) (is the current device an sm_100 GPU?)",
+                       cudaGetErrorString(e));
+  int sms = 0;
+  e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (e != cudaSuccess || sms < 1) return static_fail(RA_ECUDA, "cudaDeviceGetAttribute", cudaGetErrorString(e));
+  if (cached) {
+    g_static_slot[dev].n_sm.store(sms, std::memory_order_relaxed);
+    g_static_slot[dev].base.store(static_cast<unsigned char*>(ptr), std::memory_order_release);
+  }
+  *base = static_cast<unsigned char*>(ptr);
+  *n_sm = sms;
+  return RA_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+ra_status ra_mppi_weights_update_static(int32_t K, int32_t T, float lambda, const float* u_min, const float* u_max,
+                                        const float* d_S_tilde, const float* d_u, float* d_v_plus, void* stream) {
+  g_static_error[0] = '\0';
+  if (!u_min || !u_max || !d_S_tilde || !d_u || !d_v_plus) return static_fail(RA_EINVAL, "null pointer");
+  if (K < 1 || T < 1) return static_fail(RA_EINVAL, "K and T must be at least 1");
+  if (!(lambda > 0.0f) || !std::isfinite(lambda)) return static_fail(RA_EINVAL, "lambda must be positive and finite");
+  for (int i = 0; i < 2; ++i)
+    if (!(u_min[i] <= u_max[i])) return static_fail(RA_EINVAL, "u_min must not exceed u_max");
+  if (K > RA_STATIC_MAX_K || T > RA_MAX_T) {
+    char msg[160];
+    std::snprintf(msg, sizeof msg, "K = %d, T = %d do not fit the %d-byte static scratch (K <= %d, T <= %d); use a context",
+                  (int)K, (int)T, (int)RA_STATIC_SCRATCH_BYTES, (int)RA_STATIC_MAX_K, (int)RA_MAX_T);
+    return static_fail(RA_EUNSUPPORTED, msg);
+  }
+  unsigned char* base = nullptr;
+  int n_sm = 0;
+  if (ra_status st = static_scratch_on_current_device(&base, &n_sm)) return st;
+  double* partial = reinterpret_cast<double*>(base);
+  unsigned int* done = reinterpret_cast<unsigned int*>(base + kStaticTicketOffset);
+
+  Params p{};   // the kernel reads the sizes, the temperature and the clamp only (no closed-loop tail here)
+  p.K = K; p.T = T;
+  p.neg_log2e_over_lambda = (float)(-1.4426950408889634 / (double)lambda);
+  for (int i = 0; i < 2; ++i) { p.u_min[i] = u_min[i]; p.u_max[i] = u_max[i]; }
+  // ranges and steps per CTA as the context's update picks them: a range is what one CTA caches in registers
+  const int per_cta = kUpdateThreads * kUpdateCached;
+  const int splits = std::max(1, std::min(kMaxUpdateSplits, (K + per_cta - 1) / per_cta));
+  const int steps = std::max(1, std::min(kUpdateMaxSteps, (T * splits) / (2 * n_sm)));
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  // the ticket must start at zero; the kernel's last CTA re-arms it, but a call that was aborted half way would not have
+  cudaError_t e = cudaMemsetAsync(done, 0, sizeof(unsigned int), s);
+  if (e != cudaSuccess) return static_fail(RA_ECUDA, "cudaMemsetAsync(ticket)", cudaGetErrorString(e));
+  weights_update_kernel<float><<<dim3((T + steps - 1) / steps, splits), kUpdateThreads, 0, s>>>(
+      p, d_S_tilde, nullptr, reinterpret_cast<const float2*>(d_u), (long long)T, 1LL, d_v_plus, nullptr, nullptr, partial,
+      done, UpdateTail{nullptr, nullptr, nullptr}, steps);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return static_fail(RA_ECUDA, "kernel launch", cudaGetErrorString(e));
+  return RA_OK;
+}
+
+const char* ra_mppi_weights_update_static_error(void) { return g_static_error; }
+
+}  // extern "C"
