@@ -494,7 +494,8 @@ ra_status enqueue_costs(ra_mppi_ctx* c, const Params& p, const float* d_x0, cons
   // A = 0 is the baseline MPPI of section II: S~ = S by (14)-(16), so unless the caller
   // asks for the risk diagnostics the M noisy rollouts are not needed at all.
   if (c->cfg.A == 0.0f && !diagnostics) {
-    // cvar / pen stay zero: written once at create and by nothing else on this path
+    // pen stays zero on this path: zeroed at create, and again after every diagnostics pass of an A = 0 context (below);
+    // the update reads S + pen only, so a stale cvar from such a pass is harmless
     RA_CUDA(c, launch_sample(c, p, d_v, s));
     RA_CUDA(c, launch_nominal(c, p, d_x0, d_v, s, c->pdl));
     return RA_OK;
@@ -519,6 +520,9 @@ ra_status enqueue_costs(ra_mppi_ctx* c, const Params& p, const float* d_x0, cons
   RA_CUDA(c, c->rollout(p, c->noise_variant, c->rc, c->half, d_x0, d_L, d_xT, s, false));
   if (time_it) { RA_CUDA(c, cudaEventRecord(c->ev_k1, s)); c->timed = true; }
   RA_CUDA(c, cudaStreamWaitEvent(s, c->ev_join, 0));   // join
+  // A = 0 with diagnostics: the kernel wrote pen = A * cvar, which is NaN for a diverged rollout (0 * inf) and would then
+  // sit in S~ of every later A = 0 step, which skips the noisy rollouts and never rewrites it.  J_C is 0 by (14) at A = 0.
+  if (c->cfg.A == 0.0f) RA_CUDA(c, cudaMemsetAsync(c->d_pen, 0, sizeof(double) * (size_t)p.K, s));
   return RA_OK;
 }
 

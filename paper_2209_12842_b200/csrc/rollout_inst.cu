@@ -1,5 +1,6 @@
 // Instantiates noisy_rollout_kernel for one (dynamics, risk) pair:
 //   nvcc -DRA_INST_DYN=<0|1> -DRA_INST_RISK=<0|1|2> -c rollout_inst.cu
+#include "../../include/ra_mppi.h"
 #include "launchers.h"
 #include "rollout.cuh"
 
@@ -22,9 +23,17 @@ cudaError_t launch(const Params& p, const float* d_x0, float* d_L, float* d_xT, 
   const size_t smem = ((RA_INST_RISK == RISK_CIRCLES || RA_INST_RISK == RISK_NOMINAL) ? (size_t)((p.n_circles + 31) & ~31) * sizeof(float4) : 0) +
                       (size_t)ce_slots * p.T * sizeof(float4) + (size_t)key_rows * 32 * sizeof(uint32_t);
   auto kernel = noisy_rollout_kernel<RA_INST_DYN, RA_INST_RISK, NOISE, RC, HALF>;
-  if (smem > 48 * 1024) {   // worst case (1024 circles, T = 128, M = 512) is 65 KB
+  // Worst case over everything ra_mppi_create / ra_mppi_set_env accept: M <= 16 with two slots per lane (K >= 32768) stages
+  // 32 control-effect rows, at T = 128 that is 64 KB, plus 2 KB of keys and 16 KB for 1024 circles = 82 KB; the other
+  // layouts stay below 49 KB.  kRolloutSmemLimit covers that with room to spare (an SM holds 227 KB: two such CTAs fit).
+  constexpr int kRolloutSmemLimit = 96 * 1024;
+  static_assert((size_t)kMaxCirclesSmem * sizeof(float4) + (size_t)4 * kRolloutWarps * RA_MAX_T * sizeof(float4) +
+                    (size_t)kRolloutWarps * (RA_MAX_M / 32) * 32 * sizeof(uint32_t) <= (size_t)kRolloutSmemLimit,
+                "the largest accepted configuration must fit the dynamic shared-memory limit");
+  if (smem > (size_t)kRolloutSmemLimit) return cudaErrorInvalidConfiguration;
+  if (smem > 48 * 1024) {
     static std::atomic<int> smem_set[kMaxDevices];
-    const cudaError_t e = set_func_attr_once(smem_set, p.device, kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 80 * 1024);
+    const cudaError_t e = set_func_attr_once(smem_set, p.device, kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kRolloutSmemLimit);
     if (e != cudaSuccess) return e;
   }
   // the same L1 / shared-memory split as the nominal-rollout kernel that runs beside this one: CTAs of kernels

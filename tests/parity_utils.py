@@ -5,6 +5,8 @@ TOL_STATE_ABS = 1e-3     # rollout states at t = T: m, rad, m/s
 TOL_COST_REL = 1e-4      # CVaR and total costs
 TOL_V_ABS = 1e-4         # updated mean control
 ZERO_MARGIN_M = 1e-5     # "exact zeros must match" (G28) away from an obstacle rim by more than this
+ZERO_LEAK_REL = 1e-4     # risk kinds without a rim: GPU L where the oracle's is exactly 0, relative to the typical cost
+BOUND_MAX = 10 * 1e-4    # a v+ fallback verdict whose weight-sensitivity bound exceeds 10 TOL_V_ABS proves too little: fail
 
 # every end-to-end v+ comparison of the session: (case, verdict, err, max|dS~|, gap of the two smallest S~, bound);
 # tests/conftest.py prints the tally and writes gpurun_out/parity_verdicts.md at session end
@@ -33,8 +35,9 @@ def gpu_outputs(ctl, p, iteration=0, x0=None, v=None, **kw):
     return {k: (t.cpu().numpy() if t is not None else None) for k, t in g.items()}
 
 
-def check_rollout_parity(p, ctl, orc, iteration=0, x0=None, v=None, k_begin=0, k_end=None):
-    """Stage-wise parity of A1-A7 (SURVEY.md section 8(c) 'How parity is checked')."""
+def check_rollout_parity(p, ctl, orc, iteration=0, x0=None, v=None, k_begin=0, k_end=None, tol_cost=TOL_COST_REL):
+    """Stage-wise parity of A1-A7 (SURVEY.md section 8(c) 'How parity is checked').  tol_cost is north_star's 1e-4
+    everywhere except the one stress case that documents where it stops holding (yaw winding, test_gpu_parity.py)."""
     from oracle import oracle as O
     g = gpu_outputs(ctl, p, iteration, x0, v)
     hinge = p.risk == 0          # circle risk: the oracle also reports each rollout's closest approach to a rim
@@ -48,8 +51,8 @@ def check_rollout_parity(p, ctl, orc, iteration=0, x0=None, v=None, k_begin=0, k
     ex = np.abs(gs["xT"] - r["xT"]).max()
     assert ex < TOL_STATE_ABS, f"xT abs err {ex:.3e}"
     # A2/A4: costs
-    assert_costs_close(gs["S"], r["S"], "S")
-    assert_costs_close(gs["L"], r["L"], "L")
+    assert_costs_close(gs["S"], r["S"], "S", tol=tol_cost)
+    assert_costs_close(gs["L"], r["L"], "L", tol=tol_cost)
     if hinge:
         # exact zeros must match (G28): a rollout the oracle scores exactly 0 and whose closest approach to
         # any rim r + margin exceeds ZERO_MARGIN_M must be exactly 0 on the GPU too (exact culling, no leakage); within
@@ -59,14 +62,26 @@ def check_rollout_parity(p, ctl, orc, iteration=0, x0=None, v=None, k_begin=0, k
         # and the other way round: nothing the oracle scores > 0 clear of a rim may vanish on the GPU
         inside = (r["L"] > 0) & (r["margin"][:, 1:] > ZERO_MARGIN_M)
         assert (gs["L"][inside] > 0).all()
+    else:
+        # the other risk kinds (costmap, linear, l = q) have no rim diagnostic, but a rollout the oracle scores exactly 0
+        # may still not pick up more than rounding on the GPU: a bilinear lookup one texel off, or a leaked term, is far
+        # above ZERO_LEAK_REL of the typical cost (a position error of 1e-6 m across a cell edge of the BASELINE costmap
+        # is worth about 1e-6 / res * weight = 0.02 against typical costs of 1e3 and more)
+        zero = r["L"] == 0
+        if zero.any():
+            nz = np.abs(r["L"][r["L"] != 0])
+            scale = float(np.median(nz)) if nz.size else 1.0
+            leak = float(np.abs(gs["L"][zero]).max())
+            assert leak <= ZERO_LEAK_REL * scale, (f"{int((gs['L'][zero] != 0).sum())} of {int(zero.sum())} rollouts the oracle "
+                                                   f"scores 0 have L up to {leak:.3e} on the GPU (typical cost {scale:.3e})")
     # A5/A6 isolated: the oracle's sort-based CVaR of the GPU's own L must equal the GPU's CVaR
     k_tail = O.tail_count(p.alpha, p.M)
     iso = np.array([O.cvar_topk(O.sensitivity_scale(gs["L"][i].astype(np.float64), p.B), k_tail)
                     for i in range(gs["L"].shape[0])])
     assert_costs_close(gs["cvar"], iso, "CVaR(select kernel) vs sort of GPU L", tol=2e-6)
     # end to end
-    assert_costs_close(gs["cvar"], r["cvar"], "CVaR")
-    assert_costs_close(gs["S_tilde"], r["S_tilde"], "S_tilde")
+    assert_costs_close(gs["cvar"], r["cvar"], "CVaR", tol=tol_cost)
+    assert_costs_close(gs["S_tilde"], r["S_tilde"], "S_tilde", tol=tol_cost)
     return g, r
 
 
@@ -128,6 +143,10 @@ def check_step_parity(p, ctl, orc, r, iteration=0, x0=None, v=None, case=None):
     span = np.abs(r["u"] - ref["v_plus"][None]).max()
     bound = TOL_V_ABS + float(np.expm1(2 * D / p.lam)) * mad + p.K * np.exp(-30.0) * span
     assert err <= bound, f"v+ err {err:.3e} exceeds the weight-sensitivity bound {bound:.3e} (max|dS~| {D:.3e}, lambda {p.lam})"   # (b)
+    # the bound is rigorous but loose at small lambda (D = 1e-2 at lambda = 0.5 admits 4 % of the spread): a verdict that
+    # rests on a bound this wide could hide an update bug, so such a case must be re-posed (larger lambda, other seed)
+    assert bound <= BOUND_MAX, (f"v+ err {err:.3e} is within its weight-sensitivity bound {bound:.3e}, but a bound above "
+                                f"{BOUND_MAX:.0e} is too loose to count as parity (max|dS~| {D:.3e}, lambda {p.lam})")
     kind = "near-tie" if gap < 2 * D else "weight-sensitive"
     VERDICTS.append((name, kind, err, D, gap, bound))
     return f"{kind} (end-to-end err {err:.2e} <= bound {bound:.2e}; max|dS~| {D:.2e}, gap {gap:.2e}, lambda {p.lam})", err

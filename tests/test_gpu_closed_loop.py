@@ -87,6 +87,49 @@ def test_closed_loop_graph_teacher_forced(torch_cuda):
     assert np.array_equal(log2.cpu().numpy(), log)
 
 
+def test_closed_loop_config4_at_its_stated_size(torch_cuda):
+    """BASELINE config 4 as stated and as bench.py times it: K = 8192, M = 64, T = 50, 500 receding-horizon iterations
+    replayed from one CUDA graph (Alg.1 l.1-2, 31-33).  At this K the update kernel takes four
+    sample ranges and its last CTA combines them and applies the plant and the shift, which the K = 512 case above does
+    not reach.  The whole replay must equal the same 500 iterations issued call by call, bit for bit; and at iterations
+    {0, 1, 2, 10, 100, 499} the loop's own (x0, v, iteration) is handed to the oracle and that single step compared
+    (SURVEY.md section 8(c) item 6): stage-wise on a 96-sample slice, S~ and v+ on all K samples."""
+    torch = torch_cuda
+    import bench
+    p = bench.make_problem("C4-K8192-M64")
+    assert (p.K, p.M, p.T) == (8192, 64, 50)
+    ctl, orc = _ctl(p), O.Oracle(p)
+    n_iter, marks = 500, (0, 1, 2, 10, 100, 499)
+    d_x0, d_v = ctl.tensor(p.x0), ctl.tensor(np.zeros((p.T, 2)))
+    log, _ = ctl.closed_loop(d_x0, d_v, 0, n_iter, timing=False)
+    # call by call, keeping the trajectory on the device; the host looks only at the marked iterations
+    e_x0, e_v = ctl.tensor(p.x0), ctl.tensor(np.zeros((p.T, 2)))
+    xs = torch.empty(n_iter, p.nx + 2, device=e_x0.device)
+    checkpoints = {}
+    for i in range(n_iter):
+        if i in marks:
+            checkpoints[i] = (e_x0.cpu().numpy().astype(np.float64), e_v.cpu().numpy().astype(np.float64))
+        ctl.step(e_x0, e_v, i)
+        u = ctl.plant_shift(e_x0, e_v, i)
+        xs[i, :p.nx].copy_(e_x0)
+        xs[i, p.nx:].copy_(u)
+    torch.cuda.synchronize()
+    assert torch.isfinite(log).all()
+    diff = (log != xs).any(dim=1).nonzero()
+    assert diff.numel() == 0, f"graph replay and call-by-call differ first at iteration {int(diff[0])}"
+    assert torch.equal(e_v, d_v) and torch.equal(e_x0, d_x0)
+    for i, (x0, v) in checkpoints.items():
+        g, r = check_rollout_parity(p, ctl, orc, iteration=i, x0=x0, v=v, k_begin=4090, k_end=4186)   # across two ranges
+        rf = orc.rollout_costs(x0=x0, v=v, iteration=i, n_threads=O.host_cores(), want_L=False, want_xT=False)
+        gs = g["S_tilde"]
+        from parity_utils import assert_costs_close
+        assert_costs_close(gs, rf["S_tilde"], f"S_tilde over all K at iteration {i}")
+        verdict, err = check_step_parity(p, ctl, orc, rf, iteration=i, x0=x0, v=v,
+                                         case=f"config-4 closed loop K=8192 M=64 T=50, iteration {i} of 500 (teacher-forced)")
+        print(f"iteration {i}: x0 = {np.round(x0, 3)}, risk active on {(rf['cvar'] > 0).mean():.2f} of samples, v+ {verdict}, err {err:.2e}")
+    ctl.close()
+
+
 def test_step_host_equals_step(torch_cuda):
     torch = torch_cuda
     p = W.small(W.config3(), K=256, M=128, T=50)

@@ -218,6 +218,42 @@ def test_single_track_floor_and_x0_floor(torch_cuda):
     assert (g["xT"][..., 3] >= 0.5).all() and (g["xT"][..., 3] == 0.5).any()
 
 
+@pytest.mark.parametrize("case", ["bicycle-3-turns", "single-track-2-turns", "bicycle-15-turns"])
+def test_yaw_winding_at_T128(torch_cuda, case):
+    """The noisy rollouts take sin/cos of the yaw with MUFU.SIN/COS on the unreduced angle (the yaw is reduced to
+    [-pi, pi) once, at rollout start), so that error grows like 2^-23 |psi| with the winding inside the horizon.  Full
+    steering lock held over the longest horizon, T = 128, winds the yaw by 3 turns at config speed, by 15 turns at up to
+    25 m/s (far outside any workload), and spins a single-track car: the states at t = T must stay within north_star's
+    1e-3 of the oracle's libm sin/cos.  They do with a factor 3 to spare even at 15 turns, and the same library with an
+    exactly reduced sin/cos in its place gives the same errors to 10 % (profiles/r3_yaw_winding.md): what limits these
+    cases is the fp32 Euler sum of yaw and speed over 128 steps, not the unreduced angle.
+    Costs: these scenes score only rim-grazing rollouts (under 1 % of them, L of order 1), where a hinge of 1000 per
+    metre squared turns an in-tolerance position error into a relative cost error above 1e-4 whatever sin/cos is used, so
+    the cost checks run at 3e-3 here; the 1e-4 cost tolerance is pinned by every other case of this file."""
+    from parity_utils import rel_err
+    T = 128
+    if case.startswith("bicycle"):
+        v0, accel, min_turns = (3.0, 0.0, 2.9) if case == "bicycle-3-turns" else (6.0, 3.0, 10.0)
+        p = W.small(W.config0(near_obstacle=True), K=40, M=64, T=T)
+        p = p.replace(x0=np.array([1.0, 1.0, 3.0, v0]), v=np.tile(np.array([[0.35, accel]]), (T, 1)))
+    else:                      # initial yaw rate 12 rad/s, steering at the clamp, noisy yaw rate
+        p = W.small(W.config2(), K=40, M=64, T=T)
+        p = p.replace(dt=0.05, x0=np.array([10.0, 0.0, np.pi / 2, 4.0, 0.0, 12.0]),
+                      v=np.tile(np.array([[0.35, 4.0]]), (T, 1)),
+                      sigma_w=[0.01, 0.01, 0.005, 0.05, 0.05, 0.3])
+        min_turns = 1.5
+    ctl, orc = _ctl(p), O.Oracle(p)
+    g, r = check_rollout_parity(p, ctl, orc, tol_cost=3e-3)
+    turns = np.abs(r["xT"][..., 2] - p.x0[2]) / (2 * np.pi)
+    err = np.abs(g["xT"] - r["xT"]).max(axis=(0, 1))
+    print(f"{case}: yaw winding median {np.median(turns):.1f} turns, max {turns.max():.1f}; max |x_T err| per component "
+          f"{err}; max rel err of L {rel_err(g['L'], r['L']).max():.2e}, of S {rel_err(g['S'], r['S']).max():.2e}; "
+          f"fraction of rollouts with L > 0: {(r['L'] > 0).mean():.3f}")
+    assert np.median(turns) > min_turns, "the case does not wind the yaw"
+    assert err.max() < TOL_STATE_ABS / 2
+    ctl.close()
+
+
 # ------------------------------------------------------------------ the paper's own racing costs (NEXT row 2)
 def _racing_compare(p, g, r, sl):
     """Indicator obstacle cost (22) is a float decision: exclude rollouts whose distance to some
@@ -314,6 +350,44 @@ def test_baseline_mppi_mode_skips_the_noisy_rollouts(torch_cuda):
     with pytest.raises(B.RaMppiError) as e:
         ctl.last_rollout_ms()
     assert e.value.status == B.RA_EINVAL and "timed" in str(e.value)
+    # a diagnostics pass whose risk costs overflow (CVaR = inf) must not leave J_C = 0 * inf = NaN behind in the S~ of the
+    # A = 0 steps that follow it (they skip the noisy rollouts and so never rewrite J_C)
+    q = p.replace(risk=W.RISK_LINEAR_STATE, risk_p=[3e38, 3.0, 0.0, 0.0])   # weight * speed overflows fp32
+    c2 = _ctl(q)
+    x, v1, v2 = c2.tensor(q.x0), c2.tensor(q.v), c2.tensor(q.v)
+    c2.step(x, v1, 5)
+    out = c2.rollout_costs(x, c2.tensor(q.v), 5)
+    assert not torch.isfinite(out["cvar"]).all(), "the case does not overflow"
+    assert torch.equal(out["S"], out["S_tilde"])
+    c2.step(x, v2, 5)
+    torch.cuda.synchronize()
+    assert torch.isfinite(v2).all() and torch.equal(v1, v2)
+    c2.close()
+
+
+def test_largest_shared_memory_footprint(torch_cuda):
+    """M <= 16 with two slots per lane (K >= 32768) at T = 128 and 1024 circles is the rollout kernel's largest CTA
+    (32 control-effect rows + keys + circles = 82 KB of shared memory); also reached by set_env on a context created with
+    few circles.  Slices of samples against the oracle (first CTA, a middle one, the ragged last one); the step runs."""
+    torch = torch_cuda
+    p = _with_v(W.small(W.config1(n_obs=1024), K=32768 + 5, M=16, T=128))
+    assert p.circles.shape[0] == 1024
+    ctl, orc = _ctl(p), O.Oracle(p)
+    for k0, k1 in ((0, 24), (20000, 20016), (p.K - 9, p.K)):
+        g, r = check_rollout_parity(p, ctl, orc, k_begin=k0, k_end=k1)
+    assert (r["cvar"] > 0).mean() > 0.05, "risk path not exercised"
+    d_x0, d_v = ctl.tensor(p.x0), ctl.tensor(p.v)
+    ctl.step(d_x0, d_v, 0)
+    torch.cuda.synchronize()
+    assert torch.isfinite(d_v).all()
+    ctl.close()
+    few = p.replace(circles=p.circles[:8])
+    a = _ctl(few)
+    a.set_env(circles=p.circles)
+    ga = a.rollout_costs(a.tensor(p.x0), a.tensor(p.v), 0, want_xT=False, want_u=False)
+    torch.cuda.synchronize()
+    assert np.array_equal(ga["L"].cpu().numpy(), g["L"])
+    a.close()
 
 
 def test_set_env_replaces_obstacles_and_costmap(torch_cuda):
