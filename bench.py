@@ -42,11 +42,51 @@ ALGO_OPS = {"PAPER": _BICYCLE + 30, "PAPER-ST": _SINGLE_TRACK + 30, "C0": _BICYC
             "C3": _BICYCLE + 18, "C4": _BICYCLE}
 ALU_PEAK_LANE_OPS = 148 * 128 * 1.965e9  # 148 SMs x 128 FP32 lanes x 1.965 GHz (B200_PROFILING.md nominal)
 ISSUE_PEAK_WARP_INST = 148 * 4 * 1.965e9  # one warp instruction per cycle per SM sub-partition
-COUNTERS_CSV = os.path.join(ROOT, "profiles", "r2_rollout_counters.csv")
+COUNTERS_CSV = os.path.join(ROOT, "profiles", "r3_rollout_counters.csv")
+# the sources that decide what noisy_rollout_kernel compiles to; their hash is stored with every capture
+ROLLOUT_SOURCES = ("rollout.cuh", "models.cuh", "rng.cuh", "ra_params.cuh", "launchers.h", "rollout_inst.cu")
+
+
+def rollout_source_sha() -> str:
+    """sha256 over the rollout kernel's sources as they are in the tree now (tests/helpers/ncu_counters.py stores the same
+    hash in every row it writes, so a capture of an older kernel is recognised and not reported as current)."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in ROLLOUT_SOURCES:
+        with open(os.path.join(ROOT, "paper_2209_12842_b200", "csrc", f), "rb") as fh:
+            h.update(f.encode() + b"\0" + fh.read() + b"\0")
+    return h.hexdigest()
+
+
+def kernel_template_args(kernel_name: str):
+    """'void noisy_rollout_kernel<0, 1, 0, 2, 0>(...)' -> (0, 1, 0, 2, 0): dynamics, risk, noise variant, slots per lane, half."""
+    import re
+    m = re.search(r"noisy_rollout_kernel<([^>]*)>", kernel_name or "")
+    if not m:
+        return None
+    conv = lambda t: {"true": 1, "false": 0}.get(t.strip(), None) if t.strip() in ("true", "false") else int(t.strip().split(")")[-1])
+    try:
+        return tuple(conv(t) for t in m.group(1).split(","))
+    except ValueError:
+        return None
+
+
+def capture_status(row, variant=None, scaled=False):
+    """Is the committed capture `row` a description of the kernel that is running?  None when there is no row; otherwise
+    {"stale": bool, "why": [...], "extrapolated": bool}: stale when the rollout sources have changed since the capture, or
+    when the captured instantiation is not the one the live context launches (`variant` = ra_mppi_rollout_variant)."""
+    if not row:
+        return None
+    why = []
+    if row.get("source_sha") != rollout_source_sha():
+        why.append("rollout kernel sources changed since the capture (source_sha)")
+    if variant is not None and kernel_template_args(row.get("kernel", "")) != tuple(variant):
+        why.append(f"captured {row.get('kernel', '?')} but the context launches noisy_rollout_kernel<{', '.join(map(str, variant))}>")
+    return {"stale": bool(why), "why": why, "extrapolated": bool(scaled)}
 
 
 def load_counters():
-    """Per-launch counters of noisy_rollout_kernel from the committed `ncu --set full` captures (profiles/r2_rollout_counters.md
+    """Per-launch counters of noisy_rollout_kernel from the committed `ncu --set full` captures (profiles/r3_rollout_counters.md
     names the commands): {workload: {metric: value}}.  Absent file => {} and the derived fractions are null."""
     import csv
     out = {}
@@ -60,6 +100,9 @@ def load_counters():
             continue
         d = {}
         for k, v in zip(hdr[1:], r[1:]):
+            if k in ("kernel", "source_sha"):
+                d[k] = v
+                continue
             try:
                 d[k] = float(v.replace(",", ""))
             except ValueError:
@@ -80,7 +123,7 @@ def counter_key(name: str) -> str:
     return name
 
 
-def derived_fractions(name, state_steps, kernel_ms, ffma_peak_tlaneops, counters):
+def derived_fractions(name, state_steps, kernel_ms, ffma_peak_tlaneops, counters, variant=None):
     """Roofline fractions of one rollout-kernel launch lasting kernel_ms (measured live):
     frac = algorithmic lane-ops / measured FFMA issue rate (the contract's figure);
     frac_fp32_flop = FP32 flop/s (2 FFMA + FADD + FMUL thread instructions of the ncu capture) / measured FFMA flop/s;
@@ -89,7 +132,9 @@ def derived_fractions(name, state_steps, kernel_ms, ffma_peak_tlaneops, counters
     peak = ffma_peak_tlaneops * 1e12 if ffma_peak_tlaneops and ffma_peak_tlaneops > 0 else ALU_PEAK_LANE_OPS
     out = {"frac": ops / (kernel_ms * 1e-3) / peak, "frac_fp32_flop": None, "frac_issue": None}
     c = counters.get(counter_key(name))
-    if c:
+    st = capture_status(c, variant, scaled=bool(c) and c.get("state_steps") != state_steps)
+    out["capture"] = st
+    if c and not st["stale"]:
         scale = state_steps / c["state_steps"] if c.get("state_steps") else 1.0   # same kernel, different K
         flop = 2.0 * c["smsp__sass_thread_inst_executed_op_ffma_pred_on.sum"] + \
             c["smsp__sass_thread_inst_executed_op_fadd_pred_on.sum"] + c["smsp__sass_thread_inst_executed_op_fmul_pred_on.sum"]
@@ -316,8 +361,9 @@ def run_cuda(args):
         ops = ALGO_OPS[key] * units_step
         achieved = ops / (kernel_ms * 1e-3)
         peak = pipe_peaks["ffma"] * 1e12 if pipe_peaks.get("ffma", 0) > 0 else ALU_PEAK_LANE_OPS
-        fr = derived_fractions(args.workload, units_step, kernel_ms, pipe_peaks.get("ffma"), counters)
-        c = counters.get(counter_key(args.workload), {})
+        fr = derived_fractions(args.workload, units_step, kernel_ms, pipe_peaks.get("ffma"), counters, ctl.rollout_variant)
+        stale = bool(fr["capture"] and fr["capture"]["stale"])
+        c = {} if stale else counters.get(counter_key(args.workload), {})   # a stale capture describes another kernel: report nothing from it
         pct = lambda k: (c[k] / 100.0 if k in c else None)
         traffic = (c["dram__bytes_read.sum"] + c["dram__bytes_write.sum"]) if "dram__bytes_read.sum" in c else None
         line = {
@@ -335,11 +381,15 @@ def run_cuda(args):
                     "api": "ra_mppi_step_host (pinned host x0, v -> v+)"},
             "gpu_launches": int(ctl.launches_per_step * args.steps),
             "roofline": {
-                "bound": "alu", "kernel": "noisy_rollout_kernel",
+                "bound": "issue+xu", "kernel": "noisy_rollout_kernel",
+                "bound_note": "plain SM pipes, no tensor or HBM bound: instruction issue slots and the XU (MUFU) pipe co-limit (the contract's 'alu' class)",
                 "binding_resource": "issue slots and the XU (MUFU) pipe, co-limiting; fmaheavy behind them (pipe_busy)",
                 "achieved": achieved / 1e12, "peak": peak / 1e12,
                 "unit": "Tlane-op/s (algorithmic instructions per FP32-lane issue slot; FFMA = 1)",
                 "frac": achieved / peak,
+                "frac_definition": "useful-instruction issue slots: the method's algorithmic instructions (Philox integer work, MUFU and FP32 "
+                                   "each counted as one FP32-lane slot) per second / measured FFMA issue rate.  NOT the literal FP32 figure: "
+                                   "that is frac_fp32_flop (FP32 flop/s / FP32 peak); frac_issue counts every executed instruction",
                 # the same launch on the stricter readings: FP32 flop only, and all executed instructions
                 "frac_fp32_flop": fr["frac_fp32_flop"],
                 "fp32_flop_note": "(2 FFMA + FADD + FMUL thread instructions per launch, ncu SASS counters of the committed capture) / "
@@ -350,8 +400,11 @@ def run_cuda(args):
                               "fma": pct("sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active"),
                               "alu": pct("sm__pipe_alu_cycles_active.avg.pct_of_peak_sustained_active"),
                               "xu": pct("sm__inst_executed_pipe_xu.avg.pct_of_peak_sustained_active"),
-                              "source": "ncu --set full capture, profiles/r2_rollout_counters.csv" if c else None},
+                              "source": "ncu --set full capture, profiles/r3_rollout_counters.csv" if c else None},
                 "traffic": traffic,
+                # frac_fp32_flop, frac_issue, pipe_busy and traffic come from a committed ncu capture scaled by the live kernel time;
+                # they are null, and this is true, when the rollout sources or the launched instantiation differ from the captured ones
+                "stale_capture": stale, "capture": fr["capture"],
                 "nominal_peak": ALU_PEAK_LANE_OPS / 1e12, "frac_of_nominal": achieved / ALU_PEAK_LANE_OPS,
                 "measured_pipe_peaks_Tlaneops": pipe_peaks,
                 "algorithmic_ops_per_state_step": ALGO_OPS[key], "kernel_ms": kernel_ms,
@@ -475,10 +528,12 @@ def quick_time(p, steps=50, warmup=5, flush=None):
             b.synchronize()
             if i >= warmup:
                 (kms if timed else ms).append(ctl.last_rollout_ms() if timed else a.elapsed_time(b))
+    variant = list(ctl.rollout_variant)
     ctl.close()
     step_ms = float(np.mean(ms))
     return {"workload": f"{p.name} K={p.K} M={p.M} T={p.T}", "ms_per_step": step_ms, "iterations_per_s": 1e3 / step_ms,
-            "state_steps_per_s": p.state_steps / (step_ms * 1e-3), "rollout_kernel_ms": float(np.mean(kms))}
+            "state_steps_per_s": p.state_steps / (step_ms * 1e-3), "rollout_kernel_ms": float(np.mean(kms)),
+            "rollout_variant": variant}
 
 
 def run_workloads(ffma_peak, counters, flush=None, with_cpu=False):
@@ -501,8 +556,8 @@ def run_workloads(ffma_peak, counters, flush=None, with_cpu=False):
         p = make_problem(name) if p is None else p
         r = quick_time(p, steps=steps, flush=flush)
         r.update({"kind": tag, "name": name})
-        r.update(derived_fractions(name, p.state_steps, r["rollout_kernel_ms"], ffma_peak, counters))
-        r["roofline_bound"] = "alu"
+        r.update(derived_fractions(name, p.state_steps, r["rollout_kernel_ms"], ffma_peak, counters, r["rollout_variant"]))
+        r["roofline_bound"] = "issue+xu"
         out.append(r)
         return r, p
 
@@ -524,6 +579,13 @@ def run_workloads(ffma_peak, counters, flush=None, with_cpu=False):
               "noise_tensor_GB": noise_bytes / 1e9, "rollout_read_GBps": gbs, "hbm_peak_GBps": hbm_peak,
               "peak_source": "measured (MEASURED_PEAKS.json)" if peaks else "fallback", "frac": gbs / hbm_peak,
               "frac_note": "rollout kernel streaming the noise tensor: algorithmic bytes 4 n_x K M T / kernel time / HBM copy peak"})
+    # the write side: the generator fills the same tensor once per step.  Its time is the step minus the rollout kernel, which
+    # also contains the sampling, nominal-rollout and update kernels (about 0.03 ms here), so the rate is a lower bound
+    gen_ms = r["ms_per_step"] - r["rollout_kernel_ms"]
+    r.update({"generator_ms_upper_bound": gen_ms, "generator_write_GBps": noise_bytes / (gen_ms * 1e-3) / 1e9,
+              "generator_frac": noise_bytes / (gen_ms * 1e-3) / 1e9 / hbm_peak,
+              "generator_note": "materialise_noise_kernel writes the tensor once per step: bytes / (step - rollout kernel) / HBM copy peak; "
+                                "a lower bound (the difference also holds the three small kernels)"})
     out.append(r)
     # closed loop: config 4, K=8192, M=64, 500 receding-horizon iterations replayed from one CUDA graph
     name = "C4-K8192-M64"
@@ -547,9 +609,9 @@ def run_workloads(ffma_peak, counters, flush=None, with_cpu=False):
           "latency_ms_p50": p50, "latency_ms_p99": float(np.percentile(ms, 99)), "latency_ms_max": float(ms.max()),
           "ms_per_step": total / 500.0, "state_steps_per_s": p.state_steps * 500.0 / (total * 1e-3),
           "final_state": [float(x) for x in log[-1, :p.nx]],
-          "distance_travelled_m": float(np.hypot(np.diff(log[:, 0]), np.diff(log[:, 1])).sum()), "roofline_bound": "alu"}
+          "distance_travelled_m": float(np.hypot(np.diff(log[:, 0]), np.diff(log[:, 1])).sum()), "roofline_bound": "issue+xu"}
     # whole-iteration fractions (the graph has no event pair around the rollout kernel): iteration time as the denominator
-    cl.update(derived_fractions(name, p.state_steps, total / 500.0, ffma_peak, counters))
+    cl.update(derived_fractions(name, p.state_steps, total / 500.0, ffma_peak, counters, ctl.rollout_variant))
     cl["frac_note"] = "whole iteration (sampling + rollouts + update + plant) as the time base"
     out.append(cl)
     ctl.close()
@@ -574,17 +636,11 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-workloads", action="store_true", help="leave the per-workload array out of the line (short profiling runs)")
-    ap.add_argument("--pipe-model", action="store_true",
-                    help="print the measured issue-cost model of the SM pipes (one JSON line) and exit")
     ap.add_argument("--sharded", action="store_true",
                     help="one controller, K split over the ranks (strong scaling) instead of N independent replicas")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
-    if args.pipe_model:
-        from paper_2209_12842_b200 import binding as B
-        print(json.dumps({"report": "pipe model, cycles per warp-instruction group per SMSP at max SM clock",
-                          **B.ra_mppi_measure_pipe_model(0), "peaks_Tlaneops": B.ra_mppi_measure_pipe_peaks(0)}))
-    elif args.report:
+    if args.report:
         run_report(args)
     elif args.impl == "reference":
         run_reference(args)

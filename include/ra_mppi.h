@@ -225,13 +225,6 @@ ra_status ra_mppi_state_noise(ra_mppi_ctx* ctx, const int32_t* d_kmt, int32_t n,
  * microbenchmark kernels on the NULL stream and synchronises.  Roofline denominators only.   */
 ra_status ra_mppi_measure_pipe_peaks(int32_t device, float* h_tera_lane_ops);
 
-/* The issue-cost model behind the roofline discussion: h_cycles[8] (HOST) = cycles per
- * warp-instruction (group) per SM sub-partition at the device's maximum SM clock, 24 warps/SM, for
- * {FFMA r,c,c; FFMA r,r,r; FMUL r,r; IMAD 32-bit; SHF; IMAD.WIDE.U32 + LOP3 (one Philox half-round);
- *  the same + 2 FFMA; the same + 4 FFMA}.  The last three show that FFMAs do not overlap the wide multiply.
- * Runs eight short microbenchmark kernels on the NULL stream and synchronises.                           */
-ra_status ra_mppi_measure_pipe_model(int32_t device, float* h_cycles);
-
 /* The two integer decisions ra_mppi_create derives from fp32 parameters, without touching a device (host only):
  * *h_k_tail = ceil((1-alpha) M) clamped to [1, M], the CVaR tail size of Alg.1 l.25-26 ((12) :107);
  * *h_K0 = ceil((1-eta) K_total), the number of samples that carry the mean control (Alg.1 l.7-10).
@@ -239,6 +232,12 @@ ra_status ra_mppi_measure_pipe_model(int32_t device, float* h_cycles);
  * error (alpha = 0.7f with M = 10 counts 3, eta = 0.7f with K = 1000 counts 300).  Either pointer may be NULL.
  * RA_EINVAL: null cfg, struct_size mismatch, M or K <= 0, alpha outside (0,1), eta outside [0,1).            */
 ra_status ra_mppi_query_counts(const ra_mppi_config* cfg, int32_t* h_k_tail, int32_t* h_K0);
+
+/* Which instantiation of the rollout kernel this context launches (host only): h_variant[5] (HOST) =
+ * {dynamics, risk, noise variant (ra_noise_kind, or 3 = materialised), realisation slots per lane, 1 if half a warp
+ * carries a sample (M <= 16) else 0} -- the template arguments noisy_rollout_kernel<...> shows in a profiler, so that a
+ * stored profiler capture can be matched against the kernel that is actually running.                              */
+ra_status ra_mppi_rollout_variant(const ra_mppi_ctx* ctx, int32_t* h_variant);
 
 /* Number of kernels one ra_mppi_step launches (for launch accounting).                   */
 int32_t ra_mppi_launches_per_step(const ra_mppi_ctx* ctx);

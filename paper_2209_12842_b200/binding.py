@@ -58,7 +58,7 @@ EXPORTS = (
     "ra_mppi_step_partial", "ra_mppi_combine_partials",
     "ra_mppi_step_host", "ra_mppi_enable_kernel_timing", "ra_mppi_last_rollout_ms",
     "ra_mppi_export_costs_f64", "ra_mppi_plant_shift", "ra_mppi_closed_loop", "ra_mppi_philox", "ra_mppi_state_noise",
-    "ra_mppi_measure_pipe_peaks", "ra_mppi_measure_pipe_model", "ra_mppi_query_counts", "ra_mppi_launches_per_step", "ra_mppi_last_error", "ra_mppi_destroy",
+    "ra_mppi_measure_pipe_peaks", "ra_mppi_query_counts", "ra_mppi_rollout_variant", "ra_mppi_launches_per_step", "ra_mppi_last_error", "ra_mppi_destroy",
 )
 
 _lib = None
@@ -100,8 +100,8 @@ def open_library(path):
     L.ra_mppi_philox.argtypes = [vp, vp, i32, vp, vp]
     L.ra_mppi_state_noise.argtypes = [vp, vp, i32, u64, fp, vp]
     L.ra_mppi_measure_pipe_peaks.argtypes = [i32, C.POINTER(C.c_float)]
-    L.ra_mppi_measure_pipe_model.argtypes = [i32, C.POINTER(C.c_float)]
     L.ra_mppi_query_counts.argtypes = [C.POINTER(ra_mppi_config), C.POINTER(i32), C.POINTER(i32)]
+    L.ra_mppi_rollout_variant.argtypes = [vp, C.POINTER(i32)]
     L.ra_mppi_launches_per_step.argtypes = [vp]
     L.ra_mppi_launches_per_step.restype = i32
     L.ra_mppi_last_error.argtypes = [vp]
@@ -265,20 +265,18 @@ def ra_mppi_measure_pipe_peaks(device=0):
     return dict(zip(("ffma", "imad_wide", "lop3", "mufu"), (float(x) for x in out)))
 
 
-def ra_mppi_measure_pipe_model(device=0):
-    """{instruction group: cycles per warp-instruction group per SMSP} (see include/ra_mppi.h)."""
-    out = (C.c_float * 8)()
-    _check(None, load().ra_mppi_measure_pipe_model(int(device), out), "ra_mppi_measure_pipe_model")
-    names = ("ffma_rcc", "ffma_rrr", "fmul_rr", "imad", "shf", "imad_wide+lop3", "imad_wide+lop3+2ffma",
-             "imad_wide+lop3+4ffma")
-    return dict(zip(names, (float(x) for x in out)))
-
-
 def ra_mppi_query_counts(cfg: ra_mppi_config):
     """(k_tail, K0) as ra_mppi_create derives them from the fp32 alpha and eta (host only, no device needed)."""
     k_tail, K0 = C.c_int32(), C.c_int32()
     _check(None, load().ra_mppi_query_counts(C.byref(cfg), C.byref(k_tail), C.byref(K0)), "ra_mppi_query_counts")
     return int(k_tail.value), int(K0.value)
+
+
+def ra_mppi_rollout_variant(ctx):
+    """(dyn, risk, noise variant, slots per lane, half) = the template arguments of the rollout kernel this context launches."""
+    out = (C.c_int32 * 5)()
+    _check(ctx, load().ra_mppi_rollout_variant(ctx, out), "ra_mppi_rollout_variant")
+    return tuple(int(x) for x in out)
 
 
 def ra_mppi_launches_per_step(ctx):

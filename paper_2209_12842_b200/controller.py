@@ -145,5 +145,9 @@ class RaMppi:
         return w
 
     @property
+    def rollout_variant(self):
+        return B.ra_mppi_rollout_variant(self.ctx)
+
+    @property
     def launches_per_step(self):
         return B.ra_mppi_launches_per_step(self.ctx)

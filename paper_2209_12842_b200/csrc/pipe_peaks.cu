@@ -83,43 +83,6 @@ __global__ void __launch_bounds__(kThreads) mufu_kernel(float* out, int iters) {
   if (s == 123.456f) out[0] = s;
 }
 
-// ---- pipe-model probes (profiles/r1c): cost of one warp-instruction per SMSP by operand form and in mixes ----
-// MODE 0 FFMA r,c,c | 1 FFMA r,r,r | 2 FMUL r,r | 3 IMAD (32-bit lo) | 4 SHF | 5 IMAD.WIDE.U32 + LOP3 (Philox round pattern)
-// 6 = 5 plus 2 FFMA r,c,c per wide multiply | 7 = 5 plus 4 FFMA r,c,c per wide multiply
-template <int MODE>
-__global__ void __launch_bounds__(kThreads) probe_kernel(float* out, int iters, float ca, float cb, uint32_t ua) {
-  float x[kChains], y[kChains], z[kChains];
-  uint32_t u[kChains], v[kChains];
-#pragma unroll
-  for (int i = 0; i < kChains; ++i) {
-    x[i] = (float)(threadIdx.x + i); y[i] = 1.0f + 1e-7f * (float)(threadIdx.x + i); z[i] = 1e-9f * (float)(i + 1 + threadIdx.x);
-    u[i] = threadIdx.x * 2654435761u + i; v[i] = u[i] * 7u + 3u;
-  }
-  for (int it = 0; it < iters; ++it) {
-#pragma unroll
-    for (int j = 0; j < 16; ++j)
-#pragma unroll
-      for (int i = 0; i < kChains; ++i) {
-        if (MODE == 0) x[i] = fmaf(x[i], ca, cb);
-        if (MODE == 1) x[i] = fmaf(x[i], y[i], z[i]);
-        if (MODE == 2) x[i] = x[i] * y[i];
-        if (MODE == 3) u[i] = u[i] * ua + v[i];
-        if (MODE == 4) u[i] = __funnelshift_r(u[i], v[i], 9);
-        if (MODE >= 5) {
-          unsigned long long pr;
-          asm volatile("mul.wide.u32 %0, %1, %2;" : "=l"(pr) : "r"(u[i]), "r"(ua));
-          u[i] = (uint32_t)(pr >> 32) ^ (uint32_t)pr ^ v[i];
-          if (MODE >= 6) { x[i] = fmaf(x[i], ca, cb); y[i] = fmaf(y[i], ca, cb); }
-          if (MODE >= 7) { z[i] = fmaf(z[i], ca, cb); x[i] = fmaf(x[i], cb, ca); }
-        }
-      }
-  }
-  float s = 0.f; uint32_t t = 0;
-#pragma unroll
-  for (int i = 0; i < kChains; ++i) { s += x[i] + y[i] + z[i]; t ^= u[i] ^ v[i]; }
-  if (s == 1.2345f || t == 0x12345u) out[0] = s;
-}
-
 template <typename Launch>
 bool time_kernel(Launch launch, double ops_per_launch, float* result) {
   cudaEvent_t a, b;
@@ -162,37 +125,4 @@ extern "C" ra_status ra_mppi_measure_pipe_peaks(int32_t device, float* h_tera_la
   ok = ok && time_kernel([&] { mufu_kernel<<<grid, kThreads>>>(d_out, iters); }, ops, &h_tera_lane_ops[3]);
   cudaFree(d_out);
   return ok ? RA_OK : RA_ECUDA;
-}
-
-extern "C" ra_status ra_mppi_measure_pipe_model(int32_t device, float* h_cycles) {
-  if (!h_cycles) return RA_EINVAL;
-  int n_dev = 0;
-  if (cudaGetDeviceCount(&n_dev) != cudaSuccess || device < 0 || device >= n_dev) return RA_ECUDA;
-  if (cudaSetDevice(device) != cudaSuccess) return RA_ECUDA;
-  cudaDeviceProp prop{};
-  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return RA_ECUDA;
-  int khz = 0;
-  if (cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, device) != cudaSuccess) return RA_ECUDA;
-  float* d_out = nullptr;
-  if (cudaMalloc(&d_out, sizeof(float)) != cudaSuccess) return RA_ENOMEM;
-  const int grid = prop.multiProcessorCount * 3;   // 24 warps per SM, the rollout kernel's occupancy
-  const int iters = 256;
-  // units per launch chosen so that "result" = launches of one (wide-multiply or single) instruction group per second
-  const double groups = (double)grid * kThreads * iters * 16 * kChains;
-  bool ok = true;
-  float rate[8];
-  ok = ok && time_kernel([&] { probe_kernel<0><<<grid, kThreads>>>(d_out, iters, 1.0000001f, 1e-9f, 0xD2511F53u); }, groups, &rate[0]);
-  ok = ok && time_kernel([&] { probe_kernel<1><<<grid, kThreads>>>(d_out, iters, 1.0000001f, 1e-9f, 0xD2511F53u); }, groups, &rate[1]);
-  ok = ok && time_kernel([&] { probe_kernel<2><<<grid, kThreads>>>(d_out, iters, 1.0000001f, 1e-9f, 0xD2511F53u); }, groups, &rate[2]);
-  ok = ok && time_kernel([&] { probe_kernel<3><<<grid, kThreads>>>(d_out, iters, 1.0000001f, 1e-9f, 0xD2511F53u); }, groups, &rate[3]);
-  ok = ok && time_kernel([&] { probe_kernel<4><<<grid, kThreads>>>(d_out, iters, 1.0000001f, 1e-9f, 0xD2511F53u); }, groups, &rate[4]);
-  ok = ok && time_kernel([&] { probe_kernel<5><<<grid, kThreads>>>(d_out, iters, 1.0000001f, 1e-9f, 0xD2511F53u); }, groups, &rate[5]);
-  ok = ok && time_kernel([&] { probe_kernel<6><<<grid, kThreads>>>(d_out, iters, 1.0000001f, 1e-9f, 0xD2511F53u); }, groups, &rate[6]);
-  ok = ok && time_kernel([&] { probe_kernel<7><<<grid, kThreads>>>(d_out, iters, 1.0000001f, 1e-9f, 0xD2511F53u); }, groups, &rate[7]);
-  cudaFree(d_out);
-  if (!ok) return RA_ECUDA;
-  // rate[i] = 1e12 lane-groups/s -> cycles per warp-group per SMSP at the device's maximum SM clock
-  const double smsp_lanes = (double)prop.multiProcessorCount * 4.0 * 32.0;
-  for (int i = 0; i < 8; ++i) h_cycles[i] = (float)(smsp_lanes * (double)khz * 1e3 / ((double)rate[i] * 1e12));
-  return RA_OK;
 }

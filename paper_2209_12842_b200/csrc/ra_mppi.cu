@@ -576,6 +576,13 @@ Params with_iteration(const ra_mppi_ctx* c, uint64_t iteration) {
 
 extern "C" {
 
+ra_status ra_mppi_rollout_variant(const ra_mppi_ctx* c, int32_t* h_variant) {
+  if (!c || !h_variant) return RA_EINVAL;
+  h_variant[0] = c->cfg.dyn; h_variant[1] = c->cfg.risk; h_variant[2] = c->noise_variant;
+  h_variant[3] = c->rc; h_variant[4] = c->half ? 1 : 0;
+  return RA_OK;
+}
+
 ra_status ra_mppi_step(ra_mppi_ctx* c, const float* d_x0, float* d_v, uint64_t iteration, void* stream) {
   if (!c) return RA_EINVAL;
   if (!d_x0 || !d_v) return fail(c, RA_EINVAL, "null device pointer");

@@ -1,11 +1,14 @@
 """Compact per-launch counter table from `ncu --set full` reports of the rollout kernel (roofline accounting of bench.py).
 
-    python -m paper_2209_12842_b200.ncu_counters WORKLOAD=report.ncu-rep [WORKLOAD=report.ncu-rep ...] > profiles/<name>.csv
+    python tests/helpers/ncu_counters.py WORKLOAD=report.ncu-rep [WORKLOAD=report.ncu-rep ...] > profiles/<name>.csv
 
 Runs `ncu -i <report> --page raw --csv` (no GPU needed) for every report, keeps the first profiled launch and the metrics
 below, and prefixes each row with the workload name and its noisy state-steps per launch (K*M*T, from bench.make_problem).
 bench.py reads the table for `roofline.frac_fp32_flop`, `frac_issue`, `pipe_busy` and `traffic`; the instruction counts are
-per launch, so bench.py divides them by the kernel time it measures live.  No arithmetic of the method lives here.
+per launch, so bench.py divides them by the kernel time it measures live.  Every row carries `source_sha`, the hash of the
+rollout kernel's sources at the time the table is written (bench.rollout_source_sha): run this straight after the capture, on
+the tree that was profiled.  bench.py nulls the derived fractions when the hash or the kernel instantiation no longer matches.
+A development tool, not part of the package; no arithmetic of the method lives here.
 """
 from __future__ import annotations
 
@@ -57,15 +60,16 @@ def read_report(path):
 
 
 def main(argv):
-    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__)))))
     import bench
+    sha = bench.rollout_source_sha()
     w = csv.writer(sys.stdout, lineterminator="\n")
-    w.writerow(["workload", "state_steps", "kernel"] + METRICS)
+    w.writerow(["workload", "state_steps", "kernel", "source_sha"] + METRICS)
     for arg in argv:
         name, path = arg.split("=", 1)
         r = read_report(path)
         p = bench.make_problem(name)
-        w.writerow([bench.counter_key(name), p.state_steps, r["kernel"]] + [r[m] for m in METRICS])
+        w.writerow([bench.counter_key(name), p.state_steps, r["kernel"], sha] + [r[m] for m in METRICS])
 
 
 if __name__ == "__main__":

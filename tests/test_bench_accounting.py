@@ -12,7 +12,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 def test_every_workload_has_a_counter_row():
     counters = bench.load_counters()
-    assert counters, "profiles/r2_rollout_counters.csv is missing or empty"
+    assert counters, "profiles/r3_rollout_counters.csv is missing or empty"
     names = ["C0", "C1", "C2", "C3", "PAPER", "PAPER-ST", "C4-K8192-M64"] + \
         [f"C4-K{K}-M{M}" for K in W.C4_SWEEP_K for M in W.C4_SWEEP_M]
     for n in names:
@@ -48,6 +48,28 @@ def test_fractions_follow_their_definitions():
     # no capture -> the contract's fraction only
     f3 = bench.derived_fractions("C3", p.state_steps, kernel_ms, ffma_peak, {})
     assert f3["frac"] == f["frac"] and f3["frac_fp32_flop"] is None and f3["frac_issue"] is None
+
+
+def test_capture_belongs_to_the_sources_in_the_tree(monkeypatch):
+    """The ncu-derived fractions are only reported for the kernel they were captured from: every row of the committed table
+    carries the hash of the rollout sources it was taken on, which must be the hash of the tree; a changed source, or a
+    context that launches another instantiation than the captured one, turns the derived fractions into nulls."""
+    counters = bench.load_counters()
+    sha = bench.rollout_source_sha()
+    for key, row in counters.items():
+        assert row["source_sha"] == sha, f"{key}: the capture is of other sources -- re-capture (profiles/r3_rollout_counters.md)"
+    p = bench.make_problem("C3")
+    assert bench.kernel_template_args(counters["C3"]["kernel"]) == (0, 1, 0, 2, 0)     # bicycle, costmap, Gaussian, 2 slots, whole warp
+    ok = bench.derived_fractions("C3", p.state_steps, 0.35, 35.4, counters, variant=(0, 1, 0, 2, 0))
+    assert ok["capture"] == {"stale": False, "why": [], "extrapolated": False} and ok["frac_issue"] is not None
+    other = bench.derived_fractions("C3", p.state_steps, 0.35, 35.4, counters, variant=(0, 1, 0, 4, 0))
+    assert other["capture"]["stale"] and other["frac_issue"] is None and other["frac_fp32_flop"] is None and other["frac"] == ok["frac"]
+    scaled = bench.derived_fractions("C4-K4096-M64", 4096 * 64 * 50, 0.08, 35.4, counters)
+    assert scaled["capture"]["extrapolated"] and not scaled["capture"]["stale"]
+    monkeypatch.setattr(bench, "rollout_source_sha", lambda: "0" * 64)                 # as if rollout.cuh had been edited
+    touched = bench.derived_fractions("C3", p.state_steps, 0.35, 35.4, counters, variant=(0, 1, 0, 2, 0))
+    assert touched["capture"]["stale"] and "source_sha" in touched["capture"]["why"][0]
+    assert touched["frac_issue"] is None and touched["frac_fp32_flop"] is None
 
 
 def test_algorithmic_op_counts_match_design():
