@@ -99,6 +99,9 @@ typedef struct {
 /* Allocate a controller context on cfg->device.  cfg/env: host.  *out receives the
  * context (NULL on failure).  RA_EINVAL / RA_EUNSUPPORTED / RA_ECUDA / RA_ENOMEM.        */
 ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_mppi_ctx** out);
+/* Why the calling thread's most recent ra_mppi_create failed ("" after a success): there is no context yet whose
+ * ra_mppi_last_error could say it.  Owned by the library, valid until this thread's next create call.            */
+const char* ra_mppi_create_error(void);
 
 /* Replace the environment of an existing context (moving obstacles, a refreshed costmap): env is HOST memory,
  * copied before the call returns.  Up to 1024 circles; a costmap must keep the map_h x map_w it had at create

@@ -53,7 +53,7 @@ class ra_mppi_env(C.Structure):
 
 
 EXPORTS = (
-    "ra_mppi_create", "ra_mppi_set_env", "ra_mppi_step", "ra_mppi_rollout_costs", "ra_mppi_weights_update",
+    "ra_mppi_create", "ra_mppi_create_error", "ra_mppi_set_env", "ra_mppi_step", "ra_mppi_rollout_costs", "ra_mppi_weights_update",
     "ra_mppi_weights_update_static", "ra_mppi_weights_update_static_error",
     "ra_mppi_step_partial", "ra_mppi_combine_partials",
     "ra_mppi_step_host", "ra_mppi_enable_kernel_timing", "ra_mppi_last_rollout_ms",
@@ -81,6 +81,8 @@ def open_library(path):
     L = C.CDLL(path)
     vp, fp, u64, i32 = C.c_void_p, C.c_void_p, C.c_uint64, C.c_int32
     L.ra_mppi_create.argtypes = [C.POINTER(ra_mppi_config), C.POINTER(ra_mppi_env), C.POINTER(vp)]
+    L.ra_mppi_create_error.argtypes = []
+    L.ra_mppi_create_error.restype = C.c_char_p
     L.ra_mppi_set_env.argtypes = [vp, C.POINTER(ra_mppi_env)]
     L.ra_mppi_step.argtypes = [vp, fp, fp, u64, vp]
     L.ra_mppi_rollout_costs.argtypes = [vp, fp, fp, u64, fp, fp, fp, fp, fp, fp, vp]
@@ -108,7 +110,7 @@ def open_library(path):
     L.ra_mppi_last_error.restype = C.c_char_p
     L.ra_mppi_destroy.argtypes = [vp]
     for name in EXPORTS:
-        if name not in ("ra_mppi_launches_per_step", "ra_mppi_last_error", "ra_mppi_weights_update_static_error"):
+        if name not in ("ra_mppi_launches_per_step", "ra_mppi_last_error", "ra_mppi_weights_update_static_error", "ra_mppi_create_error"):
             getattr(L, name).restype = C.c_int
     return L
 
@@ -170,7 +172,9 @@ def _check(ctx, st, where):
 def ra_mppi_create(cfg: ra_mppi_config, env: ra_mppi_env):
     ctx = C.c_void_p()
     st = load().ra_mppi_create(C.byref(cfg), C.byref(env), C.byref(ctx))
-    _check(None, st, "ra_mppi_create")
+    if st != RA_OK:
+        why = load().ra_mppi_create_error()
+        raise RaMppiError(st, "ra_mppi_create", why.decode() if why else "")
     return ctx
 
 

@@ -32,6 +32,17 @@ def _sources():
 LIB_CHECKED = os.path.join(HERE, "libra_mppi_checked.so")
 
 
+def source_hash(jobs) -> str:
+    """sha256 over every source and header of the library, the compiler flags and the per-object defines."""
+    import hashlib
+    h = hashlib.sha256()
+    for path in _sources():
+        with open(path, "rb") as f:
+            h.update(os.path.basename(path).encode() + b"\0" + f.read() + b"\0")
+    h.update(repr((NVCC_FLAGS[:-2], [(os.path.basename(s), os.path.basename(o), d) for s, o, d in jobs])).encode())
+    return h.hexdigest()
+
+
 def _jobs(obj_dir, defs0):
     jobs = [(os.path.join(CSRC, "ra_mppi.cu"), os.path.join(obj_dir, "ra_mppi.o"), list(defs0)),
             (os.path.join(CSRC, "pipe_peaks.cu"), os.path.join(obj_dir, "pipe_peaks.o"), list(defs0))]
@@ -46,9 +57,13 @@ def build(force: bool = False, verbose: bool = False, checked: bool = False) -> 
     lib = LIB_CHECKED if checked else LIB
     obj_dir = OBJ + "_checked" if checked else OBJ
     jobs = _jobs(obj_dir, ["-DRA_CHECKED"] if checked else [])
-    newest = max(os.path.getmtime(s) for s in _sources() + [os.path.abspath(__file__)])
-    if not force and os.path.exists(lib) and os.path.getmtime(lib) >= newest:
+    # up to date = the stamp written beside the library by the build that produced it names these very sources and flags
+    # (a content hash, not mtimes: a snapshot copied to the GPU box keeps the prebuilt library only if it is of this source)
+    stamp, want = lib + ".sha256", source_hash(jobs)
+    if not force and os.path.exists(lib) and os.path.exists(stamp) and open(stamp).read().strip() == want:
         return lib
+    if os.path.exists(stamp):
+        os.remove(stamp)
     os.makedirs(obj_dir, exist_ok=True)
     extra = ["-Xptxas", "-v"] if verbose else []
 
@@ -68,6 +83,8 @@ def build(force: bool = False, verbose: bool = False, checked: bool = False) -> 
     objs = [j[1] for j in jobs]
     cmd = ["nvcc", "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", lib, *objs, "-lcudart"]
     subprocess.run(cmd, check=True)
+    with open(stamp, "w") as f:
+        f.write(want + "\n")
     return lib
 
 

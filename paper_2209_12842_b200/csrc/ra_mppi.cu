@@ -259,34 +259,46 @@ ra_status upload_env(ra_mppi_ctx* c, const ra_mppi_env* env, bool first) {
 
 }  // namespace
 
+// Why the calling thread's last ra_mppi_create failed: there is no context yet to hold the text (ra_mppi_create_error).
+namespace {
+thread_local char g_create_error[256] = "";
+ra_status create_fail(ra_status st, const char* fmt, int a = 0, int b = 0) {
+  std::snprintf(g_create_error, sizeof g_create_error, fmt, a, b);
+  return st;
+}
+}  // namespace
+
 extern "C" {
 
+const char* ra_mppi_create_error(void) { return g_create_error; }
+
 ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_mppi_ctx** out) {
-  if (!out) return RA_EINVAL;
+  g_create_error[0] = '\0';
+  if (!out) return create_fail(RA_EINVAL, "null output pointer");
   *out = nullptr;
-  if (!cfg) return RA_EINVAL;
+  if (!cfg) return create_fail(RA_EINVAL, "null config");
   ra_status st;
   if (const char* why = validate(cfg, env, &st)) {
-    std::fprintf(stderr, "ra_mppi_create: %s\n", why);
+    std::snprintf(g_create_error, sizeof g_create_error, "%s", why);
     return st;
   }
   int n_dev = 0;
-  if (cudaGetDeviceCount(&n_dev) != cudaSuccess || cfg->device < 0 || cfg->device >= n_dev) {
-    std::fprintf(stderr, "ra_mppi_create: no CUDA device %d (this library has no CPU fallback)\n", cfg->device);
-    return RA_ECUDA;
-  }
+  if (cudaGetDeviceCount(&n_dev) != cudaSuccess || cfg->device < 0 || cfg->device >= n_dev)
+    return create_fail(RA_ECUDA, "no CUDA device %d (this library has no CPU fallback)", cfg->device);
   cudaDeviceProp prop{};
-  if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess) return RA_ECUDA;
-  if (prop.major != 10) {
-    std::fprintf(stderr, "ra_mppi_create: device is sm_%d%d, built for sm_100a only\n", prop.major, prop.minor);
-    return RA_EUNSUPPORTED;
-  }
+  if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess) return create_fail(RA_ECUDA, "cudaGetDeviceProperties failed");
+  if (prop.major != 10) return create_fail(RA_EUNSUPPORTED, "device is sm_%d%d, built for sm_100a only", prop.major, prop.minor);
   ra_mppi_ctx* c = new (std::nothrow) ra_mppi_ctx();
-  if (!c) return RA_ENOMEM;
+  if (!c) return create_fail(RA_ENOMEM, "out of host memory");
   c->cfg = *cfg;
-  auto bail = [&](ra_status s) { ra_mppi_destroy(c); return s; };
+  // the context's own error text (set by upload_env and the CUDA wrappers) outlives it in the thread's create-error slot
+  auto bail = [&](ra_status s, const char* what = "") {
+    std::snprintf(g_create_error, sizeof g_create_error, "%s%s%s", what, (what[0] && !c->err.empty()) ? ": " : "", c->err.c_str());
+    ra_mppi_destroy(c);
+    return s;
+  };
   DeviceGuard on_device(cfg->device);   // the caller's current device is restored on return
-  if (!on_device.ok) return bail(RA_ECUDA);
+  if (!on_device.ok) return bail(RA_ECUDA, "cudaSetDevice failed");
   c->n_sm = prop.multiProcessorCount;
 
   Params& p = c->p;
@@ -370,7 +382,7 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
   c->rollout = pick_rollout(cfg->dyn, cfg->risk);
 
   // environment copies (buffers sized once; ra_mppi_set_env refills them)
-  if (ra_status st_env = upload_env(c, env, true)) return bail(st_env);
+  if (ra_status st_env = upload_env(c, env, true)) return bail(st_env, "environment");
   // scratch
   const size_t KT = (size_t)cfg->K * cfg->T;
   if (dev_alloc(&c->d_u_raw, KT) != cudaSuccess || dev_alloc(&c->d_ce, KT) != cudaSuccess ||
@@ -379,20 +391,20 @@ ra_status ra_mppi_create(const ra_mppi_config* cfg, const ra_mppi_env* env, ra_m
       dev_alloc(&c->d_done, 1) != cudaSuccess ||
       dev_alloc(&c->d_stage, (size_t)(8 + 2 * cfg->T)) != cudaSuccess ||
       cudaHostAlloc(reinterpret_cast<void**>(&c->h_stage), (size_t)(8 + 2 * cfg->T) * sizeof(float), cudaHostAllocDefault) != cudaSuccess)
-    return bail(RA_ENOMEM);
+    return bail(RA_ENOMEM, "device or pinned-host allocation of the context scratch failed");
   p.u_raw = c->d_u_raw; p.ce = c->d_ce; p.S = c->d_S; p.cvar = c->d_cvar; p.pen = c->d_pen;
   if (cudaMemset(c->d_loop, 0, sizeof(LoopState)) != cudaSuccess || cudaMemset(c->d_done, 0, sizeof(unsigned int)) != cudaSuccess ||
       cudaMemset(c->d_cvar, 0, (size_t)cfg->K * sizeof(float)) != cudaSuccess ||
       cudaMemset(c->d_pen, 0, (size_t)cfg->K * sizeof(double)) != cudaSuccess)   // A = 0 steps never write them
-    return bail(RA_ECUDA);
+    return bail(RA_ECUDA, "cudaMemset of the context scratch failed");
   if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
       cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess)
-    return bail(RA_ECUDA);
+    return bail(RA_ECUDA, "side stream / event creation failed");
   p.M_pad = p.R_total * p.G;
   if (cfg->noise_mode == RA_NOISE_MATERIALISED) {
     const size_t n = KT * (size_t)p.nx * (size_t)p.M_pad;
-    if (dev_alloc(&c->d_w_mat, n) != cudaSuccess) return bail(RA_ENOMEM);
+    if (dev_alloc(&c->d_w_mat, n) != cudaSuccess) return bail(RA_ENOMEM, "device allocation of the materialised noise tensor failed");
     p.w_mat = c->d_w_mat;
   }
   p.d_iter = nullptr; p.iter_imm = 0;

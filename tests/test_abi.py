@@ -53,6 +53,29 @@ def test_invalid_config_is_einval(lib, field, value):
     assert e.value.status == B.RA_EINVAL
 
 
+def test_create_says_why_it_failed(lib):
+    """A caller behind the C ABI gets the reason, not just a status code: ra_mppi_create_error, per calling thread."""
+    p = W.config0()
+    cfg, (env, keep) = B.make_config(p), B.make_env(p)
+    cfg.alpha = 1.5
+    ctx = C.c_void_p()
+    assert lib.ra_mppi_create(C.byref(cfg), C.byref(env), C.byref(ctx)) == B.RA_EINVAL and not ctx.value
+    assert b"alpha" in lib.ra_mppi_create_error()
+    with pytest.raises(B.RaMppiError) as e:
+        B.ra_mppi_create(cfg, env)
+    assert "alpha" in str(e.value)
+    cfg = B.make_config(p)
+    cfg.M = 513
+    with pytest.raises(B.RaMppiError) as e:
+        B.ra_mppi_create(cfg, env)
+    assert e.value.status == B.RA_EUNSUPPORTED and "M" in str(e.value).replace("RA_EUNSUPPORTED", "").replace("ra_mppi", "")
+    import torch
+    if not torch.cuda.is_available():
+        with pytest.raises(B.RaMppiError) as e:
+            B.ra_mppi_create(B.make_config(p), env)
+        assert "no CUDA device" in str(e.value) and "no CPU fallback" in str(e.value)
+
+
 def test_unsupported_sizes(lib):
     p = W.config0()
     for field, value in (("M", 513), ("T", 129)):
