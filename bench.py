@@ -285,6 +285,8 @@ def run_cuda(args):
     pipe_peaks = B.ra_mppi_measure_pipe_peaks(local)   # measured FFMA / IMAD.WIDE+LOP3 / LOP3 / MUFU rates
 
     p = make_problem(args.workload, rank)
+    if args.materialised:   # the HBM-bound variant: the noise tensor written by the generator, streamed by the rollout kernel
+        p = p.replace(noise_mode=W.NOISE_MATERIALISED)
     ctl = RaMppi(p, device=local)
     dev = ctl.device
     d_x0 = ctl.tensor(p.x0)
@@ -372,7 +374,7 @@ def run_cuda(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"{p.name} K={p.K} M={p.M} T={p.T}", "baseline_config_index": int(key[1]) if key[1:].isdigit() else None,
                        "l2_flush_between_steps": True, "parallelism": "replicas only" if world > 1 else "single GPU",
-                       "noise_mode": "fused"},
+                       "noise_mode": "materialised" if args.materialised else "fused"},
             "iterations_per_s": world * args.steps / (total_ms * 1e-3),
             "wall_ms_per_step_incl_flush": 1e3 * t_wall / args.steps,
             "clocks": sampler.summary(),
@@ -582,10 +584,24 @@ def run_workloads(ffma_peak, counters, flush=None, with_cpu=False):
     # the write side: the generator fills the same tensor once per step.  Its time is the step minus the rollout kernel, which
     # also contains the sampling, nominal-rollout and update kernels (about 0.03 ms here), so the rate is a lower bound
     gen_ms = r["ms_per_step"] - r["rollout_kernel_ms"]
+    # a write-only stream does not reach the copy peak (which counts bytes read + bytes written): the ceiling of a kernel that
+    # only writes is measured here with a plain device fill of a buffer larger than L2
+    fill = flush if flush is not None else torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    for _ in range(3):
+        fill.zero_()
+    ev[0].record()
+    for _ in range(10):
+        fill.zero_()
+    ev[1].record()
+    ev[1].synchronize()
+    write_peak = fill.numel() * 10 / (ev[0].elapsed_time(ev[1]) * 1e-3) / 1e9
     r.update({"generator_ms_upper_bound": gen_ms, "generator_write_GBps": noise_bytes / (gen_ms * 1e-3) / 1e9,
               "generator_frac": noise_bytes / (gen_ms * 1e-3) / 1e9 / hbm_peak,
+              "hbm_write_only_GBps": write_peak, "generator_frac_of_write_only": noise_bytes / (gen_ms * 1e-3) / 1e9 / write_peak,
               "generator_note": "materialise_noise_kernel writes the tensor once per step: bytes / (step - rollout kernel) / HBM copy peak; "
-                                "a lower bound (the difference also holds the three small kernels)"})
+                                "a lower bound (the difference also holds the three small kernels).  hbm_write_only_GBps = a device fill of 256 MB timed in this run: "
+                                "the ceiling of a write-only stream, about 0.6 of the copy peak"})
     out.append(r)
     # closed loop: config 4, K=8192, M=64, 500 receding-horizon iterations replayed from one CUDA graph
     name = "C4-K8192-M64"
@@ -636,6 +652,8 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-workloads", action="store_true", help="leave the per-workload array out of the line (short profiling runs)")
+    ap.add_argument("--materialised", action="store_true",
+                    help="time the materialised-noise (HBM-bound) variant of the workload instead of the fused one")
     ap.add_argument("--sharded", action="store_true",
                     help="one controller, K split over the ranks (strong scaling) instead of N independent replicas")
     args = ap.parse_args()

@@ -331,22 +331,52 @@ __global__ void noise_probe_kernel(const __grid_constant__ Params p, const int* 
 }
 
 // Materialised-noise generator: w[K][T][NX][M_pad] = sigma_w (.) z, the same draws the fused
-// kernel makes in registers (HBM-roofline mode of BASELINE.json).
+// kernel makes in registers (HBM-roofline mode of BASELINE.json).  A streaming kernel: consecutive threads take
+// consecutive m, so every row of M_pad floats is written in full 128-byte lines.  Where a Philox call serves two
+// steps (two words per step: n_x = 4, Gaussian or uniform) a thread owns one CALL and writes both steps' rows, so no
+// call is computed twice and half discarded (round 2 did: one thread per (k, t, m) through state_noise).
 template <int NX, int NOISE>
 __global__ void __launch_bounds__(256) materialise_noise_kernel(const __grid_constant__ Params p,
                                                                 float* __restrict__ w) {
-  const long long n = (long long)p.K * p.T * p.M_pad;
   const uint32_t c3 = iteration_field(p, STREAM_W);
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n;
-       i += (long long)gridDim.x * blockDim.x) {
-    const int m = (int)(i % p.M_pad);
-    const long long kt = i / p.M_pad;
-    const int t = (int)(kt % p.T), k = (int)(kt / p.T);
-    float z[NX];
-    state_noise<NX, NOISE>(p, (uint32_t)(k + p.k_off), (uint32_t)m, (uint32_t)t, c3, z);
-    float* o = w + (size_t)kt * NX * p.M_pad + m;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  const long long i0 = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  const size_t step_floats = (size_t)NX * p.M_pad;
+  if constexpr (NoiseWords<NX, NOISE>::value == 2) {
+    const int TP = (p.T + 1) / 2;                      // Philox calls per realisation: steps (2 tp, 2 tp + 1)
+    const long long n = (long long)p.K * TP * p.M_pad;
+    for (long long i = i0; i < n; i += stride) {
+      const int m = (int)(i % p.M_pad);
+      const long long ktp = i / p.M_pad;
+      const int tp = (int)(ktp % TP), k = (int)(ktp / TP), t = 2 * tp;
+      const uint4 q = philox4x32_10((uint32_t)(k + p.k_off), (uint32_t)m, (uint32_t)tp, c3, p.rk);
+      RA_DEVICE_CHECK(k < p.K && t < p.T && m < p.M_pad);
+      float* o = w + ((size_t)k * p.T + t) * step_floats + m;
+      float z[NX];
+      const uint32_t w0[2] = {q.x, q.y};
+      noise_from_words<NX, NOISE>(p, w0, z);
 #pragma unroll
-    for (int j = 0; j < NX; ++j) o[(size_t)j * p.M_pad] = z[j] * p.wscale[j];
+      for (int j = 0; j < NX; ++j) __stcs(o + (size_t)j * p.M_pad, z[j] * p.wscale[j]);
+      if (t + 1 < p.T) {                               // an odd horizon ends on the first half of its last call
+        const uint32_t w1[2] = {q.z, q.w};
+        noise_from_words<NX, NOISE>(p, w1, z);
+        o += step_floats;
+#pragma unroll
+        for (int j = 0; j < NX; ++j) __stcs(o + (size_t)j * p.M_pad, z[j] * p.wscale[j]);
+      }
+    }
+  } else {
+    const long long n = (long long)p.K * p.T * p.M_pad;
+    for (long long i = i0; i < n; i += stride) {
+      const int m = (int)(i % p.M_pad);
+      const long long kt = i / p.M_pad;
+      const int t = (int)(kt % p.T), k = (int)(kt / p.T);
+      float z[NX];
+      state_noise<NX, NOISE>(p, (uint32_t)(k + p.k_off), (uint32_t)m, (uint32_t)t, c3, z);
+      float* o = w + (size_t)kt * step_floats + m;
+#pragma unroll
+      for (int j = 0; j < NX; ++j) o[(size_t)j * p.M_pad] = z[j] * p.wscale[j];
+    }
   }
 }
 

@@ -198,7 +198,10 @@ def test_materialised_noise_equals_fused(torch_cuda):
     # M = 96 / 160: three / five slots of 32 realisations with two interleaved per lane, so the last group carries one
     # slot past the end (its loads must stay inside the noise tensor: ADVICE r1)
     for p in (_with_v(W.small(W.config3(), K=65, M=128, T=10)), _with_v(W.small(W.config2(), K=20, M=50, T=8)),
-              _with_v(W.small(W.config1(), K=33, M=96, T=12)), _with_v(W.small(W.config2(), K=9, M=160, T=7))):
+              _with_v(W.small(W.config1(), K=33, M=96, T=13)), _with_v(W.small(W.config2(), K=9, M=160, T=7)),
+              # odd horizons with two words per step: the generator's last Philox call serves one step only
+              _with_v(W.small(W.config3(), K=7, M=32, T=5)).replace(noise_kind=W.NOISE_UNIFORM, sigma_w=[0.2] * 4),
+              _with_v(W.small(W.config0(near_obstacle=True), K=300, M=16, T=1))):
         a = gpu_outputs(_ctl(p), p)
         b = gpu_outputs(_ctl(p.replace(noise_mode=W.NOISE_MATERIALISED)), p)
         # same draws; the fused kernel contracts sigma*z + x into one FMA, so equality is to rounding
